@@ -1,0 +1,187 @@
+"""ctypes binding of the serial C++ oracle (oracle/sdm_oracle.cpp).
+
+TEST INFRASTRUCTURE ONLY: importable from tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  The product package (paper_2103_17238_b200) never
+imports this module, and this module never imports the product package.
+
+All arrays are numpy host arrays; `coalescence_step` updates `xi` and `v` in place.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import importlib.util
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _load():
+    spec = importlib.util.spec_from_file_location("_oracle_build", os.path.join(_HERE, "build.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return C.CDLL(mod.build())
+
+
+class KernelParams(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("_pad", C.c_int32), ("b", C.c_double), ("E", C.c_double)]
+
+
+GOLOVIN = 0
+GEOMETRIC = 1
+
+_lib = _load()
+
+_i64p = np.ctypeslib.ndpointer(np.int64, flags="C_CONTIGUOUS")
+_f64p = np.ctypeslib.ndpointer(np.float64, flags="C_CONTIGUOUS")
+_i32p = np.ctypeslib.ndpointer(np.int32, flags="C_CONTIGUOUS")
+_u32p = np.ctypeslib.ndpointer(np.uint32, flags="C_CONTIGUOUS")
+
+_lib.oracle_philox4x32_10.argtypes = [_u32p, _u32p, _u32p]
+_lib.oracle_philox4x32_10.restype = None
+_lib.oracle_uniform_from_words.argtypes = [C.c_uint32, C.c_uint32]
+_lib.oracle_uniform_from_words.restype = C.c_double
+_lib.oracle_sd_random.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.POINTER(C.c_uint32), C.POINTER(C.c_double)]
+_lib.oracle_sd_random.restype = None
+_lib.oracle_sd_random_batch.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_int64, _u32p, _f64p]
+_lib.oracle_sd_random_batch.restype = None
+_lib.oracle_det_cbrt.argtypes = [C.c_double]
+_lib.oracle_det_cbrt.restype = C.c_double
+_lib.oracle_terminal_velocity.argtypes = [C.c_double]
+_lib.oracle_terminal_velocity.restype = C.c_double
+_lib.oracle_radius.argtypes = [C.c_double]
+_lib.oracle_radius.restype = C.c_double
+_lib.oracle_kernel.argtypes = [C.POINTER(KernelParams), C.c_double, C.c_double]
+_lib.oracle_kernel.restype = C.c_double
+_lib.oracle_gamma_from_p.argtypes = [C.c_double, C.c_double]
+_lib.oracle_gamma_from_p.restype = C.c_int64
+_lib.oracle_pair_update.argtypes = [C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_double),
+                                    C.POINTER(C.c_double), C.c_int64]
+_lib.oracle_pair_update.restype = C.c_int64
+_lib.oracle_coalescence_step.argtypes = [
+    _i64p, _f64p, _i32p, C.c_int64, C.c_int32, C.c_double, C.c_double, C.POINTER(KernelParams),
+    C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.oracle_coalescence_step.restype = C.c_int
+_lib.oracle_remove_zero_multiplicity.argtypes = [_i64p, _f64p, _i32p, C.c_int64]
+_lib.oracle_remove_zero_multiplicity.restype = C.c_int64
+_lib.oracle_cell_stats.argtypes = [_i64p, _f64p, _i32p, C.c_int64, C.c_int32, _i32p, _i64p, _f64p, _f64p]
+_lib.oracle_cell_stats.restype = C.c_int
+_lib.oracle_total_xi_v_int128.argtypes = [_i64p, _f64p, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_uint64)]
+_lib.oracle_total_xi_v_int128.restype = None
+_lib.oracle_run.argtypes = [_i64p, _f64p, _i32p, C.c_int64, C.c_int32, C.c_double, C.c_double,
+                            C.POINTER(KernelParams), C.c_uint64, C.c_uint64, C.c_int64, C.c_int64]
+_lib.oracle_run.restype = C.c_int64
+
+
+def kernel_params(kind: int, b: float = 0.0, E: float = 1.0) -> KernelParams:
+    return KernelParams(kind=kind, _pad=0, b=b, E=E)
+
+
+def golovin(b: float) -> KernelParams:
+    return kernel_params(GOLOVIN, b=b, E=0.0)
+
+
+def geometric(E: float = 1.0) -> KernelParams:
+    return kernel_params(GEOMETRIC, b=0.0, E=E)
+
+
+def philox4x32_10(ctr, key) -> np.ndarray:
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32)
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.zeros(4, dtype=np.uint32)
+    _lib.oracle_philox4x32_10(ctr, key, out)
+    return out
+
+
+def uniform_from_words(w2: int, w3: int) -> float:
+    return float(_lib.oracle_uniform_from_words(w2, w3))
+
+
+def sd_random(seed: int, step: int, i: int):
+    k = C.c_uint32()
+    u = C.c_double()
+    _lib.oracle_sd_random(seed, step, i, C.byref(k), C.byref(u))
+    return int(k.value), float(u.value)
+
+
+def sd_random_batch(seed: int, step: int, i0: int, n: int):
+    keys = np.zeros(n, np.uint32)
+    us = np.zeros(n, np.float64)
+    _lib.oracle_sd_random_batch(seed, step, i0, n, keys, us)
+    return keys, us
+
+
+def det_cbrt(x: float) -> float:
+    return float(_lib.oracle_det_cbrt(x))
+
+
+def terminal_velocity(r: float) -> float:
+    return float(_lib.oracle_terminal_velocity(r))
+
+
+def radius(v: float) -> float:
+    return float(_lib.oracle_radius(v))
+
+
+def kernel(kp: KernelParams, vj: float, vk: float) -> float:
+    return float(_lib.oracle_kernel(C.byref(kp), vj, vk))
+
+
+def gamma_from_p(p: float, u: float) -> int:
+    return int(_lib.oracle_gamma_from_p(p, u))
+
+
+def pair_update(xi_j: int, xi_k: int, v_j: float, v_k: float, g: int):
+    a, b = C.c_int64(xi_j), C.c_int64(xi_k)
+    c, d = C.c_double(v_j), C.c_double(v_k)
+    gt = _lib.oracle_pair_update(C.byref(a), C.byref(b), C.byref(c), C.byref(d), g)
+    return int(gt), int(a.value), int(b.value), float(c.value), float(d.value)
+
+
+def coalescence_step(xi, v, cell_id, n_cell, dt, dV, kp, seed, step, n_sd=None, debug=False):
+    """One step, in place.  With debug=True returns dict(perm, gamma, gamma_clamped, cell_start)."""
+    n = int(len(xi) if n_sd is None else n_sd)
+    out = None
+    ptrs = [None, None, None, None]
+    if debug:
+        out = dict(perm=np.zeros(n, np.int32), gamma=np.zeros(n, np.int64),
+                   gamma_clamped=np.zeros(n, np.int64), cell_start=np.zeros(n_cell + 1, np.int32))
+        ptrs = [out[k].ctypes.data for k in ("perm", "gamma", "gamma_clamped", "cell_start")]
+    rc = _lib.oracle_coalescence_step(xi, v, cell_id, n, n_cell, dt, dV, C.byref(kp), seed, step, *ptrs)
+    if rc != 0:
+        raise ValueError(f"oracle_coalescence_step failed: {rc}")
+    return out
+
+
+def remove_zero_multiplicity(xi, v, cell_id, n_sd=None) -> int:
+    n = int(len(xi) if n_sd is None else n_sd)
+    return int(_lib.oracle_remove_zero_multiplicity(xi, v, cell_id, n))
+
+
+def cell_stats(xi, v, cell_id, n_cell, n_sd=None):
+    n = int(len(xi) if n_sd is None else n_sd)
+    count = np.zeros(n_cell, np.int32)
+    sum_xi = np.zeros(n_cell, np.int64)
+    sum_xi_v = np.zeros(n_cell, np.float64)
+    sum_xi_v2 = np.zeros(n_cell, np.float64)
+    rc = _lib.oracle_cell_stats(xi, v, cell_id, n, n_cell, count, sum_xi, sum_xi_v, sum_xi_v2)
+    if rc != 0:
+        raise ValueError(f"oracle_cell_stats failed: {rc}")
+    return count, sum_xi, sum_xi_v, sum_xi_v2
+
+
+def total_xi_v_exact(xi, v, n_sd=None) -> int:
+    """Exact sum of xi*v for integer-valued v, as a Python int (128-bit accumulate)."""
+    n = int(len(xi) if n_sd is None else n_sd)
+    hi, lo = C.c_int64(), C.c_uint64()
+    _lib.oracle_total_xi_v_int128(xi, v, n, C.byref(hi), C.byref(lo))
+    return (int(hi.value) << 64) | int(lo.value)
+
+
+def run(xi, v, cell_id, n_cell, dt, dV, kp, seed, step0, n_steps, compact_every=0, n_sd=None) -> int:
+    n = int(len(xi) if n_sd is None else n_sd)
+    r = int(_lib.oracle_run(xi, v, cell_id, n, n_cell, dt, dV, C.byref(kp), seed, step0, n_steps, compact_every))
+    if r < 0:
+        raise ValueError(f"oracle_run failed: {r}")
+    return r
