@@ -1,0 +1,165 @@
+/* sdm.h -- C ABI of the B200-native Super-Droplet Method (SDM) coalescence step.
+ *
+ * What it computes: one Monte-Carlo collisional-growth step of the Super-Droplet Method
+ * ("SDM Monte-Carlo algorithm for representing collisional growth (Shima et al., 2009)",
+ * /root/reference/PAPER.md:15 Introduction; reference entry PAPER.md:188) on super-droplets
+ * carrying the attributes `volume` and `n` = multiplicity, in an environment
+ * that supplies the time step `dt` and the cell volume `dv`, with a coalescence
+ * kernel object (PAPER.md:66, 75 Golovin; PAPER.md:96 geometric sweep-out).  The statement of
+ * each operation is BASELINE.json `north_star` (a)-(d) as read in SURVEY.md section 8(c) and
+ * DESIGN.md "Readings".
+ *
+ * Conventions (apply to every call unless stated otherwise)
+ *  - Array arguments are DEVICE pointers owned by the caller; scalars are passed by value.
+ *    Pointers marked "host" are host pointers.  The library never allocates device memory: the
+ *    caller hands it a workspace of sdm_workspace_bytes() bytes at sdm_init().
+ *  - Structure-of-arrays state: multiplicity int64[n_sd], volume fp64[n_sd] (m^3), cell_id
+ *    int32[n_sd] in [0, n_cell).  8-byte arrays must be 16-byte aligned (cudaMalloc / torch are).
+ *  - All work is enqueued on the cudaStream_t given to sdm_init(); calls are asynchronous unless
+ *    they return a value to the host (documented per call).
+ *  - Errors: every entry point returns an sdm_status (0 = SDM_OK, negative = error).  Nothing is
+ *    printed, nothing throws.  Misuse visible on the host -> SDM_ERR_INVALID_ARG / SDM_ERR_CAPACITY
+ *    before any kernel is launched.  Data errors only visible on the device (cell_id outside
+ *    [0, n_cell), multiplicity < 0) set a sticky flag reported by sdm_poll_error() and by the next
+ *    synchronising call as SDM_ERR_BAD_DATA; the step stays memory-safe but its output is then
+ *    unspecified.
+ *  - There is no CPU fallback: without a CUDA device sdm_init() returns SDM_ERR_CUDA.
+ */
+#ifndef SDM_B200_H_
+#define SDM_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sdm_ctx sdm_ctx; /* opaque, host memory, freed by sdm_destroy() */
+
+typedef enum {
+    SDM_OK = 0,
+    SDM_ERR_INVALID_ARG = -1,
+    SDM_ERR_CAPACITY = -2,
+    SDM_ERR_CUDA = -3,
+    SDM_ERR_BAD_DATA = -4
+} sdm_status;
+
+typedef enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GEOMETRIC = 1 } sdm_kernel_kind;
+
+/* Coalescence kernel K(v_j, v_k) [m^3 s^-1] (north_star (c)):
+ *   Golovin:  K = b (v_j + v_k), b in s^-1, volumes in m^3.
+ *   geometric:     K = E pi (r_j + r_k)^2 |v_t(r_j) - v_t(r_k)|, r = cbrt(3 v / 4 pi),
+ *                                v_t a three-regime power law (R16). */
+typedef struct {
+    int32_t kind; /* sdm_kernel_kind */
+    int32_t _pad;
+    double b; /* Golovin coefficient, >= 0 */
+    double E; /* geometric collision efficiency, >= 0 (configs use 1.0) */
+} sdm_kernel_params;
+
+/* Path selection for sdm_coalescence_step (sdm_set_path).  Every path produces the same bits. */
+typedef enum {
+    SDM_PATH_AUTO = 0,    /* pick by size / cell ordering (default) */
+    SDM_PATH_GENERAL = 1, /* global LSD radix sort of (cell_id, Philox key): north_star (b) */
+    SDM_PATH_CELL_SORTED = 2 /* per-cell shared-memory sort, only legal when cell_id is non-decreasing;
+                                falls back to GENERAL (same result) when it is not */
+} sdm_path;
+
+/* Bytes of device workspace sdm_init() needs for problems up to (max_n_sd, max_n_cell).
+ * Returns 0 when the arguments are invalid (max_n_sd < 0, max_n_sd >= 2^30, max_n_cell < 1). */
+size_t sdm_workspace_bytes(int64_t max_n_sd, int32_t max_n_cell);
+
+/* Create a context bound to `device`, the caller's workspace and the caller's stream.
+ *   out            host: receives the context
+ *   workspace_dev  device memory, >= sdm_workspace_bytes(max_n_sd, max_n_cell), 256-byte aligned,
+ *                  owned by the caller and kept alive until sdm_destroy()
+ *   cuda_stream    a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); 0 = default stream
+ * Launches no kernel except one memset of the workspace header.
+ * Errors: INVALID_ARG (null out/workspace, bad sizes), CAPACITY (workspace too small), CUDA. */
+int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, void* workspace_dev,
+             size_t workspace_bytes, void* cuda_stream);
+
+/* One SDM coalescence step (north_star (a)-(c)):
+ *   a1  per super-droplet i one Philox-4x32-10 block, counter {lo(i),hi(i),lo(step),hi(step)},
+ *       key {lo(seed),hi(seed)}: word 0 = permutation key, words 3:2 -> 53-bit uniform;
+ *   a2  per-cell counts and their exclusive scan;
+ *   a3  stable ascending sort of indices by (cell_id << 32 | key): the per-cell random shuffle;
+ *   a4  neighbours (2a, 2a+1) of each cell's shuffled run form pairs; for a pair with xi_j >= xi_k
+ *       p = K(v_j,v_k) xi_j (dt/dV) (n_c(n_c-1)/2)/floor(n_c/2); gamma = floor(p) + [u < p - floor(p)];
+ *       gamma~ = min(gamma, floor(xi_j/xi_k)); xi_j -= gamma~ xi_k, v_k += gamma~ v_j, and when xi_j
+ *       reaches 0 the pair splits: xi_j = floor(xi_k/2), xi_k -= floor(xi_k/2), both get the new volume.
+ * multiplicity and volume are updated IN PLACE at the original indices; cell_id is read-only; super-
+ * droplets are never reordered.  Asynchronous.  (seed, step, array index) fully determine the random
+ * numbers, so a run can be resumed bit-exactly.  n_sd == 0 is a no-op.
+ * Errors: INVALID_ARG (null pointers, n_sd < 0, n_cell < 1, dt <= 0, dV <= 0, non-finite dt/dV,
+ * unknown kernel kind, b < 0 or E < 0), CAPACITY (n_sd > max_n_sd, n_cell > max_n_cell), CUDA. */
+int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, const int32_t* cell_id,
+                         int64_t n_sd, int32_t n_cell, double dt, double dV,
+                         const sdm_kernel_params* kp, uint64_t seed, uint64_t step);
+
+/* Stable stream compaction (north_star (d)): removes every entry whose
+ * multiplicity is 0 from (multiplicity, volume, cell_id), in place; survivors keep their relative
+ * order (required: the Philox counter is the array index).  The prefix [0, *n_sd_out) is the result,
+ * the tail is unspecified.  Writes *n_sd_out on the HOST and therefore synchronises the stream; also
+ * reports a pending SDM_ERR_BAD_DATA. */
+int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* volume, int32_t* cell_id,
+                                 int64_t n_sd, int64_t* n_sd_out /* host */);
+
+/* Per-cell statistics: count[c], sum xi, sum xi*v, sum xi*v*v over the
+ * super-droplets of each cell.  Each output is a device array of length n_cell, or NULL to skip it.
+ * Integer outputs are exact; the fp64 sums are accumulated in an unspecified order (compare at
+ * 1e-12 relative).  Asynchronous. */
+int sdm_cell_stats(sdm_ctx* ctx, const int64_t* multiplicity, const double* volume,
+                   const int32_t* cell_id, int64_t n_sd, int32_t n_cell, int32_t* count,
+                   int64_t* sum_xi, double* sum_xi_v, double* sum_xi_v2);
+
+/* Parity instrumentation (off by default; never on in timed runs).  Registers device arrays that
+ * every later sdm_coalescence_step fills; pass NULL to switch an output off again.
+ *   perm_out[s]           int32[n_sd]  original index at shuffled position s
+ *   gamma_out[i]          int64[n_sd]  gamma of the pair whose first-shuffled member is i, else 0
+ *   gamma_clamped_out[i]  int64[n_sd]  gamma~ likewise
+ *   cell_start_out[c]     int32[n_cell+1] exclusive scan of the per-cell counts */
+int sdm_debug_outputs(sdm_ctx* ctx, int32_t* perm_out, int64_t* gamma_out, int64_t* gamma_clamped_out,
+                      int32_t* cell_start_out);
+
+/* Selects the implementation path of sdm_coalescence_step (see sdm_path).  Returns INVALID_ARG for an
+ * unknown value. */
+int sdm_set_path(sdm_ctx* ctx, int path);
+
+/* Which path the most recent sdm_coalescence_step took (an sdm_path value other than AUTO), or 0 if
+ * none ran yet.  Synchronises the stream when the decision was taken on the device. */
+int sdm_last_path(sdm_ctx* ctx);
+
+/* End-to-end variant with HOST buffers (bench.py `e2e`): copies multiplicity, volume and cell_id to the
+ * device staging area bound with sdm_bind_host_staging(), runs sdm_coalescence_step there, copies
+ * multiplicity and volume back, and synchronises.  Host buffers should be pinned for full PCIe speed. */
+size_t sdm_host_staging_bytes(int64_t max_n_sd);
+int sdm_bind_host_staging(sdm_ctx* ctx, void* staging_dev, size_t staging_bytes);
+int sdm_coalescence_step_host(sdm_ctx* ctx, int64_t* multiplicity_host, double* volume_host,
+                              const int32_t* cell_id_host, int64_t n_sd, int32_t n_cell, double dt,
+                              double dV, const sdm_kernel_params* kp, uint64_t seed, uint64_t step);
+
+/* Synchronises the stream and returns the sticky status (SDM_OK, SDM_ERR_BAD_DATA, SDM_ERR_CUDA),
+ * clearing SDM_ERR_BAD_DATA. */
+int sdm_poll_error(sdm_ctx* ctx);
+
+/* Number of kernel launches (memsets excluded) the library has enqueued on this context so far. */
+int64_t sdm_launch_count(sdm_ctx* ctx);
+
+/* Test hooks for the a1 row alone: fills key[i] (uint32) and u[i] (fp64) for i in [i0, i0+n) --
+ * device arrays -- with the same device code the step uses.  Asynchronous. */
+int sdm_philox_fill(sdm_ctx* ctx, uint64_t seed, uint64_t step, uint64_t i0, int64_t n,
+                    uint32_t* key_out, double* u_out);
+
+/* Test hook for the kernel function alone: K_out[i] = K(vj[i], vk[i]) on device arrays. */
+int sdm_kernel_eval(sdm_ctx* ctx, const sdm_kernel_params* kp, const double* vj, const double* vk,
+                    int64_t n, double* K_out);
+
+const char* sdm_strerror(int status);
+void sdm_destroy(sdm_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SDM_B200_H_ */

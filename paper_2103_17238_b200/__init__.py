@@ -1,0 +1,29 @@
+"""paper_2103_17238_b200 -- B200-native Super-Droplet Method coalescence step.
+
+Thin Python binding over the C-ABI library `libsdm_b200.so` (include/sdm.h).  It only marshals
+arguments: every step of the hot path runs in the hand-written sm_100a kernels under csrc/.
+PyTorch is used for device memory and streams, nothing else.  There is no CPU fallback: without
+the built CUDA library, or without a CUDA device, the calls raise.
+"""
+from .binding import (  # noqa: F401
+    GEOMETRIC,
+    GOLOVIN,
+    PATH_AUTO,
+    PATH_CELL_SORTED,
+    PATH_GENERAL,
+    KernelParams,
+    SDMContext,
+    SDMError,
+    geometric,
+    golovin,
+    host_staging_bytes,
+    library_path,
+    load_library,
+    workspace_bytes,
+)
+
+__all__ = [
+    "SDMContext", "SDMError", "KernelParams", "golovin", "geometric", "GOLOVIN", "GEOMETRIC",
+    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "workspace_bytes", "host_staging_bytes",
+    "load_library", "library_path",
+]

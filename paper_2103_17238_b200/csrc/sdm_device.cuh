@@ -1,0 +1,147 @@
+// Device-side building blocks of the B200 SDM coalescence step (sm_100a).
+// Nothing here is shared with oracle/: the arithmetic is restated from BASELINE.json north_star
+// (a)-(c) and the readings in DESIGN.md.  Every fp64 expression that decides an integer uses
+// explicit round-to-nearest intrinsics (__dmul_rn/__dadd_rn/__dsub_rn) so no FMA can be formed,
+// in the operation order DESIGN.md R10/R13/R17 fixes.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace sdm {
+
+typedef unsigned long long u64;
+typedef unsigned int u32;
+
+// ------------------------------------------------------------------------------------------
+// a1: Philox-4x32-10 (north_star (a); Salmon et al. 2011).  The ten round keys depend only on
+// (seed) and are the same for every super-droplet, so the host precomputes them once per step.
+// ------------------------------------------------------------------------------------------
+struct PhiloxKeys {
+    u32 k0[10];
+    u32 k1[10];
+    u32 step_lo, step_hi;
+};
+
+__host__ __device__ inline PhiloxKeys make_philox_keys(u64 seed, u64 step) {
+    PhiloxKeys pk;
+    u32 a = (u32)seed, b = (u32)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        pk.k0[r] = a;
+        pk.k1[r] = b;
+        a += 0x9E3779B9u;
+        b += 0xBB67AE85u;
+    }
+    pk.step_lo = (u32)step;
+    pk.step_hi = (u32)(step >> 32);
+    return pk;
+}
+
+struct PhiloxOut {
+    u32 w0, w1, w2, w3;
+};
+
+__device__ __forceinline__ PhiloxOut philox4x32_10(const PhiloxKeys& pk, u64 i) {
+    u32 c0 = (u32)i, c1 = (u32)(i >> 32), c2 = pk.step_lo, c3 = pk.step_hi;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const u64 p0 = (u64)0xD2511F53u * (u64)c0;  // IMAD.WIDE.U32
+        const u64 p1 = (u64)0xCD9E8D57u * (u64)c2;
+        const u32 n0 = (u32)(p1 >> 32) ^ c1 ^ pk.k0[r];
+        const u32 n2 = (u32)(p0 >> 32) ^ c3 ^ pk.k1[r];
+        c1 = (u32)p1;
+        c3 = (u32)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    PhiloxOut o;
+    o.w0 = c0; o.w1 = c1; o.w2 = c2; o.w3 = c3;
+    return o;
+}
+
+// Permutation key only (word 0).
+__device__ __forceinline__ u32 philox_perm_key(const PhiloxKeys& pk, u64 i) { return philox4x32_10(pk, i).w0; }
+
+// 53-bit uniform in [0,1) from words 3:2 (R3).
+__device__ __forceinline__ double uniform_from_words(u32 w2, u32 w3) {
+    const u64 bits = (((u64)w3 << 32) | (u64)w2) >> 11;
+    return __dmul_rn((double)bits, 0x1.0p-53);
+}
+
+// ------------------------------------------------------------------------------------------
+// Relaxed / release / acquire accesses at gpu scope for the decoupled look-back tile states.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ u32 ld_relaxed_u32(const u32* p) {
+    u32 v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_u32(u32* p, u32 v) {
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ u32 ld_acquire_u32(const u32* p) {
+    u32 v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u32(u32* p, u32 v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+__device__ __forceinline__ u32 lanemask_lt() {
+    u32 m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// Streaming (read-once / write-once) global accesses: keep L1 for the gathers that reuse lines.
+__device__ __forceinline__ u64 ld_stream_u64(const u64* p) {
+    u64 v;
+    asm volatile("ld.global.L1::no_allocate.u64 %0, [%1];" : "=l"(v) : "l"(p));
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------
+// Coalescence kernels (north_star (c); R15-R17).  No FMA anywhere.
+// ------------------------------------------------------------------------------------------
+struct KernelParams {
+    int kind;  // 0 Golovin, 1 geometric
+    double b;
+    double Epi;  // E * pi, one host-side product (E * 3.141592653589793)
+};
+
+// R17: libm-free cube root: integer seed for x^(-1/3), four Newton steps, r = x z^2, one polish.
+__device__ __forceinline__ double det_cbrt(double x) {
+    if (x == 0.0) return 0.0;
+    const long long xb = __double_as_longlong(x);
+    const long long zb = 0x553F0A3D70A3D70BLL - xb / 3;
+    double z = __longlong_as_double(zb);
+    const double four_thirds = 0x1.5555555555555p+0;
+    const double one_third = 0x1.5555555555555p-2;
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+        const double z3 = __dmul_rn(__dmul_rn(z, z), z);
+        z = __dmul_rn(z, __dsub_rn(four_thirds, __dmul_rn(one_third, __dmul_rn(x, z3))));
+    }
+    double r = __dmul_rn(__dmul_rn(x, z), z);
+    const double r3 = __dmul_rn(__dmul_rn(r, r), r);
+    r = __dsub_rn(r, __dmul_rn(__dsub_rn(r3, x), __dmul_rn(__dmul_rn(z, z), one_third)));
+    return r;
+}
+
+// R16: three-regime power-law fall speed (exponents 2, 1, 1/2), SI.
+__device__ __forceinline__ double terminal_velocity(double r) {
+    if (r < 40e-6) return __dmul_rn(1.19e8, __dmul_rn(r, r));
+    if (r < 600e-6) return __dmul_rn(8e3, r);
+    return __dmul_rn(2.01e2, __dsqrt_rn(r));
+}
+
+__device__ __forceinline__ double coalescence_kernel(const KernelParams& kp, double vj, double vk) {
+    if (kp.kind == 0) return __dmul_rn(kp.b, __dadd_rn(vj, vk));
+    const double rj = det_cbrt(__dmul_rn(vj, 0.238732414637843));
+    const double rk = det_cbrt(__dmul_rn(vk, 0.238732414637843));
+    const double s = __dadd_rn(rj, rk);
+    const double dv = fabs(__dsub_rn(terminal_velocity(rj), terminal_velocity(rk)));
+    return __dmul_rn(__dmul_rn(kp.Epi, __dmul_rn(s, s)), dv);
+}
+
+}  // namespace sdm

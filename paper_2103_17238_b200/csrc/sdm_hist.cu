@@ -1,0 +1,181 @@
+// Rows a1 + a2 of SURVEY.md section 8(a): Philox permutation keys, the radix-digit histograms of
+// the composite sort key (cell_id << 32 | key), the per-cell histogram and its exclusive scan.
+//
+//   k_keys_hist  reads cell_id (4 B/SD), writes sortkey u64 (8 B/SD)            -> HBM bound, 12 B/SD
+//   k_cell_scan  one CTA, chained warp-shuffle scan over the n_cell counts       -> latency bound
+#include "sdm_internal.h"
+
+namespace sdm {
+
+constexpr int HIST_BLOCK = 256;
+constexpr int HIST_ROUNDS = 4;        // items per thread per chunk
+constexpr int SMEM_CELLS = 2048;      // cell histograms this small are built in shared memory
+
+template <bool HAS_CELLS>
+__global__ void __launch_bounds__(HIST_BLOCK)
+k_keys_hist(const int32_t* __restrict__ cell_id, long long n_sd, int n_cell, int n_cpass,
+            PhiloxKeys pk, u64* __restrict__ sortkey, u32* __restrict__ digit_hist,
+            u32* __restrict__ cell_count, u32* __restrict__ ctl, u32* __restrict__ sticky) {
+    __shared__ u32 s_hist[MAX_PASSES][RADIX];
+    __shared__ u32 s_cells[HAS_CELLS ? SMEM_CELLS : 1];
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const bool smem_cells = HAS_CELLS && n_cell <= SMEM_CELLS;
+
+    for (int q = tid; q < MAX_PASSES * RADIX; q += HIST_BLOCK) (&s_hist[0][0])[q] = 0;
+    if (smem_cells)
+        for (int q = tid; q < n_cell; q += HIST_BLOCK) s_cells[q] = 0;
+    __syncthreads();
+
+    const long long chunk = (long long)HIST_BLOCK * HIST_ROUNDS;
+    const long long n_chunks = (n_sd + chunk - 1) / chunk;
+    bool bad = false, unsorted = false;
+    for (long long ch = blockIdx.x; ch < n_chunks; ch += gridDim.x) {
+        const long long base = ch * chunk;
+        int c[HIST_ROUNDS];
+#pragma unroll
+        for (int r = 0; r < HIST_ROUNDS; ++r) {
+            const long long i = base + (long long)r * HIST_BLOCK + tid;
+            c[r] = 0;
+            if (HAS_CELLS && i < n_sd) c[r] = __ldg(cell_id + i);
+        }
+#pragma unroll
+        for (int r = 0; r < HIST_ROUNDS; ++r) {
+            const long long i = base + (long long)r * HIST_BLOCK + tid;
+            const bool valid = i < n_sd;
+            int cc = c[r];
+            if (HAS_CELLS) {
+                if (valid && (cc < 0 || cc >= n_cell)) { bad = true; cc = cc < 0 ? 0 : n_cell - 1; }
+                // cell_id non-decreasing?  (selects the cell-sorted fast path)
+                int prev = __shfl_up_sync(0xffffffffu, cc, 1);
+                if (lane == 0) prev = (valid && i > 0) ? __ldg(cell_id + i - 1) : cc;
+                if (valid && prev > cc) unsorted = true;
+            }
+            const u32 active = __ballot_sync(0xffffffffu, valid);
+            if (valid) {
+                const u32 key = philox_perm_key(pk, (u64)i);
+                sortkey[i] = ((u64)(u32)cc << 32) | (u64)key;
+                atomicAdd(&s_hist[0][key & 0xFF], 1u);
+                atomicAdd(&s_hist[1][(key >> 8) & 0xFF], 1u);
+                atomicAdd(&s_hist[2][(key >> 16) & 0xFF], 1u);
+                atomicAdd(&s_hist[3][key >> 24], 1u);
+                if (HAS_CELLS) {
+                    // warp-aggregated: one leader per distinct cell in this warp round
+                    const u32 peers = __match_any_sync(active, cc);
+                    if ((peers & lanemask_lt()) == 0) {
+                        const u32 cnt = __popc(peers);
+                        if (smem_cells) atomicAdd(&s_cells[cc], cnt);
+                        else atomicAdd(&cell_count[cc], cnt);
+                        for (int q = 0; q < n_cpass; ++q)
+                            atomicAdd(&s_hist[4 + q][((u32)cc >> (8 * q)) & 0xFF], cnt);
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int q = tid; q < (4 + n_cpass) * RADIX; q += HIST_BLOCK) {
+        const u32 h = (&s_hist[0][0])[q];
+        if (h) atomicAdd(&digit_hist[q], h);
+    }
+    if (smem_cells)
+        for (int q = tid; q < n_cell; q += HIST_BLOCK) {
+            const u32 h = s_cells[q];
+            if (h) atomicAdd(&cell_count[q], h);
+        }
+    if (bad) sticky[STICKY_BAD_DATA] = 1u;
+    if (unsorted) ctl[CTL_UNSORTED] = 1u;
+}
+
+// Exclusive scan of the per-cell counts -> cell_start[0..n_cell]; one CTA of 1024 threads walks the
+// array in coalesced slabs of 4096 counts, carrying the running total (chained warp-shuffle scans).
+constexpr int SCAN_BLOCK = 1024;
+
+__global__ void __launch_bounds__(SCAN_BLOCK)
+k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, int n_cell, u32 n_sd_total,
+            int32_t* __restrict__ dbg_cell_start) {
+    __shared__ u32 s_warp[32];
+    __shared__ u32 s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    if (n_cell == 1) {  // box model: the single cell holds every super-droplet
+        if (tid == 0) {
+            cell_start[0] = 0;
+            cell_start[1] = n_sd_total;
+            if (dbg_cell_start) { dbg_cell_start[0] = 0; dbg_cell_start[1] = (int32_t)n_sd_total; }
+        }
+        return;
+    }
+    for (int base = 0; base < n_cell; base += SCAN_BLOCK * 4) {
+        const int c0 = base + tid * 4;
+        u32 x[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) x[j] = (c0 + j < n_cell) ? cell_count[c0 + j] : 0u;
+        const u32 tsum = x[0] + x[1] + x[2] + x[3];
+        u32 incl = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const u32 y = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += y;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            u32 w = s_warp[lane];
+            u32 wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const u32 y = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += y;
+            }
+            s_warp[lane] = wi - w;  // exclusive warp offsets
+        }
+        __syncthreads();
+        const u32 carry = s_carry;
+        u32 run = carry + s_warp[warp] + (incl - tsum);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (c0 + j < n_cell) {
+                cell_start[c0 + j] = run;
+                if (dbg_cell_start) dbg_cell_start[c0 + j] = (int32_t)run;
+            }
+            run += x[j];
+        }
+        __syncthreads();
+        if (tid == SCAN_BLOCK - 1) s_carry = run;  // inclusive total through this slab
+        __syncthreads();
+    }
+    if (tid == 0) {
+        cell_start[n_cell] = n_sd_total;
+        if (dbg_cell_start) dbg_cell_start[n_cell] = (int32_t)n_sd_total;
+    }
+}
+
+cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
+                             const Plan& plan, const PhiloxKeys& pk, u64* sortkey_out) {
+    const long long chunk = (long long)HIST_BLOCK * HIST_ROUNDS;
+    long long n_chunks = (n_sd + chunk - 1) / chunk;
+    int grid = (int)(n_chunks < (long long)ctx->sm_count * 8 ? n_chunks : (long long)ctx->sm_count * 8);
+    if (grid < 1) grid = 1;
+    const int n_cpass = plan.n_pass - 4;
+    if (n_cell > 1)
+        k_keys_hist<true><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, pk, sortkey_out,
+                                                                 ctx->ws.digit_hist, ctx->ws.cell_count,
+                                                                 ctx->ws.ctl, ctx->ws.sticky);
+    else
+        k_keys_hist<false><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, pk, sortkey_out,
+                                                                  ctx->ws.digit_hist, ctx->ws.cell_count,
+                                                                  ctx->ws.ctl, ctx->ws.sticky);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cell_scan(sdm_ctx* ctx, int32_t n_cell, int64_t n_sd) {
+    k_cell_scan<<<1, SCAN_BLOCK, 0, ctx->stream>>>(ctx->ws.cell_count, ctx->ws.cell_start, n_cell, (u32)n_sd,
+                                                   ctx->dbg_cell_start);
+    ctx->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace sdm

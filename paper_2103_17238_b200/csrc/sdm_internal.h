@@ -1,0 +1,110 @@
+// Host-side internals shared by the translation units of libsdm_b200.so: the context, the
+// workspace map and the launcher prototypes.  See DESIGN.md "Data layout in HBM".
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/sdm.h"
+#include "sdm_device.cuh"
+
+namespace sdm {
+
+constexpr int RADIX_BITS = 8;
+constexpr int RADIX = 1 << RADIX_BITS;
+constexpr int MAX_PASSES = 8;  // 4 key digits + up to 4 cell-id digits (n_cell <= 2^31)
+
+// Onesweep pass tile: SORT_BLOCK threads x SORT_ITEMS keys.
+constexpr int SORT_BLOCK = 256;
+constexpr int SORT_ITEMS = 16;
+constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
+
+// Compaction tile.
+constexpr int CMP_BLOCK = 256;
+constexpr int CMP_ITEMS = 8;
+constexpr int CMP_TILE = CMP_BLOCK * CMP_ITEMS;
+
+// Words of the per-step control block (zeroed by one memset at the start of every step).
+enum CtlWord {
+    CTL_UNSORTED = 0,     // set when cell_id is not non-decreasing
+    CTL_TICKET0 = 8,      // CTL_TICKET0 + pass: dynamic tile tickets of the sort passes
+    CTL_CMP_TICKET = 24,  // compaction ticket
+    CTL_ZERO_COUNT = 25,  // compaction: number of zero-multiplicity entries (low word)
+    CTL_WORDS = 64
+};
+// Sticky words (zeroed at init and by sdm_poll_error only).
+enum StickyWord { STICKY_BAD_DATA = 0, STICKY_WORDS = 64 };
+
+struct Workspace {
+    // [zeroed per step] ------------------------------------------------
+    u32* ctl;         // CTL_WORDS
+    u32* digit_hist;  // MAX_PASSES * RADIX
+    u32* cell_count;  // max_n_cell + 1
+    u32* tile_state;  // MAX_PASSES * max_tiles * RADIX   (decoupled look-back)
+    size_t zero_bytes_fixed;  // ctl + digit_hist (contiguous from ctl)
+    // [not zeroed] -----------------------------------------------------
+    u32* sticky;      // STICKY_WORDS
+    u32* cell_start;  // max_n_cell + 1
+    u64* buf_a;       // max_n_sd
+    u64* buf_b;       // max_n_sd
+    u32* cmp_state;   // max compaction tiles
+    size_t total_bytes;
+};
+
+struct Plan {  // per-step derived quantities
+    int cbits;     // bits of (n_cell - 1)
+    int idxbits;   // bits of (n_sd - 1), at least 1
+    int n_pass;    // 4 + ceil(cbits / 8)
+    int n_tiles;   // ceil(n_sd / SORT_TILE)
+};
+
+}  // namespace sdm
+
+struct sdm_ctx {
+    int device;
+    cudaStream_t stream;
+    int64_t max_n_sd;
+    int32_t max_n_cell;
+    int64_t max_tiles;
+    sdm::Workspace ws;
+    int path;
+    int last_path;
+    int cuda_error;  // sticky cudaError_t
+    int64_t launches;
+    // debug outputs
+    int32_t* dbg_perm;
+    int64_t* dbg_gamma;
+    int64_t* dbg_gamma_clamped;
+    int32_t* dbg_cell_start;
+    // host staging
+    void* staging;
+    size_t staging_bytes;
+    int sm_count;
+};
+
+namespace sdm {
+
+Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell);
+Plan make_plan(int64_t n_sd, int32_t n_cell);
+
+// Launchers (each enqueues on ctx->stream and bumps ctx->launches).  Return cudaError_t.
+cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
+                             const Plan& plan, const PhiloxKeys& pk, u64* sortkey_out);
+cudaError_t launch_cell_scan(sdm_ctx* ctx, int32_t n_cell, int64_t n_sd);
+cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, int64_t n_sd,
+                             const Plan& plan);
+cudaError_t launch_pair(sdm_ctx* ctx, const u64* sorted, int64_t* xi, double* v, int64_t n_sd,
+                        int32_t n_cell, const Plan& plan, double dtdV, const KernelParams& kp,
+                        const PhiloxKeys& pk);
+cudaError_t launch_debug_perm(sdm_ctx* ctx, const u64* sorted, int64_t n_sd, const Plan& plan);
+cudaError_t launch_count_zero(sdm_ctx* ctx, const int64_t* xi, int64_t n_sd);
+cudaError_t launch_compact(sdm_ctx* ctx, int64_t* xi, double* v, int32_t* cell_id, int64_t n_sd);
+cudaError_t launch_cell_stats(sdm_ctx* ctx, const int64_t* xi, const double* v, const int32_t* cell_id,
+                              int64_t n_sd, int32_t n_cell, int32_t* count, int64_t* sum_xi,
+                              double* sum_xi_v, double* sum_xi_v2);
+cudaError_t launch_philox_fill(sdm_ctx* ctx, const PhiloxKeys& pk, u64 i0, int64_t n, u32* key_out,
+                               double* u_out);
+cudaError_t launch_kernel_eval(sdm_ctx* ctx, const KernelParams& kp, const double* vj, const double* vk,
+                               int64_t n, double* K_out);
+
+}  // namespace sdm
