@@ -136,9 +136,13 @@ int sdm_last_path(sdm_ctx* ctx);
  * multiplicity and volume back, and synchronises.  Host buffers should be pinned for full PCIe speed. */
 size_t sdm_host_staging_bytes(int64_t max_n_sd);
 int sdm_bind_host_staging(sdm_ctx* ctx, void* staging_dev, size_t staging_bytes);
+/* With compact != 0 the step is followed by sdm_remove_zero_multiplicity on the staged arrays; the
+ * surviving prefix of all three arrays is copied back and *n_sd_out (host, may be NULL when
+ * compact == 0) receives the new count; cell_id_host is then written too. */
 int sdm_coalescence_step_host(sdm_ctx* ctx, int64_t* multiplicity_host, double* volume_host,
-                              const int32_t* cell_id_host, int64_t n_sd, int32_t n_cell, double dt,
-                              double dV, const sdm_kernel_params* kp, uint64_t seed, uint64_t step);
+                              int32_t* cell_id_host, int64_t n_sd, int32_t n_cell, double dt, double dV,
+                              const sdm_kernel_params* kp, uint64_t seed, uint64_t step, int compact,
+                              int64_t* n_sd_out /* host */);
 
 /* Synchronises the stream and returns the sticky status (SDM_OK, SDM_ERR_BAD_DATA, SDM_ERR_CUDA),
  * clearing SDM_ERR_BAD_DATA. */
@@ -146,6 +150,15 @@ int sdm_poll_error(sdm_ctx* ctx);
 
 /* Number of kernel launches (memsets excluded) the library has enqueued on this context so far. */
 int64_t sdm_launch_count(sdm_ctx* ctx);
+
+/* Per-kernel timing for bench.py's roofline line.  While enabled, every kernel launch is bracketed by
+ * a CUDA-event pair on the context's stream.  sdm_profile_read synchronises the stream, adds up the
+ * elapsed milliseconds and the launch counts per kernel class (arrays of SDM_PROF_CLASSES entries,
+ * host) since the last read, and resets the accumulation. */
+enum { SDM_PROF_KEYS_HIST = 0, SDM_PROF_CELL_SCAN, SDM_PROF_RADIX_PASS, SDM_PROF_PAIR, SDM_PROF_COUNT_ZERO,
+       SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CLASSES };
+int sdm_profile_enable(sdm_ctx* ctx, int on);
+int sdm_profile_read(sdm_ctx* ctx, double* ms_out /* host */, int64_t* launches_out /* host */);
 
 /* Test hooks for the a1 row alone: fills key[i] (uint32) and u[i] (fp64) for i in [i0, i0+n) --
  * device arrays -- with the same device code the step uses.  Asynchronous. */

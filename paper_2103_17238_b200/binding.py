@@ -23,8 +23,11 @@ EXPORTS = [
     "sdm_workspace_bytes", "sdm_init", "sdm_coalescence_step", "sdm_remove_zero_multiplicity",
     "sdm_cell_stats", "sdm_debug_outputs", "sdm_set_path", "sdm_last_path", "sdm_host_staging_bytes",
     "sdm_bind_host_staging", "sdm_coalescence_step_host", "sdm_poll_error", "sdm_launch_count",
-    "sdm_philox_fill", "sdm_kernel_eval", "sdm_strerror", "sdm_destroy",
+    "sdm_philox_fill", "sdm_kernel_eval", "sdm_strerror", "sdm_destroy", "sdm_profile_enable",
+    "sdm_profile_read",
 ]
+
+PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other"]
 
 
 class SDMError(RuntimeError):
@@ -83,7 +86,12 @@ def load_library():
     lib.sdm_host_staging_bytes.restype = C.c_size_t
     lib.sdm_bind_host_staging.argtypes = [vp, vp, C.c_size_t]
     lib.sdm_bind_host_staging.restype = C.c_int
-    lib.sdm_coalescence_step_host.argtypes = [vp, vp, vp, vp, i64, i32, dbl, dbl, kpp, u64, u64]
+    lib.sdm_coalescence_step_host.argtypes = [vp, vp, vp, vp, i64, i32, dbl, dbl, kpp, u64, u64, C.c_int,
+                                              C.POINTER(i64)]
+    lib.sdm_profile_enable.argtypes = [vp, C.c_int]
+    lib.sdm_profile_enable.restype = C.c_int
+    lib.sdm_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
+    lib.sdm_profile_read.restype = C.c_int
     lib.sdm_coalescence_step_host.restype = C.c_int
     lib.sdm_poll_error.argtypes = [vp]
     lib.sdm_poll_error.restype = C.c_int
@@ -235,17 +243,32 @@ class SDMContext:
     def last_path(self) -> int:
         return int(self._lib.sdm_last_path(self._h))
 
-    def coalescence_step_host(self, multiplicity, volume, cell_id, n_cell, dt, dV, kp, seed, step, n_sd=None):
-        """Host (ideally pinned) torch CPU tensors in and out; copies are inside the call."""
+    def coalescence_step_host(self, multiplicity, volume, cell_id, n_cell, dt, dV, kp, seed, step, n_sd=None,
+                              compact=False) -> int:
+        """Host (ideally pinned) torch CPU tensors in and out; copies are inside the call.  Returns n_sd
+        after the optional compaction."""
         t = self._torch
         n = int(multiplicity.shape[0] if n_sd is None else n_sd)
         for x in (multiplicity, volume, cell_id):
             if x.device.type != "cpu":
                 raise ValueError("coalescence_step_host takes CPU tensors")
+        n_out = C.c_int64(n)
         rc = self._lib.sdm_coalescence_step_host(self._h, _ptr(multiplicity, t.int64), _ptr(volume, t.float64),
                                                  _ptr(cell_id, t.int32), n, int(n_cell), float(dt), float(dV),
-                                                 C.byref(kp), int(seed), int(step))
+                                                 C.byref(kp), int(seed), int(step), int(bool(compact)),
+                                                 C.byref(n_out))
         _check(rc, "sdm_coalescence_step_host")
+        return int(n_out.value)
+
+    def profile_enable(self, on: bool):
+        _check(self._lib.sdm_profile_enable(self._h, int(bool(on))), "sdm_profile_enable")
+
+    def profile_read(self):
+        """dict kernel class -> (milliseconds, launches) since the last read."""
+        ms = (C.c_double * len(PROF_CLASSES))()
+        cnt = (C.c_int64 * len(PROF_CLASSES))()
+        _check(self._lib.sdm_profile_read(self._h, ms, cnt), "sdm_profile_read")
+        return {name: (float(ms[i]), int(cnt[i])) for i, name in enumerate(PROF_CLASSES)}
 
     def poll_error(self) -> int:
         return int(self._lib.sdm_poll_error(self._h))

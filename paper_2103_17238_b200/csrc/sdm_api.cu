@@ -74,6 +74,15 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 
 using namespace sdm;
 
+static void free_ctx(sdm_ctx* ctx) {
+    if (!ctx) return;
+    if (ctx->prof_events) {
+        for (ProfEvent& e : *ctx->prof_events) { cudaEventDestroy(e.start); cudaEventDestroy(e.stop); }
+        delete ctx->prof_events;
+    }
+    delete ctx;
+}
+
 extern "C" {
 
 size_t sdm_workspace_bytes(int64_t max_n_sd, int32_t max_n_cell) {
@@ -94,6 +103,8 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
     sdm_ctx* ctx = new (std::nothrow) sdm_ctx();
     if (!ctx) return SDM_ERR_CUDA;
     std::memset(ctx, 0, sizeof(*ctx));
+    ctx->prof_events = new (std::nothrow) std::vector<ProfEvent>();
+    if (!ctx->prof_events) { delete ctx; return SDM_ERR_CUDA; }
     ctx->device = device;
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     ctx->max_n_sd = max_n_sd;
@@ -102,20 +113,44 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
     ctx->path = SDM_PATH_AUTO;
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms <= 0) {
-        delete ctx;
+        free_ctx(ctx);
         return SDM_ERR_CUDA;
     }
     ctx->sm_count = sms;
     if (cudaMemsetAsync(ctx->ws.sticky, 0, STICKY_WORDS * 4, ctx->stream) != cudaSuccess ||
         cudaMemsetAsync(ctx->ws.ctl, 0, CTL_WORDS * 4, ctx->stream) != cudaSuccess) {
-        delete ctx;
+        free_ctx(ctx);
         return SDM_ERR_CUDA;
     }
     *out = ctx;
     return SDM_OK;
 }
 
-void sdm_destroy(sdm_ctx* ctx) { delete ctx; }
+void sdm_destroy(sdm_ctx* ctx) { free_ctx(ctx); }
+
+int sdm_profile_enable(sdm_ctx* ctx, int on) {
+    if (!ctx) return SDM_ERR_INVALID_ARG;
+    ctx->profiling = on ? 1 : 0;
+    return SDM_OK;
+}
+
+int sdm_profile_read(sdm_ctx* ctx, double* ms_out, int64_t* launches_out) {
+    if (!ctx || !ms_out || !launches_out) return SDM_ERR_INVALID_ARG;
+    for (int c = 0; c < PROF_CLASSES; ++c) { ms_out[c] = 0.0; launches_out[c] = 0; }
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
+    int rc;
+    if ((rc = note_cuda(ctx, cudaStreamSynchronize(ctx->stream)))) return rc;
+    for (size_t i = 0; i < ctx->prof_used; ++i) {
+        ProfEvent& e = (*ctx->prof_events)[i];
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, e.start, e.stop) == cudaSuccess) {
+            ms_out[e.cls] += (double)ms;
+            launches_out[e.cls] += 1;
+        }
+    }
+    ctx->prof_used = 0;
+    return SDM_OK;
+}
 
 const char* sdm_strerror(int status) {
     switch (status) {
@@ -308,11 +343,13 @@ int sdm_bind_host_staging(sdm_ctx* ctx, void* staging_dev, size_t staging_bytes)
 }
 
 int sdm_coalescence_step_host(sdm_ctx* ctx, int64_t* multiplicity_host, double* volume_host,
-                              const int32_t* cell_id_host, int64_t n_sd, int32_t n_cell, double dt, double dV,
-                              const sdm_kernel_params* kp, uint64_t seed, uint64_t step) {
+                              int32_t* cell_id_host, int64_t n_sd, int32_t n_cell, double dt, double dV,
+                              const sdm_kernel_params* kp, uint64_t seed, uint64_t step, int compact,
+                              int64_t* n_sd_out) {
     int rc = validate_step(ctx, multiplicity_host, volume_host, cell_id_host, n_sd, n_cell, dt, dV, kp);
     if (rc != SDM_OK) return rc;
-    if (!ctx->staging) return SDM_ERR_INVALID_ARG;
+    if (!ctx->staging || (compact && !n_sd_out)) return SDM_ERR_INVALID_ARG;
+    if (n_sd_out) *n_sd_out = n_sd;
     if (n_sd == 0) return SDM_OK;
     if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
     const size_t n = (size_t)ctx->max_n_sd;
@@ -326,8 +363,16 @@ int sdm_coalescence_step_host(sdm_ctx* ctx, int64_t* multiplicity_host, double* 
     if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_c, cell_id_host, (size_t)n_sd * 4, cudaMemcpyHostToDevice, st)))) return rc;
     rc = sdm_coalescence_step(ctx, d_xi, d_v, d_c, n_sd, n_cell, dt, dV, kp, seed, step);
     if (rc != SDM_OK) return rc;
-    if ((rc = note_cuda(ctx, cudaMemcpyAsync(multiplicity_host, d_xi, (size_t)n_sd * 8, cudaMemcpyDeviceToHost, st)))) return rc;
-    if ((rc = note_cuda(ctx, cudaMemcpyAsync(volume_host, d_v, (size_t)n_sd * 8, cudaMemcpyDeviceToHost, st)))) return rc;
+    int64_t n_out = n_sd;
+    if (compact) {
+        rc = sdm_remove_zero_multiplicity(ctx, d_xi, d_v, d_c, n_sd, &n_out);
+        if (rc != SDM_OK) return rc;
+        *n_sd_out = n_out;
+        if (n_out != n_sd)
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(cell_id_host, d_c, (size_t)n_out * 4, cudaMemcpyDeviceToHost, st)))) return rc;
+    }
+    if ((rc = note_cuda(ctx, cudaMemcpyAsync(multiplicity_host, d_xi, (size_t)n_out * 8, cudaMemcpyDeviceToHost, st)))) return rc;
+    if ((rc = note_cuda(ctx, cudaMemcpyAsync(volume_host, d_v, (size_t)n_out * 8, cudaMemcpyDeviceToHost, st)))) return rc;
     return note_cuda(ctx, cudaStreamSynchronize(st));
 }
 

@@ -180,16 +180,16 @@ cudaError_t launch_count_zero(sdm_ctx* ctx, const int64_t* xi, int64_t n_sd) {
     long long want = (n_sd / 2 + 255) / 256;
     int grid = (int)(want < (long long)ctx->sm_count * 8 ? want : (long long)ctx->sm_count * 8);
     if (grid < 1) grid = 1;
+    LaunchScope scope(ctx, PROF_COUNT_ZERO);
     k_count_zero<<<grid, 256, 0, ctx->stream>>>(reinterpret_cast<const long long*>(xi), n_sd, ctx->ws.ctl);
-    ctx->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_compact(sdm_ctx* ctx, int64_t* xi, double* v, int32_t* cell_id, int64_t n_sd) {
     const u32 n_tiles = (u32)((n_sd + CMP_TILE - 1) / CMP_TILE);
+    LaunchScope scope(ctx, PROF_COMPACT);
     k_compact<<<n_tiles, CMP_BLOCK, 0, ctx->stream>>>(reinterpret_cast<long long*>(xi), v, cell_id, (u32)n_sd,
                                                       ctx->ws.ctl + CTL_CMP_TICKET, ctx->ws.cmp_state);
-    ctx->launches++;
     return cudaGetLastError();
 }
 
@@ -199,26 +199,26 @@ cudaError_t launch_cell_stats(sdm_ctx* ctx, const int64_t* xi, const double* v, 
     long long want = (n_sd + 255) / 256;
     int grid = (int)(want < (long long)ctx->sm_count * 16 ? want : (long long)ctx->sm_count * 16);
     if (grid < 1) grid = 1;
+    LaunchScope scope(ctx, PROF_CELL_STATS);
     k_cell_stats<<<grid, 256, 0, ctx->stream>>>(reinterpret_cast<const long long*>(xi), v, cell_id, n_sd, n_cell,
                                                 count, reinterpret_cast<unsigned long long*>(sum_xi), sum_xi_v,
                                                 sum_xi_v2, ctx->ws.sticky);
-    ctx->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_philox_fill(sdm_ctx* ctx, const PhiloxKeys& pk, u64 i0, int64_t n, u32* key_out,
                                double* u_out) {
     const u32 grid = (u32)((n + 255) / 256);
+    LaunchScope scope(ctx, PROF_OTHER);
     k_philox_fill<<<grid, 256, 0, ctx->stream>>>(pk, i0, n, key_out, u_out);
-    ctx->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_kernel_eval(sdm_ctx* ctx, const KernelParams& kp, const double* vj, const double* vk,
                                int64_t n, double* K_out) {
     const u32 grid = (u32)((n + 255) / 256);
+    LaunchScope scope(ctx, PROF_OTHER);
     k_kernel_eval<<<grid, 256, 0, ctx->stream>>>(kp, vj, vk, n, K_out);
-    ctx->launches++;
     return cudaGetLastError();
 }
 

@@ -159,6 +159,7 @@ cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd,
     int grid = (int)(n_chunks < (long long)ctx->sm_count * 8 ? n_chunks : (long long)ctx->sm_count * 8);
     if (grid < 1) grid = 1;
     const int n_cpass = plan.n_pass - 4;
+    LaunchScope scope(ctx, PROF_KEYS_HIST);
     if (n_cell > 1)
         k_keys_hist<true><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, pk, sortkey_out,
                                                                  ctx->ws.digit_hist, ctx->ws.cell_count,
@@ -167,14 +168,13 @@ cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd,
         k_keys_hist<false><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, pk, sortkey_out,
                                                                   ctx->ws.digit_hist, ctx->ws.cell_count,
                                                                   ctx->ws.ctl, ctx->ws.sticky);
-    ctx->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_cell_scan(sdm_ctx* ctx, int32_t n_cell, int64_t n_sd) {
+    LaunchScope scope(ctx, PROF_CELL_SCAN);
     k_cell_scan<<<1, SCAN_BLOCK, 0, ctx->stream>>>(ctx->ws.cell_count, ctx->ws.cell_start, n_cell, (u32)n_sd,
                                                    ctx->dbg_cell_start);
-    ctx->launches++;
     return cudaGetLastError();
 }
 

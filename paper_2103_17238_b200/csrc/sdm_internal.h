@@ -3,6 +3,7 @@
 #pragma once
 #include <cstddef>
 #include <cstdint>
+#include <vector>
 #include <cuda_runtime.h>
 
 #include "../../include/sdm.h"
@@ -60,6 +61,13 @@ struct Plan {  // per-step derived quantities
 
 }  // namespace sdm
 
+namespace sdm {
+// Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
+enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CLASSES };
+struct ProfEvent { cudaEvent_t start, stop; int cls; };
+}  // namespace sdm
+
 struct sdm_ctx {
     int device;
     cudaStream_t stream;
@@ -80,9 +88,36 @@ struct sdm_ctx {
     void* staging;
     size_t staging_bytes;
     int sm_count;
+    // optional per-launch CUDA-event timing (sdm_profile_enable)
+    int profiling;
+    std::vector<sdm::ProfEvent>* prof_events;
+    size_t prof_used;
 };
 
 namespace sdm {
+
+// RAII bracket around one kernel launch: counts it and, when profiling is on, records a CUDA-event pair
+// on the launching stream.
+struct LaunchScope {
+    sdm_ctx* ctx;
+    cudaEvent_t stop;
+    LaunchScope(sdm_ctx* c, int cls) : ctx(c), stop(nullptr) {
+        ctx->launches++;
+        if (!ctx->profiling) return;
+        if (ctx->prof_used == ctx->prof_events->size()) {
+            ProfEvent e;
+            if (cudaEventCreate(&e.start) != cudaSuccess || cudaEventCreate(&e.stop) != cudaSuccess) return;
+            ctx->prof_events->push_back(e);
+        }
+        ProfEvent& e = (*ctx->prof_events)[ctx->prof_used++];
+        e.cls = cls;
+        cudaEventRecord(e.start, ctx->stream);
+        stop = e.stop;
+    }
+    ~LaunchScope() {
+        if (stop) cudaEventRecord(stop, ctx->stream);
+    }
+};
 
 Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell);
 Plan make_plan(int64_t n_sd, int32_t n_cell);

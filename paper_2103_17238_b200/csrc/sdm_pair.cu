@@ -94,8 +94,7 @@ __global__ void __launch_bounds__(PAIR_BLOCK) k_pair(const PairArgs a) {
     u32 c0 = a.single_cell ? 0u : (u32)(P0 >> a.cshift);
     u32 start = a.single_cell ? 0u : __ldg(a.cell_start + c0);
     u32 end = a.single_cell ? a.n_sd : __ldg(a.cell_start + c0 + 1);
-    u32 f;  // first position of the pair this thread owns
-    u64 Pf, Pg;
+    u64 Pf, Pg;  // packed words of the pair this thread owns (first, second)
     if (((s0 - start) & 1u) == 0u) {
         if (s0 + 1u >= end) {
             // s0 is the unpaired last SD of its cell; s0+1 (if any) opens the next cell at offset 0
@@ -104,9 +103,9 @@ __global__ void __launch_bounds__(PAIR_BLOCK) k_pair(const PairArgs a) {
             start = s0 + 1u;
             end = __ldg(a.cell_start + c1 + 1);
             if (s0 + 2u >= end) return;
-            f = s0 + 1u; Pf = P1; Pg = a.sorted[s0 + 2u];
+            Pf = P1; Pg = a.sorted[s0 + 2u];
         } else {
-            f = s0; Pf = P0; Pg = P1;
+            Pf = P0; Pg = P1;
         }
     } else {
         // s0 is the second member of the previous thread's pair; s0+1 has even offset if in the same cell
@@ -117,9 +116,8 @@ __global__ void __launch_bounds__(PAIR_BLOCK) k_pair(const PairArgs a) {
             end = __ldg(a.cell_start + c1 + 1);
         }
         if (s0 + 2u >= end) return;
-        f = s0 + 1u; Pf = P1; Pg = a.sorted[s0 + 2u];
+        Pf = P1; Pg = a.sorted[s0 + 2u];
     }
-    (void)f;
     pair_collide(a, (u32)(Pf & idx_mask), (u32)(Pg & idx_mask), end - start);
 }
 
@@ -148,15 +146,15 @@ cudaError_t launch_pair(sdm_ctx* ctx, const u64* sorted, int64_t* xi, double* v,
     a.dbg_gamma_clamped = reinterpret_cast<long long*>(ctx->dbg_gamma_clamped);
     const u32 n_threads = (u32)((n_sd + 1) / 2);
     const u32 grid = (n_threads + PAIR_BLOCK - 1) / PAIR_BLOCK;
+    LaunchScope scope(ctx, PROF_PAIR);
     k_pair<<<grid, PAIR_BLOCK, 0, ctx->stream>>>(a);
-    ctx->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_debug_perm(sdm_ctx* ctx, const u64* sorted, int64_t n_sd, const Plan& plan) {
     const u32 grid = (u32)((n_sd + 255) / 256);
+    LaunchScope scope(ctx, PROF_OTHER);
     k_debug_perm<<<grid, 256, 0, ctx->stream>>>(sorted, (u32)n_sd, plan.idxbits, ctx->dbg_perm);
-    ctx->launches++;
     return cudaGetLastError();
 }
 

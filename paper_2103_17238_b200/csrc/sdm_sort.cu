@@ -161,6 +161,7 @@ cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, in
     u32* ticket = ctx->ws.ctl + CTL_TICKET0 + pass;
     u32* state = ctx->ws.tile_state + (size_t)pass * (size_t)plan.n_tiles * RADIX;
     const u32* ghist = ctx->ws.digit_hist + pass * RADIX;
+    LaunchScope scope(ctx, PROF_RADIX_PASS);
     if (pass == 0) {
         k_radix_pass<true><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(in, out, (u32)n_sd, SORT_TILE_BITS, plan.idxbits,
                                                                           ghist, ticket, state);
@@ -169,7 +170,6 @@ cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, in
         k_radix_pass<false><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(in, out, (u32)n_sd, shift,
                                                                            plan.idxbits, ghist, ticket, state);
     }
-    ctx->launches++;
     return cudaGetLastError();
 }
 
