@@ -58,13 +58,18 @@ typedef struct {
     double E; /* geometric collision efficiency, >= 0 (configs use 1.0) */
 } sdm_kernel_params;
 
-/* Path selection for sdm_coalescence_step (sdm_set_path).  Every path produces the same bits. */
-typedef enum {
-    SDM_PATH_AUTO = 0,    /* pick by size / cell ordering (default) */
-    SDM_PATH_GENERAL = 1, /* global LSD radix sort of (cell_id, Philox key): north_star (b) */
-    SDM_PATH_CELL_SORTED = 2 /* per-cell shared-memory sort, only legal when cell_id is non-decreasing;
-                                falls back to GENERAL (same result) when it is not */
-} sdm_path;
+/* Path selection for sdm_coalescence_step (sdm_set_path).  Every path produces the same bits.
+ *   GENERAL      global stable LSD radix sort of (cell_id, Philox key): north_star (b).  Any input.
+ *   CELL_SORTED  per-cell register-resident sort fused with the pair kernel.  Legal
+ *                only when cell_id is non-decreasing and no cell holds more than 256 super-droplets; the
+ *                kernel checks both on the device: on a violation the step is NOT applied and the
+ *                sticky SDM_ERR_BAD_DATA flag is set.
+ *   AUTO         (default) the first step on a given (cell_id pointer, n_sd, n_cell) takes GENERAL, which
+ *                also records whether the array is sorted and its largest cell; later steps on the same
+ *                triple take CELL_SORTED when that verdict allows it.  If cell_id was then modified in
+ *                place so that the verdict no longer holds, the device check above catches it (step
+ *                skipped, SDM_ERR_BAD_DATA at the next poll, verdict reset). */
+typedef enum { SDM_PATH_AUTO = 0, SDM_PATH_GENERAL = 1, SDM_PATH_CELL_SORTED = 2 } sdm_path;
 
 /* Bytes of device workspace sdm_init() needs for problems up to (max_n_sd, max_n_cell).
  * Returns 0 when the arguments are invalid (max_n_sd < 0, max_n_sd >= 2^30, max_n_cell < 1). */
@@ -156,7 +161,8 @@ int64_t sdm_launch_count(sdm_ctx* ctx);
  * elapsed milliseconds and the launch counts per kernel class (arrays of SDM_PROF_CLASSES entries,
  * host) since the last read, and resets the accumulation. */
 enum { SDM_PROF_KEYS_HIST = 0, SDM_PROF_CELL_SCAN, SDM_PROF_RADIX_PASS, SDM_PROF_PAIR, SDM_PROF_COUNT_ZERO,
-       SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CLASSES };
+       SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CELL_BOUNDS, SDM_PROF_CELL_FUSED,
+       SDM_PROF_CLASSES };
 int sdm_profile_enable(sdm_ctx* ctx, int on);
 int sdm_profile_read(sdm_ctx* ctx, double* ms_out /* host */, int64_t* launches_out /* host */);
 

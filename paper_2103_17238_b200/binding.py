@@ -27,7 +27,8 @@ EXPORTS = [
     "sdm_profile_read",
 ]
 
-PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other"]
+PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
+                "cell_bounds", "cell_fused"]
 
 
 class SDMError(RuntimeError):

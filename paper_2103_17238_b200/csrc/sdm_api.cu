@@ -80,6 +80,8 @@ static void free_ctx(sdm_ctx* ctx) {
         for (ProfEvent& e : *ctx->prof_events) { cudaEventDestroy(e.start); cudaEventDestroy(e.stop); }
         delete ctx->prof_events;
     }
+    if (ctx->verdict_host) cudaFreeHost(ctx->verdict_host);
+    if (ctx->verdict_event) cudaEventDestroy(ctx->verdict_event);
     delete ctx;
 }
 
@@ -117,6 +119,11 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
         return SDM_ERR_CUDA;
     }
     ctx->sm_count = sms;
+    if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->verdict_host), sizeof(Verdict), cudaHostAllocDefault) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->verdict_event, cudaEventDisableTiming) != cudaSuccess) {
+        free_ctx(ctx);
+        return SDM_ERR_CUDA;
+    }
     if (cudaMemsetAsync(ctx->ws.sticky, 0, STICKY_WORDS * 4, ctx->stream) != cudaSuccess ||
         cudaMemsetAsync(ctx->ws.ctl, 0, CTL_WORDS * 4, ctx->stream) != cudaSuccess) {
         free_ctx(ctx);
@@ -217,23 +224,42 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         return SDM_OK;
     }
 
-    // zero the per-step control block, the digit histograms, the cell counts and the look-back states
-    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
-    if (n_cell > 1)
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.cell_count, 0, ((size_t)n_cell + 1) * 4, st)))) return rc;
-    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)plan.n_pass * plan.n_tiles * RADIX * 4, st))))
-        return rc;
     if (ctx->dbg_gamma)
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_gamma, 0, (size_t)n_sd * 8, st)))) return rc;
     if (ctx->dbg_gamma_clamped)
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_gamma_clamped, 0, (size_t)n_sd * 8, st)))) return rc;
-
     const PhiloxKeys pk = make_philox_keys(seed, step);
     KernelParams dkp;
     dkp.kind = kp->kind;
     dkp.b = kp->b;
     dkp.Epi = kp->E * 3.141592653589793;
     const double dtdV = dt / dV;
+
+    // ---- path selection (include/sdm.h, sdm_path) ----
+    bool fast = false;
+    if (n_cell > 1) {
+        if (ctx->path == SDM_PATH_CELL_SORTED) {
+            fast = true;
+        } else if (ctx->path == SDM_PATH_AUTO && ctx->verdict_valid && ctx->verdict_cell_ptr == cell_id &&
+                   ctx->verdict_n_sd == n_sd && ctx->verdict_n_cell == n_cell &&
+                   cudaEventQuery(ctx->verdict_event) == cudaSuccess) {
+            fast = ctx->verdict_host->unsorted == 0 && ctx->verdict_host->max_count <= (u32)CELL_FAST_MAX;
+        }
+    }
+    if (fast) {
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, CTL_WORDS * 4, st)))) return rc;
+        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, multiplicity, volume, cell_id, n_sd, n_cell, dtdV, dkp, pk))))
+            return rc;
+        ctx->last_path = SDM_PATH_CELL_SORTED;
+        return SDM_OK;
+    }
+
+    // zero the per-step control block, the digit histograms, the cell counts and the look-back states
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
+    if (n_cell > 1)
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.cell_count, 0, ((size_t)n_cell + 1) * 4, st)))) return rc;
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)plan.n_pass * plan.n_tiles * RADIX * 4, st))))
+        return rc;
 
     // a1 + a2: keys, digit histograms, cell histogram; then the cell scan
     if ((rc = note_cuda(ctx, launch_keys_hist(ctx, cell_id, n_sd, n_cell, plan, pk, ws.buf_b)))) return rc;
@@ -252,6 +278,18 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
     if ((rc = note_cuda(ctx, launch_pair(ctx, sorted, multiplicity, volume, n_sd, n_cell, plan, dtdV, dkp, pk))))
         return rc;
     ctx->last_path = SDM_PATH_GENERAL;
+    // what this step learned about cell_id feeds AUTO's choice for the next one (asynchronous copy)
+    ctx->verdict_valid = 0;
+    if (n_cell > 1 && ctx->path == SDM_PATH_AUTO) {
+        if ((rc = note_cuda(ctx, cudaMemcpyAsync(ctx->verdict_host, ws.ctl + CTL_UNSORTED, sizeof(Verdict),
+                                                 cudaMemcpyDeviceToHost, st))))
+            return rc;
+        if ((rc = note_cuda(ctx, cudaEventRecord(ctx->verdict_event, st)))) return rc;
+        ctx->verdict_cell_ptr = cell_id;
+        ctx->verdict_n_sd = n_sd;
+        ctx->verdict_n_cell = n_cell;
+        ctx->verdict_valid = 1;
+    }
     return SDM_OK;
 }
 
@@ -285,8 +323,12 @@ int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* vo
         if ((rc = note_cuda(ctx, launch_compact(ctx, multiplicity, volume, cell_id, n_sd)))) return rc;
     }
     *n_sd_out = n_sd - zeros;
+    // stable compaction keeps a sorted cell_id sorted and cannot grow a cell: the verdict carries over
+    if (ctx->verdict_valid && ctx->verdict_cell_ptr == cell_id && ctx->verdict_n_sd == n_sd)
+        ctx->verdict_n_sd = n_sd - zeros;
     if (host_words[1]) {
         cudaMemsetAsync(ctx->ws.sticky, 0, STICKY_WORDS * 4, st);
+        ctx->verdict_valid = 0;
         return SDM_ERR_BAD_DATA;
     }
     return SDM_OK;
@@ -322,6 +364,7 @@ int sdm_poll_error(sdm_ctx* ctx) {
     if ((rc = note_cuda(ctx, cudaStreamSynchronize(ctx->stream)))) return rc;
     if (bad) {
         cudaMemsetAsync(ctx->ws.sticky, 0, STICKY_WORDS * 4, ctx->stream);
+        ctx->verdict_valid = 0;  // AUTO re-learns the cell order on the next step
         return SDM_ERR_BAD_DATA;
     }
     return SDM_OK;

@@ -93,17 +93,20 @@ constexpr int SCAN_BLOCK = 1024;
 
 __global__ void __launch_bounds__(SCAN_BLOCK)
 k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, int n_cell, u32 n_sd_total,
-            int32_t* __restrict__ dbg_cell_start) {
+            int32_t* __restrict__ dbg_cell_start, u32* __restrict__ ctl) {
     __shared__ u32 s_warp[32];
     __shared__ u32 s_carry;
+    __shared__ u32 s_max;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_carry = 0;
+    if (tid == 0) { s_carry = 0; s_max = 0; }
+    u32 my_max = 0;
     __syncthreads();
     if (n_cell == 1) {  // box model: the single cell holds every super-droplet
         if (tid == 0) {
             cell_start[0] = 0;
             cell_start[1] = n_sd_total;
             if (dbg_cell_start) { dbg_cell_start[0] = 0; dbg_cell_start[1] = (int32_t)n_sd_total; }
+            ctl[CTL_MAX_COUNT] = n_sd_total;
         }
         return;
     }
@@ -113,6 +116,7 @@ k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, in
 #pragma unroll
         for (int j = 0; j < 4; ++j) x[j] = (c0 + j < n_cell) ? cell_count[c0 + j] : 0u;
         const u32 tsum = x[0] + x[1] + x[2] + x[3];
+        my_max = max(my_max, max(max(x[0], x[1]), max(x[2], x[3])));
         u32 incl = tsum;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -146,9 +150,13 @@ k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, in
         if (tid == SCAN_BLOCK - 1) s_carry = run;  // inclusive total through this slab
         __syncthreads();
     }
+    my_max = __reduce_max_sync(0xffffffffu, my_max);
+    if (lane == 0) atomicMax(&s_max, my_max);
+    __syncthreads();
     if (tid == 0) {
         cell_start[n_cell] = n_sd_total;
         if (dbg_cell_start) dbg_cell_start[n_cell] = (int32_t)n_sd_total;
+        ctl[CTL_MAX_COUNT] = s_max;
     }
 }
 
@@ -174,7 +182,7 @@ cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd,
 cudaError_t launch_cell_scan(sdm_ctx* ctx, int32_t n_cell, int64_t n_sd) {
     LaunchScope scope(ctx, PROF_CELL_SCAN);
     k_cell_scan<<<1, SCAN_BLOCK, 0, ctx->stream>>>(ctx->ws.cell_count, ctx->ws.cell_start, n_cell, (u32)n_sd,
-                                                   ctx->dbg_cell_start);
+                                                   ctx->dbg_cell_start, ctx->ws.ctl);
     return cudaGetLastError();
 }
 

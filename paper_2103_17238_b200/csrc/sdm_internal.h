@@ -20,6 +20,9 @@ constexpr int SORT_BLOCK = 256;
 constexpr int SORT_ITEMS = 16;
 constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
 
+// Largest cell the register-resident per-cell sort of the fast path handles (one warp, 8 keys per lane).
+constexpr int CELL_FAST_MAX = 256;
+
 // Compaction tile.
 constexpr int CMP_BLOCK = 256;
 constexpr int CMP_ITEMS = 8;
@@ -27,7 +30,8 @@ constexpr int CMP_TILE = CMP_BLOCK * CMP_ITEMS;
 
 // Words of the per-step control block (zeroed by one memset at the start of every step).
 enum CtlWord {
-    CTL_UNSORTED = 0,     // set when cell_id is not non-decreasing
+    CTL_UNSORTED = 0,     // set when cell_id is not non-decreasing (fast path: the step is skipped)
+    CTL_MAX_COUNT = 1,    // general path: largest per-cell count (feeds the host-side path verdict)
     CTL_TICKET0 = 8,      // CTL_TICKET0 + pass: dynamic tile tickets of the sort passes
     CTL_CMP_TICKET = 24,  // compaction ticket
     CTL_ZERO_COUNT = 25,  // compaction: number of zero-multiplicity entries (low word)
@@ -64,7 +68,10 @@ struct Plan {  // per-step derived quantities
 namespace sdm {
 // Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
 enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
-                 PROF_CELL_STATS, PROF_OTHER, PROF_CLASSES };
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CLASSES };
+// What the last general-path step learned about the cell_id array (pinned host memory, written by an
+// asynchronous copy; valid once `verdict_event` has completed).
+struct Verdict { u32 unsorted; u32 max_count; };
 struct ProfEvent { cudaEvent_t start, stop; int cls; };
 }  // namespace sdm
 
@@ -92,6 +99,13 @@ struct sdm_ctx {
     int profiling;
     std::vector<sdm::ProfEvent>* prof_events;
     size_t prof_used;
+    // AUTO path selection: verdict of the last general-path step about (cell_id pointer, n_sd, n_cell)
+    sdm::Verdict* verdict_host;  // pinned
+    cudaEvent_t verdict_event;
+    const void* verdict_cell_ptr;
+    int64_t verdict_n_sd;
+    int32_t verdict_n_cell;
+    int verdict_valid;
 };
 
 namespace sdm {
@@ -131,6 +145,8 @@ cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, in
 cudaError_t launch_pair(sdm_ctx* ctx, const u64* sorted, int64_t* xi, double* v, int64_t n_sd,
                         int32_t n_cell, const Plan& plan, double dtdV, const KernelParams& kp,
                         const PhiloxKeys& pk);
+cudaError_t launch_cell_fused(sdm_ctx* ctx, int64_t* xi, double* v, const int32_t* cell_id, int64_t n_sd,
+                              int32_t n_cell, double dtdV, const KernelParams& kp, const PhiloxKeys& pk);
 cudaError_t launch_debug_perm(sdm_ctx* ctx, const u64* sorted, int64_t n_sd, const Plan& plan);
 cudaError_t launch_count_zero(sdm_ctx* ctx, const int64_t* xi, int64_t n_sd);
 cudaError_t launch_compact(sdm_ctx* ctx, int64_t* xi, double* v, int32_t* cell_id, int64_t n_sd);

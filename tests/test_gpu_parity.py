@@ -158,6 +158,96 @@ def test_small_configs_auto_path(dev, name):
     _run_parity(W.small(name), dev, path=None, bit_exact=True)
 
 
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg3z", "cfg4", "cfg4s"])
+def test_small_configs_cell_sorted_path(dev, name):
+    """per-cell register sort fused with the pair kernel; same bits as the oracle."""
+    sdm = _sdm()
+    st = _run_parity(W.small(name), dev, path=sdm.PATH_CELL_SORTED, bit_exact=True)
+    if name == "cfg4s":
+        assert st["clamped"] > 0 and st["removed"] > 0
+
+
+@pytest.mark.parametrize("per_cell", [1, 2, 3, 31, 32, 33, 63, 64, 65, 127, 129, 255, 256])
+def test_cell_sorted_path_cell_sizes(dev, per_cell):
+    """every register-tile width of the per-cell sort, at and around its boundaries, plus empty cells"""
+    sdm = _sdm()
+    rng = np.random.default_rng(per_cell)
+    n_cell = 41
+    counts = np.full(n_cell, per_cell)
+    counts[[3, 4, 17, 40]] = 0                      # empty cells, including the last one
+    counts[5] = max(per_cell - 1, 0)
+    cell = np.repeat(np.arange(n_cell, dtype=np.int32), counts)
+    n = len(cell)
+    xi = rng.integers(1, 60, n).astype(np.int64)
+    xi[rng.random(n) < 0.2] = 9
+    v = rng.integers(1, 9, n).astype(np.float64)
+    w = W.Workload("edge", xi, v, cell, n_cell, 1.0, 1.0, W.GOLOVIN, 2.0 ** -9, 0.0, 4, 2)
+    _run_parity(w, dev, path=sdm.PATH_CELL_SORTED, bit_exact=True)
+
+
+def test_auto_path_switches_to_cell_sorted(dev):
+    sdm = _sdm()
+    w = W.small("cfg3")
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        kp = _gkp(w)
+        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 0)
+        assert ctx.last_path() == sdm.PATH_GENERAL          # first sight of this cell_id array
+        torch.cuda.synchronize()
+        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 1)
+        assert ctx.last_path() == sdm.PATH_CELL_SORTED      # verdict: sorted, cells <= 256
+        # an interleaved array never leaves the general path
+        wi = W.small("cfg3", interleave=True)
+        xi2, v2, cell2 = _to_dev(wi, dev)
+        for s in range(3):
+            ctx.coalescence_step(xi2, v2, cell2, wi.n_cell, wi.dt, wi.dV, kp, 42, s)
+            torch.cuda.synchronize()
+            assert ctx.last_path() == sdm.PATH_GENERAL
+        # cells larger than the fast path's limit: general path
+        big = W.cfg3(n_cell=8, per_cell=300, n_steps=3)
+        xb, vb, cb = _to_dev(big, dev)
+        for s in range(3):
+            ctx.coalescence_step(xb, vb, cb, big.n_cell, big.dt, big.dV, kp, 42, s)
+            torch.cuda.synchronize()
+            assert ctx.last_path() == sdm.PATH_GENERAL
+        assert ctx.poll_error() == 0
+
+
+def test_cell_sorted_path_refuses_unsorted_input(dev):
+    """explicit CELL_SORTED on an unsorted array, and AUTO with a verdict that went stale because
+    cell_id was modified in place: the step is not applied and SDM_ERR_BAD_DATA is reported."""
+    sdm = _sdm()
+    w = W.small("cfg3")
+    kp = _gkp(w)
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        cell[100], cell[5000] = cell[5000].item(), cell[100].item()      # break the order
+        ctx.set_path(sdm.PATH_CELL_SORTED)
+        before = xi.clone(), v.clone()
+        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 0)
+        assert ctx.poll_error() == -4
+        assert torch.equal(xi, before[0]) and torch.equal(v, before[1])
+        # AUTO: learn "sorted", then break the array in place
+        ctx.set_path(sdm.PATH_AUTO)
+        xi, v, cell = _to_dev(w, dev)
+        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 0)
+        torch.cuda.synchronize()
+        cell[100], cell[5000] = cell[5000].item(), cell[100].item()
+        before = xi.clone(), v.clone()
+        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 1)
+        assert ctx.last_path() == sdm.PATH_CELL_SORTED
+        assert ctx.poll_error() == -4                                     # caught on the device
+        assert torch.equal(xi, before[0]) and torch.equal(v, before[1])
+        # the verdict was reset: the next step takes the general path and matches the oracle
+        ow = w.copy()
+        oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), 42, 0)
+        ow.cell_id[100], ow.cell_id[5000] = ow.cell_id[5000], ow.cell_id[100]
+        oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), 42, 1)
+        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 1)
+        assert ctx.last_path() == sdm.PATH_GENERAL and ctx.poll_error() == 0
+        assert np.array_equal(xi.cpu().numpy(), ow.xi)
+
+
 def test_worked_step_on_device(dev):
     """The SURVEY P12 worked example straight through the C ABI."""
     sdm = _sdm()
