@@ -218,7 +218,8 @@ def run_ours(args):
 
     ctx = sdm.SDMContext(n0, w.n_cell, device=dev, host_staging=True)
     if args.path:
-        ctx.set_path({"auto": sdm.PATH_AUTO, "general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED}[args.path])
+        ctx.set_path({"auto": sdm.PATH_AUTO, "general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED,
+                      "hybrid": sdm.PATH_HYBRID}[args.path])
     stream = torch.cuda.current_stream(dev)
 
     def one_step(s, n):
@@ -356,7 +357,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "ours",
             "config": workload_config(w, args.workload, {"parallelism": f"independent shards x{world} (no collective)",
-                                                         "path": {1: "general_lsd_radix", 2: "cell_sorted"}.get(last_path, str(last_path))}),
+                                                         "path": {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid"}.get(last_path, str(last_path))}),
             "roofline": roofline, "step_roofline": {"algorithmic_bytes_per_sd_step": step_bytes, "gbs": step_gbs,
                                                     "frac": step_gbs / peak, "peak": peak},
             "kernels": kernels, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
@@ -375,7 +376,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
-    ap.add_argument("--path", default=None, choices=[None, "auto", "general", "cell_sorted"])
+    ap.add_argument("--path", default=None, choices=[None, "auto", "general", "cell_sorted", "hybrid"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

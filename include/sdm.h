@@ -61,15 +61,19 @@ typedef struct {
 /* Path selection for sdm_coalescence_step (sdm_set_path).  Every path produces the same bits.
  *   GENERAL      global stable LSD radix sort of (cell_id, Philox key): north_star (b).  Any input.
  *   CELL_SORTED  per-cell register-resident sort fused with the pair kernel.  Legal
- *                only when cell_id is non-decreasing and no cell holds more than 256 super-droplets; the
- *                kernel checks both on the device: on a violation the step is NOT applied and the
- *                sticky SDM_ERR_BAD_DATA flag is set.
+ *                only when cell_id is non-decreasing and no cell holds more than 256 super-droplets.
+ *   HYBRID       LSD radix passes over the cell_id digits only (grouping the indices by cell), then the same
+ *                fused per-cell sort + pair kernel, gathering through the sorted indices.  Any order of
+ *                cell_id; legal when n_cell > 1 and no cell holds more than 256 super-droplets.
+ *                CELL_SORTED and HYBRID verify their preconditions on the device BEFORE anything is updated:
+ *                on a violation the step is NOT applied and the sticky SDM_ERR_BAD_DATA flag is set.
  *   AUTO         (default) the first step on a given (cell_id pointer, n_sd, n_cell) takes GENERAL, which
  *                also records whether the array is sorted and its largest cell; later steps on the same
- *                triple take CELL_SORTED when that verdict allows it.  If cell_id was then modified in
- *                place so that the verdict no longer holds, the device check above catches it (step
- *                skipped, SDM_ERR_BAD_DATA at the next poll, verdict reset). */
-typedef enum { SDM_PATH_AUTO = 0, SDM_PATH_GENERAL = 1, SDM_PATH_CELL_SORTED = 2 } sdm_path;
+ *                triple take CELL_SORTED or HYBRID when that verdict allows it.  If cell_id was then
+ *                modified in place so that the verdict no longer holds, the device check above catches it
+ *                (step skipped, SDM_ERR_BAD_DATA at the next poll, verdict reset).  Calling sdm_set_path()
+ *                -- with any value -- also resets the verdict: do so after rewriting cell_id in place. */
+typedef enum { SDM_PATH_AUTO = 0, SDM_PATH_GENERAL = 1, SDM_PATH_CELL_SORTED = 2, SDM_PATH_HYBRID = 3 } sdm_path;
 
 /* Bytes of device workspace sdm_init() needs for problems up to (max_n_sd, max_n_cell).
  * Returns 0 when the arguments are invalid (max_n_sd < 0, max_n_sd >= 2^30, max_n_cell < 1). */
@@ -132,6 +136,12 @@ int sdm_debug_outputs(sdm_ctx* ctx, int32_t* perm_out, int64_t* gamma_out, int64
  * unknown value. */
 int sdm_set_path(sdm_ctx* ctx, int path);
 
+/* Test / tuning knobs.  SDM_OPT_NARROW_KEY_BITS: number of Philox-key bits (1..24, default 24) kept in the
+ * 32-bit sort word of the fused per-cell kernel; fewer bits make its exact wide-word redo frequent (tests).
+ * The result never depends on it.  Returns INVALID_ARG for an unknown option or value. */
+enum { SDM_OPT_NARROW_KEY_BITS = 0 };
+int sdm_set_option(sdm_ctx* ctx, int option, int64_t value);
+
 /* Which path the most recent sdm_coalescence_step took (an sdm_path value other than AUTO), or 0 if
  * none ran yet.  Synchronises the stream when the decision was taken on the device. */
 int sdm_last_path(sdm_ctx* ctx);
@@ -162,7 +172,7 @@ int64_t sdm_launch_count(sdm_ctx* ctx);
  * host) since the last read, and resets the accumulation. */
 enum { SDM_PROF_KEYS_HIST = 0, SDM_PROF_CELL_SCAN, SDM_PROF_RADIX_PASS, SDM_PROF_PAIR, SDM_PROF_COUNT_ZERO,
        SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CELL_BOUNDS, SDM_PROF_CELL_FUSED,
-       SDM_PROF_CLASSES };
+       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_CLASSES };
 int sdm_profile_enable(sdm_ctx* ctx, int on);
 int sdm_profile_read(sdm_ctx* ctx, double* ms_out /* host */, int64_t* launches_out /* host */);
 

@@ -11,6 +11,8 @@ from .binding import (  # noqa: F401
     PATH_AUTO,
     PATH_CELL_SORTED,
     PATH_GENERAL,
+    PATH_HYBRID,
+    OPT_NARROW_KEY_BITS,
     KernelParams,
     SDMContext,
     SDMError,
@@ -24,6 +26,6 @@ from .binding import (  # noqa: F401
 
 __all__ = [
     "SDMContext", "SDMError", "KernelParams", "golovin", "geometric", "GOLOVIN", "GEOMETRIC",
-    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "workspace_bytes", "host_staging_bytes",
+    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "OPT_NARROW_KEY_BITS", "workspace_bytes", "host_staging_bytes",
     "load_library", "library_path",
 ]

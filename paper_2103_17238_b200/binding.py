@@ -16,6 +16,8 @@ GEOMETRIC = 1
 PATH_AUTO = 0
 PATH_GENERAL = 1
 PATH_CELL_SORTED = 2
+PATH_HYBRID = 3
+OPT_NARROW_KEY_BITS = 0
 
 SDM_OK = 0
 
@@ -24,11 +26,11 @@ EXPORTS = [
     "sdm_cell_stats", "sdm_debug_outputs", "sdm_set_path", "sdm_last_path", "sdm_host_staging_bytes",
     "sdm_bind_host_staging", "sdm_coalescence_step_host", "sdm_poll_error", "sdm_launch_count",
     "sdm_philox_fill", "sdm_kernel_eval", "sdm_strerror", "sdm_destroy", "sdm_profile_enable",
-    "sdm_profile_read",
+    "sdm_profile_read", "sdm_set_option",
 ]
 
 PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
-                "cell_bounds", "cell_fused"]
+                "cell_bounds", "cell_fused", "cell_digit_hist"]
 
 
 class SDMError(RuntimeError):
@@ -81,6 +83,8 @@ def load_library():
     lib.sdm_debug_outputs.restype = C.c_int
     lib.sdm_set_path.argtypes = [vp, C.c_int]
     lib.sdm_set_path.restype = C.c_int
+    lib.sdm_set_option.argtypes = [vp, C.c_int, i64]
+    lib.sdm_set_option.restype = C.c_int
     lib.sdm_last_path.argtypes = [vp]
     lib.sdm_last_path.restype = C.c_int
     lib.sdm_host_staging_bytes.argtypes = [i64]
@@ -240,6 +244,9 @@ class SDMContext:
 
     def set_path(self, path: int):
         _check(self._lib.sdm_set_path(self._h, int(path)), "sdm_set_path")
+
+    def set_option(self, option: int, value: int):
+        _check(self._lib.sdm_set_option(self._h, int(option), int(value)), "sdm_set_option")
 
     def last_path(self) -> int:
         return int(self._lib.sdm_last_path(self._h))

@@ -58,6 +58,9 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     return w;
 }
 
+// hybrid words: (cell_id << idxbits | index) in 64 bits, and pass 0 stages (cell_id << 12 | tile-local index)
+static bool hybrid_fits(const Plan& p) { return p.cbits >= 1 && p.cbits + p.idxbits <= 64 && p.cbits + 12 <= 64; }
+
 static bool sizes_ok(int64_t max_n_sd, int32_t max_n_cell) {
     return max_n_sd >= 0 && max_n_sd < (1LL << 30) && max_n_cell >= 1;
 }
@@ -113,6 +116,7 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
     ctx->max_n_cell = max_n_cell;
     ctx->ws = carve_workspace(workspace_dev, max_n_sd, max_n_cell);
     ctx->path = SDM_PATH_AUTO;
+    ctx->narrow_key_bits = 24;
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms <= 0) {
         free_ctx(ctx);
@@ -171,9 +175,19 @@ const char* sdm_strerror(int status) {
 }
 
 int sdm_set_path(sdm_ctx* ctx, int path) {
-    if (!ctx || path < SDM_PATH_AUTO || path > SDM_PATH_CELL_SORTED) return SDM_ERR_INVALID_ARG;
+    if (!ctx || path < SDM_PATH_AUTO || path > SDM_PATH_HYBRID) return SDM_ERR_INVALID_ARG;
     ctx->path = path;
+    ctx->verdict_valid = 0;  // AUTO re-learns the cell order on its next step
     return SDM_OK;
+}
+
+int sdm_set_option(sdm_ctx* ctx, int option, int64_t value) {
+    if (!ctx) return SDM_ERR_INVALID_ARG;
+    if (option == SDM_OPT_NARROW_KEY_BITS && value >= 1 && value <= 24) {
+        ctx->narrow_key_bits = (int)value;
+        return SDM_OK;
+    }
+    return SDM_ERR_INVALID_ARG;
 }
 
 int sdm_last_path(sdm_ctx* ctx) { return ctx ? ctx->last_path : 0; }
@@ -236,21 +250,47 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
     const double dtdV = dt / dV;
 
     // ---- path selection (include/sdm.h, sdm_path) ----
-    bool fast = false;
+    int path = SDM_PATH_GENERAL;
     if (n_cell > 1) {
-        if (ctx->path == SDM_PATH_CELL_SORTED) {
-            fast = true;
+        if (ctx->path == SDM_PATH_CELL_SORTED || ctx->path == SDM_PATH_HYBRID) {
+            path = ctx->path;
         } else if (ctx->path == SDM_PATH_AUTO && ctx->verdict_valid && ctx->verdict_cell_ptr == cell_id &&
                    ctx->verdict_n_sd == n_sd && ctx->verdict_n_cell == n_cell &&
                    cudaEventQuery(ctx->verdict_event) == cudaSuccess) {
-            fast = ctx->verdict_host->unsorted == 0 && ctx->verdict_host->max_count <= (u32)CELL_FAST_MAX;
+            if (ctx->verdict_host->max_count <= (u32)CELL_FAST_MAX)
+                path = ctx->verdict_host->unsorted ? SDM_PATH_HYBRID : SDM_PATH_CELL_SORTED;
         }
     }
-    if (fast) {
+    if (path == SDM_PATH_HYBRID && !hybrid_fits(plan)) path = SDM_PATH_GENERAL;
+    if (path == SDM_PATH_CELL_SORTED) {
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, CTL_WORDS * 4, st)))) return rc;
-        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, multiplicity, volume, cell_id, n_sd, n_cell, dtdV, dkp, pk))))
+        if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, 0, cell_id, n_sd, n_cell, 0)))) return rc;
+        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, 0, nullptr, 0, multiplicity, volume, n_sd, n_cell, dtdV, dkp, pk))))
             return rc;
         ctx->last_path = SDM_PATH_CELL_SORTED;
+        return SDM_OK;
+    }
+    if (path == SDM_PATH_HYBRID) {
+        const int n_cpass = plan.n_pass - 4;
+        const bool narrow = plan.cbits + plan.idxbits <= 32 && plan.cbits + 12 <= 32;
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)n_cpass * plan.n_tiles * RADIX * 4, st))))
+            return rc;
+        if ((rc = note_cuda(ctx, launch_cell_digit_hist(ctx, cell_id, n_sd, n_cell, plan)))) return rc;
+        void* in = nullptr;
+        void* out = ws.buf_a;
+        for (int pass = 0; pass < n_cpass; ++pass) {
+            if ((rc = note_cuda(ctx, launch_cell_sort_pass(ctx, pass, narrow, cell_id, in, out, n_sd, n_cell, plan))))
+                return rc;
+            in = out;
+            out = (out == (void*)ws.buf_a) ? (void*)ws.buf_b : (void*)ws.buf_a;
+        }
+        const int kind = narrow ? 2 : 1;
+        if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, kind, in, n_sd, n_cell, plan.idxbits)))) return rc;
+        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, kind, in, plan.idxbits, multiplicity, volume, n_sd, n_cell, dtdV,
+                                                   dkp, pk))))
+            return rc;
+        ctx->last_path = SDM_PATH_HYBRID;
         return SDM_OK;
     }
 

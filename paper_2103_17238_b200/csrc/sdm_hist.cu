@@ -160,6 +160,59 @@ k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, in
     }
 }
 
+// Hybrid path: histograms of the cell_id digits alone (no Philox keys, no per-cell counts): reads cell_id
+// once (4 B/SD).  Digit q of cell_id lands in digit_hist[(4 + q) * RADIX ...] (after the four key digits).
+constexpr int CDH_ITEMS = 4;
+
+__global__ void __launch_bounds__(HIST_BLOCK)
+k_cell_digit_hist(const int32_t* __restrict__ cell_id, u32 n_sd, int n_cell, int n_cpass, int vec_ok,
+                  u32* __restrict__ digit_hist, u32* __restrict__ sticky) {
+    __shared__ u32 s_hist[4][RADIX];
+    const int tid = threadIdx.x;
+    for (int q = tid; q < 4 * RADIX; q += HIST_BLOCK) (&s_hist[0][0])[q] = 0;
+    __syncthreads();
+    bool bad = false;
+    const u32 chunk = HIST_BLOCK * CDH_ITEMS;
+    for (u32 base = blockIdx.x * chunk; base < n_sd; base += gridDim.x * chunk) {
+        const u32 i0 = base + tid * CDH_ITEMS;
+        int c[CDH_ITEMS];
+        if (vec_ok && i0 + CDH_ITEMS <= n_sd) {
+            const int4 v = __ldg(reinterpret_cast<const int4*>(cell_id + i0));
+            c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
+        } else {
+#pragma unroll
+            for (int k = 0; k < CDH_ITEMS; ++k) c[k] = (i0 + k < n_sd) ? __ldg(cell_id + i0 + k) : -1;
+        }
+#pragma unroll
+        for (int k = 0; k < CDH_ITEMS; ++k) {
+            if (i0 + k < n_sd) {
+                int cc = c[k];
+                if (cc < 0 || cc >= n_cell) { bad = true; cc = cc < 0 ? 0 : n_cell - 1; }
+                for (int q = 0; q < n_cpass; ++q) atomicAdd(&s_hist[q][((u32)cc >> (8 * q)) & 0xFFu], 1u);
+            }
+        }
+    }
+    __syncthreads();
+    for (int q = tid; q < n_cpass * RADIX; q += HIST_BLOCK) {
+        const u32 h = (&s_hist[0][0])[q];
+        if (h) atomicAdd(&digit_hist[4 * RADIX + q], h);
+    }
+    if (bad) sticky[STICKY_BAD_DATA] = 1u;
+}
+
+cudaError_t launch_cell_digit_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
+                                   const Plan& plan) {
+    const long long chunk = (long long)HIST_BLOCK * CDH_ITEMS;
+    long long n_chunks = (n_sd + chunk - 1) / chunk;
+    int grid = (int)(n_chunks < (long long)ctx->sm_count * 8 ? n_chunks : (long long)ctx->sm_count * 8);
+    if (grid < 1) grid = 1;
+    const int vec_ok = (reinterpret_cast<uintptr_t>(cell_id) & 15u) == 0;
+    LaunchScope scope(ctx, PROF_CELL_DIGIT_HIST);
+    k_cell_digit_hist<<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, (u32)n_sd, n_cell, plan.n_pass - 4, vec_ok,
+                                                            ctx->ws.digit_hist, ctx->ws.sticky);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
                              const Plan& plan, const PhiloxKeys& pk, u64* sortkey_out) {
     const long long chunk = (long long)HIST_BLOCK * HIST_ROUNDS;

@@ -68,7 +68,7 @@ struct Plan {  // per-step derived quantities
 namespace sdm {
 // Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
 enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
-                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CLASSES };
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_CLASSES };
 // What the last general-path step learned about the cell_id array (pinned host memory, written by an
 // asynchronous copy; valid once `verdict_event` has completed).
 struct Verdict { u32 unsorted; u32 max_count; };
@@ -95,6 +95,7 @@ struct sdm_ctx {
     void* staging;
     size_t staging_bytes;
     int sm_count;
+    int narrow_key_bits;  // key bits kept in the fused kernel's 32-bit sort word (SDM_OPT_NARROW_KEY_BITS)
     // optional per-launch CUDA-event timing (sdm_profile_enable)
     int profiling;
     std::vector<sdm::ProfEvent>* prof_events;
@@ -145,8 +146,15 @@ cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, in
 cudaError_t launch_pair(sdm_ctx* ctx, const u64* sorted, int64_t* xi, double* v, int64_t n_sd,
                         int32_t n_cell, const Plan& plan, double dtdV, const KernelParams& kp,
                         const PhiloxKeys& pk);
-cudaError_t launch_cell_fused(sdm_ctx* ctx, int64_t* xi, double* v, const int32_t* cell_id, int64_t n_sd,
-                              int32_t n_cell, double dtdV, const KernelParams& kp, const PhiloxKeys& pk);
+cudaError_t launch_cell_sort_pass(sdm_ctx* ctx, int pass, bool narrow, const int32_t* cell_id, const void* in,
+                                  void* out, int64_t n_sd, int32_t n_cell, const Plan& plan);
+cudaError_t launch_cell_digit_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
+                                   const Plan& plan);
+cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
+                               int idxbits);
+cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int64_t* xi, double* v,
+                              int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
+                              const PhiloxKeys& pk);
 cudaError_t launch_debug_perm(sdm_ctx* ctx, const u64* sorted, int64_t n_sd, const Plan& plan);
 cudaError_t launch_count_zero(sdm_ctx* ctx, const int64_t* xi, int64_t n_sd);
 cudaError_t launch_compact(sdm_ctx* ctx, int64_t* xi, double* v, int32_t* cell_id, int64_t n_sd);

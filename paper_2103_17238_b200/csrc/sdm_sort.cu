@@ -1,18 +1,22 @@
-// Row a3 of SURVEY.md section 8(a): the per-cell shuffle as a stable LSD radix sort of
-// (cell_id << 32 | Philox key), 8-bit digits, one kernel launch per digit ("Onesweep" structure:
-// the digit histograms of ALL passes were built up-front by k_keys_hist, so each pass reads its
-// input once and scatters it once; the global offsets travel between tiles by decoupled look-back).
+// Row a3 of SURVEY.md section 8(a): stable LSD radix sort passes, 8-bit digits, one launch per digit
+// ("Onesweep" structure: the digit histograms of ALL passes are built up-front -- k_keys_hist for the
+// general path, k_cell_digit_hist for the hybrid path -- so each pass reads its input once and scatters
+// it once; the global offsets travel between tiles by decoupled look-back).
 //
-// Element format.  Pass 1 reads sortkey = (cell_id << 32 | key) (48 significant bits) with the
-// super-droplet index implicit in the position, and writes
-//      packed = ((sortkey >> 8) << idxbits) | index              (needs 40 + cbits-16.. <= 64 bits)
-// every later pass reads and writes `packed`, taking its digit at bit idxbits + 8 (pass - 1).
-// One 8-byte word per element per pass: a single LDG.64 / STS.64 / LDS.64 / STG.64 per element.
+// Three element flows share one kernel template:
+//   MODE_KEY_FIRST   general path, pass 0.  in: u64 sortkey = (cell_id << 32 | Philox key), index implicit
+//                    in the position.  out: packed = ((sortkey >> 8) << idxbits) | index.
+//   MODE_CELL_FIRST  hybrid path, pass 0.  in: int32 cell_id, index implicit.  out: (cell_id << idxbits) | index
+//                    in a u64 or (when it fits) u32 word.
+//   MODE_LATER       every later pass: reads and writes the same word, digit at `shift`.
+// One word per element per pass: a single LDG / STS / LDS / STG per element.
 //
 // Stability (required: ties between equal keys must keep index order, R4): within a tile
 // the elements are ranked warp by warp in load order -- warp w owns the contiguous slab
-// [w*32*ITEMS, (w+1)*32*ITEMS), round k covers 32 consecutive elements -- with
-// __match_any_sync peer masks; ranks follow (warp, round, lane) = memory order.
+// [w*32*ITEMS, (w+1)*32*ITEMS), round k covers 32 consecutive elements.  The peers of a lane (lanes of
+// the same round with the same digit) come from eight ballots, one per digit bit: fixed-latency work
+// that pipelines across the 16 rounds, unlike MATCH.ANY, whose cost grows with the number of distinct
+// digits in the warp (profiles/r1a_README.md).  Ranks follow (warp, round, lane) = memory order.
 #include "sdm_internal.h"
 
 namespace sdm {
@@ -24,6 +28,8 @@ constexpr int SORT_WARPS = SORT_BLOCK / 32;
 constexpr int SORT_TILE_BITS = 12;
 static_assert((1 << SORT_TILE_BITS) == SORT_TILE, "tile-local index width");
 static_assert(SORT_BLOCK == RADIX, "one thread per digit");
+
+enum { MODE_KEY_FIRST = 0, MODE_CELL_FIRST = 1, MODE_LATER = 2 };
 
 // Block-wide exclusive scan of one value per thread (SORT_BLOCK == RADIX threads).
 __device__ __forceinline__ u32 block_excl_scan_256(u32 x, u32* s_warp /*[8]*/, int lane, int warp) {
@@ -43,12 +49,23 @@ __device__ __forceinline__ u32 block_excl_scan_256(u32 x, u32* s_warp /*[8]*/, i
     return woff + incl - x;
 }
 
-template <bool FIRST>
-__global__ void __launch_bounds__(SORT_BLOCK, 3)
-k_radix_pass(const u64* __restrict__ in, u64* __restrict__ out, u32 n_sd, int shift, int idxbits,
+template <typename T>
+__device__ __forceinline__ T ld_stream(const T* p);
+template <>
+__device__ __forceinline__ u64 ld_stream<u64>(const u64* p) { return ld_stream_u64(p); }
+template <>
+__device__ __forceinline__ u32 ld_stream<u32>(const u32* p) {
+    u32 v;
+    asm volatile("ld.global.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+
+template <typename TIn, typename TW, int MODE>
+__global__ void __launch_bounds__(SORT_BLOCK, 4)
+k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shift, int idxbits, int n_cell,
              const u32* __restrict__ ghist /*[RADIX] global histogram of this digit*/,
              u32* __restrict__ ticket, u32* __restrict__ tile_state /*[n_tiles][RADIX]*/) {
-    __shared__ u64 s_stage[SORT_TILE];
+    __shared__ TW s_stage[SORT_TILE];
     __shared__ u32 s_whist[SORT_WARPS][RADIX];
     __shared__ u32 s_goff[RADIX];
     __shared__ u32 s_warp[SORT_WARPS];
@@ -62,37 +79,55 @@ k_radix_pass(const u64* __restrict__ in, u64* __restrict__ out, u32 n_sd, int sh
     const u32 tile = s_tile;
     const u32 base = tile * (u32)SORT_TILE;
     const u32 n_valid = min((u32)SORT_TILE, n_sd - base);
+    const int dshift = (MODE == MODE_LATER) ? shift : SORT_TILE_BITS;  // where the digit sits in the staged word
 
     // ---- load (warp-striped: round k of warp w = 32 consecutive elements) ----
-    u64 item[SORT_ITEMS];
+    TW item[SORT_ITEMS];
     const u32 wbase = warp * 32u * SORT_ITEMS + lane;
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
         const u32 off = wbase + k * 32u;
-        u64 x = ~0ull;  // out-of-range elements sort to the end of the last tile (digit 255)
+        TW x = (TW)~(TW)0;  // out-of-range elements sort to the end of the last tile (digit 255)
         if (off < n_valid) {
-            x = ld_stream_u64(in + base + off);
-            if (FIRST) x = (x << SORT_TILE_BITS) | (u64)off;  // tile-local index below the sort key
+            if constexpr (MODE == MODE_CELL_FIRST) {
+                int c = (int)ld_stream<u32>(reinterpret_cast<const u32*>(in) + base + off);
+                c = c < 0 ? 0 : (c >= n_cell ? n_cell - 1 : c);  // bad data was flagged by the histogram kernel
+                x = ((TW)(u32)c << SORT_TILE_BITS) | (TW)off;
+            } else if constexpr (MODE == MODE_KEY_FIRST) {
+                x = ((TW)ld_stream<TIn>(in + base + off) << SORT_TILE_BITS) | (TW)off;  // tile-local index below the key
+            } else {
+                x = (TW)ld_stream<TIn>(in + base + off);
+            }
         }
         item[k] = x;
     }
 
-    // ---- rank within the warp, round by round (stable) ----
-    u32 rank[SORT_ITEMS];
+    // ---- peers of every element inside its round: 8 ballots per round, all rounds independent ----
+    u32 info[SORT_ITEMS];  // [4:0] lanes before me with my digit, [13:8] lanes with my digit (1..32)
     const u32 lt = lanemask_lt();
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
-        const u32 d = (u32)(item[k] >> shift) & 0xFFu;
-        const u32 peers = __match_any_sync(0xffffffffu, d);
-        const u32 pre = __popc(peers & lt);
-        u32 old = 0;
-        if (pre == 0) {
-            old = s_whist[warp][d];
-            s_whist[warp][d] = old + __popc(peers);
+        const u32 d = (u32)(item[k] >> dshift) & 0xFFu;
+        u32 peers = 0xffffffffu;
+#pragma unroll
+        for (int b = 0; b < RADIX_BITS; ++b) {
+            const bool bit = (d >> b) & 1u;
+            const u32 m = __ballot_sync(0xffffffffu, bit);
+            peers &= bit ? m : ~m;
         }
-        old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
-        rank[k] = old + pre;
+        info[k] = __popc(peers & lt) | (__popc(peers) << 8);
+    }
+
+    // ---- running per-warp digit counters: every lane reads the counter, the first peer advances it ----
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        const u32 d = (u32)(item[k] >> dshift) & 0xFFu;
+        const u32 pre = info[k] & 0xFFu;
+        const u32 old = s_whist[warp][d];
         __syncwarp();
+        if (pre == 0) s_whist[warp][d] = old + (info[k] >> 8);
+        __syncwarp();
+        info[k] = old + pre;  // rank among this warp's elements with digit d
     }
     __syncthreads();
 
@@ -116,8 +151,8 @@ k_radix_pass(const u64* __restrict__ in, u64* __restrict__ out, u32 n_sd, int sh
     // ---- stage in shared memory in sorted order ----
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
-        const u32 d = (u32)(item[k] >> shift) & 0xFFu;
-        s_stage[s_whist[warp][d] + rank[k]] = item[k];
+        const u32 d = (u32)(item[k] >> dshift) & 0xFFu;
+        s_stage[s_whist[warp][d] + info[k]] = item[k];
     }
 
     // ---- decoupled look-back: global position of this tile's first element of digit d ----
@@ -145,17 +180,21 @@ k_radix_pass(const u64* __restrict__ in, u64* __restrict__ out, u32 n_sd, int sh
     for (int j = 0; j < SORT_ITEMS; ++j) {
         const u32 p = j * SORT_BLOCK + tid;
         if (p < n_valid) {
-            u64 x = s_stage[p];
-            const u32 d = (u32)(x >> shift) & 0xFFu;
-            if (FIRST) {
-                const u64 idx = (u64)base + (x & (u64)(SORT_TILE - 1));
+            TW x = s_stage[p];
+            const u32 d = (u32)(x >> dshift) & 0xFFu;
+            if (MODE == MODE_KEY_FIRST) {
+                const TW idx = (TW)base + (x & (TW)(SORT_TILE - 1));
                 x = ((x >> (SORT_TILE_BITS + 8)) << idxbits) | idx;  // drop digit 0, append the global index
+            } else if (MODE == MODE_CELL_FIRST) {
+                const TW idx = (TW)base + (x & (TW)(SORT_TILE - 1));
+                x = ((x >> SORT_TILE_BITS) << idxbits) | idx;  // keep the whole cell_id above the global index
             }
             out[s_goff[d] + p] = x;
         }
     }
 }
 
+// General path (north_star (b)): pass 0 reads the 8-byte sort keys, later passes the packed words.
 cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, int64_t n_sd,
                              const Plan& plan) {
     u32* ticket = ctx->ws.ctl + CTL_TICKET0 + pass;
@@ -163,12 +202,41 @@ cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, in
     const u32* ghist = ctx->ws.digit_hist + pass * RADIX;
     LaunchScope scope(ctx, PROF_RADIX_PASS);
     if (pass == 0) {
-        k_radix_pass<true><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(in, out, (u32)n_sd, SORT_TILE_BITS, plan.idxbits,
-                                                                          ghist, ticket, state);
+        k_radix_pass<u64, u64, MODE_KEY_FIRST><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(
+            in, out, (u32)n_sd, 0, plan.idxbits, 0, ghist, ticket, state);
     } else {
         const int shift = plan.idxbits + 8 * (pass - 1);
-        k_radix_pass<false><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(in, out, (u32)n_sd, shift,
-                                                                           plan.idxbits, ghist, ticket, state);
+        k_radix_pass<u64, u64, MODE_LATER><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(
+            in, out, (u32)n_sd, shift, plan.idxbits, 0, ghist, ticket, state);
+    }
+    return cudaGetLastError();
+}
+
+// Hybrid path: LSD passes over the cell_id digits only; words are (cell_id << idxbits | index).
+// `narrow` selects 4-byte words (legal when cbits + idxbits <= 32 and cbits + 12 <= 32).
+cudaError_t launch_cell_sort_pass(sdm_ctx* ctx, int pass, bool narrow, const int32_t* cell_id, const void* in,
+                                  void* out, int64_t n_sd, int32_t n_cell, const Plan& plan) {
+    u32* ticket = ctx->ws.ctl + CTL_TICKET0 + pass;
+    u32* state = ctx->ws.tile_state + (size_t)pass * (size_t)plan.n_tiles * RADIX;
+    const u32* ghist = ctx->ws.digit_hist + (4 + pass) * RADIX;  // cell digits live after the four key digits
+    LaunchScope scope(ctx, PROF_RADIX_PASS);
+    const int shift = plan.idxbits + 8 * pass;
+    if (narrow) {
+        if (pass == 0)
+            k_radix_pass<int32_t, u32, MODE_CELL_FIRST><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(
+                cell_id, reinterpret_cast<u32*>(out), (u32)n_sd, 0, plan.idxbits, n_cell, ghist, ticket, state);
+        else
+            k_radix_pass<u32, u32, MODE_LATER><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(
+                reinterpret_cast<const u32*>(in), reinterpret_cast<u32*>(out), (u32)n_sd, shift, plan.idxbits, n_cell,
+                ghist, ticket, state);
+    } else {
+        if (pass == 0)
+            k_radix_pass<int32_t, u64, MODE_CELL_FIRST><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(
+                cell_id, reinterpret_cast<u64*>(out), (u32)n_sd, 0, plan.idxbits, n_cell, ghist, ticket, state);
+        else
+            k_radix_pass<u64, u64, MODE_LATER><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(
+                reinterpret_cast<const u64*>(in), reinterpret_cast<u64*>(out), (u32)n_sd, shift, plan.idxbits, n_cell,
+                ghist, ticket, state);
     }
     return cudaGetLastError();
 }

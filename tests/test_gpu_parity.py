@@ -51,7 +51,7 @@ def _assert_vol_close(got, want, what=""):
     assert rel.max(initial=0.0) <= VOL_RTOL, f"{what}: max rel volume error {rel.max()}"
 
 
-def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False):
+def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key_bits=None, expect_last_path=None):
     """Steps the oracle and the GPU side by side over w.n_steps steps, comparing after every step."""
     sdm = _sdm()
     ow = w.copy()
@@ -59,6 +59,8 @@ def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False):
     with sdm.SDMContext(max(n, 1), w.n_cell, device=dev) as ctx:
         if path is not None:
             ctx.set_path(path)
+        if narrow_key_bits is not None:
+            ctx.set_option(sdm.OPT_NARROW_KEY_BITS, narrow_key_bits)
         xi, v, cell = _to_dev(w, dev)
         dbg = ctx.debug_outputs(n, w.n_cell) if check_debug else None
         okp, gkp = _okp(w), _gkp(w)
@@ -92,6 +94,8 @@ def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False):
                 assert np.array_equal(xi[:n].cpu().numpy(), ow.xi[:n])
                 assert np.array_equal(cell[:n].cpu().numpy(), ow.cell_id[:n])
                 _assert_vol_close(v[:n].cpu().numpy(), ow.v[:n], f"after compaction {s}")
+        if expect_last_path is not None:
+            assert ctx.last_path() == expect_last_path
         return stats
 
 
@@ -167,6 +171,59 @@ def test_small_configs_cell_sorted_path(dev, name):
         assert st["clamped"] > 0 and st["removed"] > 0
 
 
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg3z", "cfg4", "cfg4s"])
+@pytest.mark.parametrize("interleave", [True, False])
+def test_small_configs_hybrid_path(dev, name, interleave):
+    """cell-digit LSD passes + fused per-cell sort/pair kernel: any order of cell_id, same bits as the oracle."""
+    sdm = _sdm()
+    st = _run_parity(W.small(name, interleave=interleave), dev, path=sdm.PATH_HYBRID, bit_exact=True,
+                     expect_last_path=sdm.PATH_HYBRID)
+    if name == "cfg4s":
+        assert st["clamped"] > 0 and st["removed"] > 0
+
+
+@pytest.mark.parametrize("path", ["cell_sorted", "hybrid"])
+@pytest.mark.parametrize("bits", [1, 5, 12])
+def test_fused_kernel_wide_redo(dev, path, bits):
+    """With only a few key bits in the 32-bit sort word nearly every cell has neighbours whose truncated keys
+    tie, so the exact 64-bit redo runs all the time; the result must not change."""
+    sdm = _sdm()
+    if path == "cell_sorted":
+        _run_parity(W.small("cfg4"), dev, path=sdm.PATH_CELL_SORTED, bit_exact=True, narrow_key_bits=bits)
+    else:
+        _run_parity(W.small("cfg3", interleave=True), dev, path=sdm.PATH_HYBRID, bit_exact=True, narrow_key_bits=bits)
+
+
+@pytest.mark.parametrize("n,n_cell", [(5000, 257), (9000, 70_000), (4096, 4096), (300, 1_000_000), (3000, 2)])
+def test_hybrid_cell_count_extremes(dev, n, n_cell):
+    """one more than a digit, more cells than SDs, 17+ and 20 cell bits (8-byte words), one cell digit"""
+    sdm = _sdm()
+    rng = np.random.default_rng(n_cell + 1)
+    cell = rng.integers(0, n_cell, n).astype(np.int32)
+    if n_cell == 2:                                   # 200 + 256 SDs: the largest legal cell, one cell digit
+        cell = np.concatenate([np.zeros(200, np.int32), np.ones(256, np.int32)])
+        rng.shuffle(cell)
+        n = len(cell)
+    xi = rng.integers(1, 1000, n).astype(np.int64)
+    xi[rng.random(n) < 0.2] = 77
+    v = rng.integers(1, 9, n).astype(np.float64)
+    w = W.Workload("edge", xi, v, cell, n_cell, 1.0, 1.0, W.GOLOVIN, 2.0 ** -10, 0.0, 3, 2)
+    _run_parity(w, dev, path=sdm.PATH_HYBRID, bit_exact=True, expect_last_path=sdm.PATH_HYBRID)
+
+
+def test_hybrid_path_refuses_large_cells(dev):
+    """a cell of more than 256 SDs: the device check skips the whole step and reports it"""
+    sdm = _sdm()
+    w = W.cfg3(n_cell=8, per_cell=300, n_steps=1, interleave=True)
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        before = xi.clone(), v.clone()
+        ctx.set_path(sdm.PATH_HYBRID)
+        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), 42, 0)
+        assert ctx.poll_error() == -4
+        assert torch.equal(xi, before[0]) and torch.equal(v, before[1])
+
+
 @pytest.mark.parametrize("per_cell", [1, 2, 3, 31, 32, 33, 63, 64, 65, 127, 129, 255, 256])
 def test_cell_sorted_path_cell_sizes(dev, per_cell):
     """every register-tile width of the per-cell sort, at and around its boundaries, plus empty cells"""
@@ -196,13 +253,13 @@ def test_auto_path_switches_to_cell_sorted(dev):
         torch.cuda.synchronize()
         ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 1)
         assert ctx.last_path() == sdm.PATH_CELL_SORTED      # verdict: sorted, cells <= 256
-        # an interleaved array never leaves the general path
+        # an interleaved array with small cells: general once, then the hybrid path
         wi = W.small("cfg3", interleave=True)
         xi2, v2, cell2 = _to_dev(wi, dev)
         for s in range(3):
             ctx.coalescence_step(xi2, v2, cell2, wi.n_cell, wi.dt, wi.dV, kp, 42, s)
             torch.cuda.synchronize()
-            assert ctx.last_path() == sdm.PATH_GENERAL
+            assert ctx.last_path() == (sdm.PATH_GENERAL if s == 0 else sdm.PATH_HYBRID)
         # cells larger than the fast path's limit: general path
         big = W.cfg3(n_cell=8, per_cell=300, n_steps=3)
         xb, vb, cb = _to_dev(big, dev)
