@@ -220,6 +220,8 @@ def run_ours(args):
     if args.path:
         ctx.set_path({"auto": sdm.PATH_AUTO, "general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED,
                       "hybrid": sdm.PATH_HYBRID}[args.path])
+    if not args.no_track_zeros:
+        ctx.set_option(sdm.OPT_TRACK_ZEROS, 1)  # a5 fused into a4 (include/sdm.h): bench never writes xi in between
     stream = torch.cuda.current_stream(dev)
 
     def one_step(s, n):
@@ -310,8 +312,13 @@ def run_ours(args):
                     "frac": kernels[dom]["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
                     "ms_per_launch": kernels[dom]["ms_per_launch"], "launches": kernels[dom]["launches"],
                     "algorithmic_bytes_per_launch": kernels[dom]["algorithmic_bytes_per_launch"]}
-    step_bytes = ab["_step_total"] + (8 if w.compact_every == 1 else 0)
-    step_gbs = step_bytes * (sd_steps / args.steps) / (elapsed_ms / args.steps * 1e-3) / 1e9
+    # bytes the executed path must move per SD-step = sum of its kernels' algorithmic bytes; next to it the
+    # figure SURVEY 8(d) quotes for north_star's own pass structure (general LSD path + separate zero scan)
+    step_bytes = sum(ab.get(nm, 0) * k["launches"] for nm, k in kernels.items()) / max(args.steps, 1)
+    ns_bytes = ab["_step_total"] + (8 if w.compact_every == 1 else 0)
+    sd_per_s = (sd_steps / args.steps) / (elapsed_ms / args.steps * 1e-3)
+    step_gbs = step_bytes * sd_per_s / 1e9
+    ns_gbs = ns_bytes * sd_per_s / 1e9
 
     # ---- e2e: HOST buffers through the C ABI, copies inside the timed region ----
     e2e = None
@@ -357,9 +364,13 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "ours",
             "config": workload_config(w, args.workload, {"parallelism": f"independent shards x{world} (no collective)",
-                                                         "path": {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid"}.get(last_path, str(last_path))}),
+                                                         "path": {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid"}.get(last_path, str(last_path)),
+                                                         "track_zeros": not args.no_track_zeros}),
             "roofline": roofline, "step_roofline": {"algorithmic_bytes_per_sd_step": step_bytes, "gbs": step_gbs,
-                                                    "frac": step_gbs / peak, "peak": peak},
+                                                    "frac": step_gbs / peak, "peak": peak,
+                                                    "north_star_bytes_per_sd_step": ns_bytes,
+                                                    "north_star_equivalent_gbs": ns_gbs,
+                                                    "north_star_equivalent_frac": ns_gbs / peak},
             "kernels": kernels, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
             "ms_per_step_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
         }
@@ -378,6 +389,7 @@ def main():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--path", default=None, choices=[None, "auto", "general", "cell_sorted", "hybrid"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-track-zeros", action="store_true", help="keep the separate zero-count kernel (a5)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

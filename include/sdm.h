@@ -138,8 +138,16 @@ int sdm_set_path(sdm_ctx* ctx, int path);
 
 /* Test / tuning knobs.  SDM_OPT_NARROW_KEY_BITS: number of Philox-key bits (1..24, default 24) kept in the
  * 32-bit sort word of the fused per-cell kernel; fewer bits make its exact wide-word redo frequent (tests).
- * The result never depends on it.  Returns INVALID_ARG for an unknown option or value. */
-enum { SDM_OPT_NARROW_KEY_BITS = 0 };
+ * The result never depends on it.
+ * SDM_OPT_TRACK_ZEROS (0 / 1, default 0): row a5 fused into row a4.  When 1, the fused per-cell kernel
+ * (CELL_SORTED and HYBRID paths) also counts, exactly, the zero multiplicities the array holds after the
+ * step (it reads every multiplicity anyway), and a sdm_remove_zero_multiplicity call on the same
+ * (multiplicity pointer, n_sd) that DIRECTLY follows that step on this context reads the count instead
+ * of scanning the array again.  Contract: between the two calls the caller does not write the
+ * multiplicity array (if it does, it sets the option again, which drops the stored count).  The GENERAL
+ * path, a refused step and any other call order fall back to the counting kernel; results are identical.
+ * Returns INVALID_ARG for an unknown option or value. */
+enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1 };
 int sdm_set_option(sdm_ctx* ctx, int option, int64_t value);
 
 /* Which path the most recent sdm_coalescence_step took (an sdm_path value other than AUTO), or 0 if

@@ -18,6 +18,7 @@ PATH_GENERAL = 1
 PATH_CELL_SORTED = 2
 PATH_HYBRID = 3
 OPT_NARROW_KEY_BITS = 0
+OPT_TRACK_ZEROS = 1
 
 SDM_OK = 0
 

@@ -71,6 +71,13 @@ static int note_cuda(sdm_ctx* ctx, cudaError_t e) {
     return SDM_ERR_CUDA;
 }
 
+// The fused kernels leave the post-step number of zero multiplicities in ctl[CTL_ZERO_COUNT].
+static void note_zero_hint(sdm_ctx* ctx, const void* xi, int64_t n_sd) {
+    ctx->zero_hint_valid = ctx->track_zeros;
+    ctx->zero_hint_xi = xi;
+    ctx->zero_hint_n_sd = n_sd;
+}
+
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 }  // namespace sdm
@@ -187,6 +194,11 @@ int sdm_set_option(sdm_ctx* ctx, int option, int64_t value) {
         ctx->narrow_key_bits = (int)value;
         return SDM_OK;
     }
+    if (option == SDM_OPT_TRACK_ZEROS && (value == 0 || value == 1)) {
+        ctx->track_zeros = (int)value;
+        ctx->zero_hint_valid = 0;
+        return SDM_OK;
+    }
     return SDM_ERR_INVALID_ARG;
 }
 
@@ -262,12 +274,21 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         }
     }
     if (path == SDM_PATH_HYBRID && !hybrid_fits(plan)) path = SDM_PATH_GENERAL;
+    // register tile of the fused kernel: 32 * rmax >= the largest cell (known from the verdict under AUTO)
+    int rmax = CELL_FAST_MAX / 32;
+    if (ctx->path == SDM_PATH_AUTO && path != SDM_PATH_GENERAL) {
+        const u32 mc = ctx->verdict_host->max_count;
+        rmax = mc <= 64 ? 2 : (mc <= 128 ? 4 : 8);
+    }
+    ctx->zero_hint_valid = 0;
     if (path == SDM_PATH_CELL_SORTED) {
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, CTL_WORDS * 4, st)))) return rc;
-        if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, 0, cell_id, n_sd, n_cell, 0)))) return rc;
-        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, 0, nullptr, 0, multiplicity, volume, n_sd, n_cell, dtdV, dkp, pk))))
+        if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, 0, cell_id, n_sd, n_cell, 0, rmax)))) return rc;
+        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, 0, nullptr, 0, rmax, multiplicity, volume, n_sd, n_cell, dtdV, dkp,
+                                                   pk))))
             return rc;
         ctx->last_path = SDM_PATH_CELL_SORTED;
+        note_zero_hint(ctx, multiplicity, n_sd);
         return SDM_OK;
     }
     if (path == SDM_PATH_HYBRID) {
@@ -286,11 +307,12 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
             out = (out == (void*)ws.buf_a) ? (void*)ws.buf_b : (void*)ws.buf_a;
         }
         const int kind = narrow ? 2 : 1;
-        if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, kind, in, n_sd, n_cell, plan.idxbits)))) return rc;
-        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, kind, in, plan.idxbits, multiplicity, volume, n_sd, n_cell, dtdV,
-                                                   dkp, pk))))
+        if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, kind, in, n_sd, n_cell, plan.idxbits, rmax)))) return rc;
+        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, kind, in, plan.idxbits, rmax, multiplicity, volume, n_sd, n_cell,
+                                                   dtdV, dkp, pk))))
             return rc;
         ctx->last_path = SDM_PATH_HYBRID;
+        note_zero_hint(ctx, multiplicity, n_sd);
         return SDM_OK;
     }
 
@@ -344,18 +366,32 @@ int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* vo
     *n_sd_out = n_sd;
     int rc;
     cudaStream_t st = ctx->stream;
-    u32 host_words[2] = {0, 0};  // [0] zero count, [1] sticky bad-data flag
-    if (n_sd > 0) {
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_CMP_TICKET, 0, 8, st)))) return rc;
-        if ((rc = note_cuda(ctx, launch_count_zero(ctx, multiplicity, n_sd)))) return rc;
-        if ((rc = note_cuda(ctx, cudaMemcpyAsync(&host_words[0], ctx->ws.ctl + CTL_ZERO_COUNT, 4,
+    u32 host_words[3] = {0, 0, 0};  // [0] zero count, [1] sticky bad-data flag, [2] "the fused step was skipped"
+    // SDM_OPT_TRACK_ZEROS: the fused step kernel that just updated this very array counted its zeros
+    bool hinted = ctx->zero_hint_valid && ctx->zero_hint_xi == multiplicity && ctx->zero_hint_n_sd == n_sd && n_sd > 0;
+    ctx->zero_hint_valid = 0;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        if (n_sd > 0) {
+            if (hinted) {
+                if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_CMP_TICKET, 0, 4, st)))) return rc;
+                if ((rc = note_cuda(ctx, cudaMemcpyAsync(&host_words[2], ctx->ws.ctl + CTL_UNSORTED, 4,
+                                                         cudaMemcpyDeviceToHost, st))))
+                    return rc;
+            } else {
+                if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_CMP_TICKET, 0, 8, st)))) return rc;
+                if ((rc = note_cuda(ctx, launch_count_zero(ctx, multiplicity, n_sd)))) return rc;
+            }
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(&host_words[0], ctx->ws.ctl + CTL_ZERO_COUNT, 4,
+                                                     cudaMemcpyDeviceToHost, st))))
+                return rc;
+        }
+        if ((rc = note_cuda(ctx, cudaMemcpyAsync(&host_words[1], ctx->ws.sticky + STICKY_BAD_DATA, 4,
                                                  cudaMemcpyDeviceToHost, st))))
             return rc;
+        if ((rc = note_cuda(ctx, cudaStreamSynchronize(st)))) return rc;
+        if (!(hinted && host_words[2])) break;
+        hinted = false;  // the step refused its input and counted nothing: count now
     }
-    if ((rc = note_cuda(ctx, cudaMemcpyAsync(&host_words[1], ctx->ws.sticky + STICKY_BAD_DATA, 4,
-                                             cudaMemcpyDeviceToHost, st))))
-        return rc;
-    if ((rc = note_cuda(ctx, cudaStreamSynchronize(st)))) return rc;
     const int64_t zeros = host_words[0];
     if (zeros > 0) {
         const size_t n_tiles = (size_t)((n_sd + CMP_TILE - 1) / CMP_TILE);

@@ -22,14 +22,16 @@
 
 namespace sdm {
 
-constexpr int CF_BLOCK = 256;
-constexpr int CF_WARPS = CF_BLOCK / 32;
+constexpr int CF_WARPS = 4;
+constexpr int CF_BLOCK = CF_WARPS * 32;
 constexpr int CB_BLOCK = 256;
-constexpr int CB_ITEMS = 4;
+constexpr int CB_ITEMS = 8;
 
 // ---------------------------------------------------------------------------------------------
 // Cell boundaries of an array whose cells are contiguous.  SRC = 0: cell_id int32[n];
 // SRC = 1: sorted words u64 (cell << idxbits | index);  SRC = 2: the same in u32 words.
+// Eight positions per thread, read with 16-byte loads (VEC; the scalar instantiation serves a
+// misaligned cell_id); the cell-size check re-reads position i - max_cell the same way (L2 hits).
 // ---------------------------------------------------------------------------------------------
 template <int SRC>
 __device__ __forceinline__ int cell_at(const void* src, u32 i, int idxbits) {
@@ -38,21 +40,44 @@ __device__ __forceinline__ int cell_at(const void* src, u32 i, int idxbits) {
     return (int)(__ldg(reinterpret_cast<const u32*>(src) + i) >> idxbits);
 }
 
-template <int SRC>
+template <int SRC, bool VEC>
+__device__ __forceinline__ void cells_at8(const void* src, u32 i0, u32 n_sd, int idxbits, int (&c)[CB_ITEMS]) {
+    if (VEC && i0 + CB_ITEMS <= n_sd) {  // i0 is a multiple of 8 and the base is 16-byte aligned
+        if (SRC == 1) {
+            const ulonglong2* p = reinterpret_cast<const ulonglong2*>(reinterpret_cast<const u64*>(src) + i0);
+#pragma unroll
+            for (int q = 0; q < CB_ITEMS / 2; ++q) {
+                const ulonglong2 w = __ldg(p + q);
+                c[2 * q] = (int)(w.x >> idxbits);
+                c[2 * q + 1] = (int)(w.y >> idxbits);
+            }
+        } else {
+            const uint4* p = reinterpret_cast<const uint4*>(reinterpret_cast<const u32*>(src) + i0);
+#pragma unroll
+            for (int q = 0; q < CB_ITEMS / 4; ++q) {
+                const uint4 w = __ldg(p + q);
+                c[4 * q] = (int)(w.x >> idxbits);      // SRC = 0: idxbits = 0, the word is the cell_id itself
+                c[4 * q + 1] = (int)(w.y >> idxbits);
+                c[4 * q + 2] = (int)(w.z >> idxbits);
+                c[4 * q + 3] = (int)(w.w >> idxbits);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < CB_ITEMS; ++k) c[k] = (i0 + k < n_sd) ? cell_at<SRC>(src, i0 + k, idxbits) : 0x7fffffff;
+    }
+}
+
+template <int SRC, bool VEC>
 __global__ void __launch_bounds__(CB_BLOCK)
 k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32 max_cell,
               u32* __restrict__ cell_start, u32* __restrict__ ctl, u32* __restrict__ sticky,
               int32_t* __restrict__ dbg_cell_start) {
     const u32 i0 = (blockIdx.x * CB_BLOCK + threadIdx.x) * CB_ITEMS;  // lanes past the end stay for the shuffle
-    int c[CB_ITEMS];
-    const bool full = i0 + CB_ITEMS <= n_sd;
-    if (full && SRC == 0) {  // n_sd-independent alignment: the launcher guarantees 16-byte alignment
-        const int4 q = __ldg(reinterpret_cast<const int4*>(reinterpret_cast<const int*>(src) + i0));
-        c[0] = q.x; c[1] = q.y; c[2] = q.z; c[3] = q.w;
-    } else {
-#pragma unroll
-        for (int k = 0; k < CB_ITEMS; ++k) c[k] = (i0 + k < n_sd) ? cell_at<SRC>(src, i0 + k, idxbits) : 0x7fffffff;
-    }
+    int c[CB_ITEMS], back[CB_ITEMS];
+    cells_at8<SRC, VEC>(src, i0, n_sd, idxbits, c);
+    const bool has_back = i0 >= max_cell && i0 < n_sd;  // max_cell is a multiple of 8: same alignment as i0
+    if (has_back) cells_at8<SRC, VEC>(src, i0 - max_cell, n_sd, idxbits, back);
     int prev = __shfl_up_sync(0xffffffffu, c[CB_ITEMS - 1], 1);
     if ((threadIdx.x & 31) == 0) prev = (i0 == 0 || i0 > n_sd) ? -1 : cell_at<SRC>(src, i0 - 1, idxbits);
     bool bad = false;
@@ -65,10 +90,12 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
                 bad = true;
             } else {
                 // a cell larger than the fused kernel's register tile: position i - max_cell is in it too
-                if (i >= max_cell && cell_at<SRC>(src, i - max_cell, idxbits) == cc) bad = true;
-                for (int q = prev + 1; q <= cc; ++q) {  // i opens cell cc and every empty cell before it
-                    cell_start[q] = i;
-                    if (dbg_cell_start) dbg_cell_start[q] = (int32_t)i;
+                if (has_back && back[k] == cc) bad = true;
+                if (cc != prev) {
+                    for (int q = prev + 1; q <= cc; ++q) {  // i opens cell cc and every empty cell before it
+                        cell_start[q] = i;
+                        if (dbg_cell_start) dbg_cell_start[q] = (int32_t)i;
+                    }
                 }
                 if (i == n_sd - 1) {
                     for (int q = cc + 1; q <= n_cell; ++q) {
@@ -155,7 +182,7 @@ struct FusedArgs {
     u64 idx_mask;
     int32_t* dbg_perm;
     u32* sticky;
-    const u32* ctl;
+    u32* ctl;
 };
 
 // Original array index of position e of the run that starts at `start`.
@@ -166,45 +193,68 @@ __device__ __forceinline__ u32 run_index(const FusedArgs& a, u32 start, u32 e) {
     return __ldg(reinterpret_cast<const u32*>(a.run_idx) + start + e) & (u32)a.idx_mask;
 }
 
-// Applies the pair rule to the sorted run: sorted slot s = lane*R + r holds run position pos[r].
-template <int WORD, int R>
-__device__ __forceinline__ void collide_sorted(const FusedArgs& a, u32 start, u32 n_c, int lane, const u32 (&pos)[R]) {
-    if (a.dbg_perm) {
+// Per-warp staging of one cell in shared memory, indexed by the position e in the run: the attributes
+// are loaded ONCE, coalesced, before the (ALU-bound) key generation and sort, so the HBM latency hides
+// under them; the pair phase then reads its two members by sorted position from shared memory.
+template <int WORD, int RMAX>
+struct CellStage {
+    longlong2 xv[32 * RMAX];  // (multiplicity, volume bits)
+    uint2 uw[32 * RMAX];      // Philox words 2, 3 of the SD (its uniform, used if it lands on an even slot)
+    u32 key[32 * RMAX];       // full Philox permutation key (wide redo only)
+    u32 idx[WORD == 0 ? 1 : 32 * RMAX];  // HYBRID: original index
+};
+
+template <int R>
+__device__ __forceinline__ u32 select_reg(const u32 (&x)[R], int i) {
+    u32 v = x[0];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const u32 s = lane * R + r;
-            if (s < n_c) a.dbg_perm[start + s] = (int32_t)run_index<WORD>(a, start, pos[r]);
-        }
-    }
-    if (R >= 2) {
-#pragma unroll
-        for (int r = 0; r + 1 < R; r += 2) {
-            const u32 s = lane * R + r;
-            if (s + 1 < n_c)
-                pair_collide<false>(a.pair, run_index<WORD>(a, start, pos[r]), run_index<WORD>(a, start, pos[r + 1]), n_c);
-        }
-    } else {
-        const u32 nxt = __shfl_down_sync(0xffffffffu, pos[0], 1);
-        if ((lane & 1) == 0 && (u32)lane + 1 < n_c)
-            pair_collide<false>(a.pair, run_index<WORD>(a, start, pos[0]), run_index<WORD>(a, start, nxt), n_c);
-    }
+    for (int r = 1; r < R; ++r)
+        if (i == r) v = x[r];
+    return v;
 }
 
-template <int WORD, int R>
-__device__ __forceinline__ void warp_cell(const FusedArgs& a, u32 start, u32 n_c, int lane) {
-    u32 key[R];
+// One warp, one cell of 2 <= n_c <= 32 R super-droplets (n_c = 1 only counts its zero).  Returns this
+// lane's share of the number of zero multiplicities the cell holds AFTER the step.
+template <int WORD, int RMAX, int R>
+__device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMAX>& st, u32 start, u32 n_c, int lane) {
+    static_assert(R <= RMAX, "register tile within the staging tile");
+    const PairArgs& pa = a.pair;
+    u32 zeros = 0;
+    // ---- a1 + load: striped positions e = 32 r + lane (coalesced), everything parked in shared memory ----
+    u32 idx[R];
+    long long xi[R];
+    double vol[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const u32 e = 32u * r + lane;
+        idx[r] = 0; xi[r] = 1; vol[r] = 0.0;
+        if (e < n_c) {
+            idx[r] = run_index<WORD>(a, start, e);
+            xi[r] = pa.xi[idx[r]];
+            vol[r] = pa.v[idx[r]];
+        }
+    }
     u32 x[R];
     const int drop = 32 - a.key_bits;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const u32 e = lane * R + r;
-        key[r] = 0;
-        x[r] = 0xFFFFFFFFu;  // padding sorts to the end (a real word ends in e < n_c <= 255 when its key is all ones)
+        const u32 e = 32u * r + lane;
+        x[r] = 0xFFFFFFFFu;  // padding sorts to the end
         if (e < n_c) {
-            key[r] = philox_perm_key(a.pair.pk, (u64)run_index<WORD>(a, start, e));
-            x[r] = ((key[r] >> drop) << 8) | e;
+            zeros += (xi[r] == 0);
+            const PhiloxOut w = philox4x32_10(pa.pk, (u64)idx[r]);
+            st.xv[e] = make_longlong2(xi[r], __double_as_longlong(vol[r]));
+            st.uw[e] = make_uint2(w.w2, w.w3);
+            st.key[e] = w.w0;
+            if (WORD != 0) st.idx[e] = idx[r];
+            x[r] = ((w.w0 >> drop) << 8) | e;
         }
     }
+    if (n_c < 2) {
+        if (a.dbg_perm && lane == 0) a.dbg_perm[start] = (int32_t)idx[0];
+        return zeros;
+    }
+    // ---- a3: sort (truncated key, position) words; slot s = lane R + r afterwards ----
     warp_bitonic_sort<u32, R>(x, lane);
     // neighbours with equal truncated keys: their order is decided by the dropped bits -> wide redo
     bool tie = false;
@@ -212,13 +262,14 @@ __device__ __forceinline__ void warp_cell(const FusedArgs& a, u32 start, u32 n_c
     for (int r = 0; r + 1 < R; ++r) tie |= (((x[r] ^ x[r + 1]) >> 8) == 0) && ((u32)(lane * R + r + 1) < n_c);
     const u32 nxt = __shfl_down_sync(0xffffffffu, x[0], 1);
     tie |= (lane < 31) && (((x[R - 1] ^ nxt) >> 8) == 0) && ((u32)(lane * R + R) < n_c);
+    __syncwarp();  // the staging writes of all lanes are visible from here on
     u32 pos[R];
     if (__any_sync(0xffffffffu, tie)) {
         u64 wide[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const u32 e = lane * R + r;
-            wide[r] = (e < n_c) ? (((u64)key[r] << 32) | (u64)e) : ~0ull;
+        for (int r = 0; r < R; ++r) {  // the real words occupy the first n_c slots of the narrow result
+            const u32 e = x[r] & 0xFFu;
+            wide[r] = ((u32)(lane * R + r) < n_c) ? (((u64)st.key[e] << 32) | (u64)e) : ~0ull;
         }
         warp_bitonic_sort<u64, R>(wide, lane);
 #pragma unroll
@@ -227,53 +278,123 @@ __device__ __forceinline__ void warp_cell(const FusedArgs& a, u32 start, u32 n_c
 #pragma unroll
         for (int r = 0; r < R; ++r) pos[r] = x[r] & 0xFFu;
     }
-    collide_sorted<WORD, R>(a, start, n_c, lane, pos);
+    if (a.dbg_perm) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const u32 s = lane * R + r;
+            if (s < n_c) a.dbg_perm[start + s] = (int32_t)(WORD == 0 ? start + pos[r] : st.idx[pos[r]]);
+        }
+    }
+    // ---- a4, phase A: every pair of neighbouring slots -- can its gamma be non-zero? ----
+    constexpr int NP = (R >= 2) ? R / 2 : 1;
+    u32 first[NP], second[NP];  // run positions of the pair's members, in shuffled order
+    u32 need = 0;               // bit q: pair q of this lane must run the full rule
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        bool valid;
+        if (R >= 2) {
+            first[q] = pos[2 * q];
+            second[q] = pos[(2 * q + 1) % R];
+            valid = (u32)(lane * R + 2 * q + 1) < n_c;
+        } else {
+            first[q] = pos[0];
+            second[q] = __shfl_down_sync(0xffffffffu, pos[0], 1);
+            valid = ((lane & 1) == 0) && ((u32)lane + 1u < n_c);
+        }
+        if (valid) {
+            if (pa.dbg_gamma) {
+                need |= 1u << q;
+            } else {
+                const longlong2 A = st.xv[first[q]], B = st.xv[second[q]];
+                if (A.x != 0 && B.x != 0) {  // a dead partner: gamma~ = 0 whatever gamma is (R7)
+                    const bool swap = A.x < B.x;
+                    const uint2 w = st.uw[first[q]];
+                    const double vA = __longlong_as_double(A.y), vB = __longlong_as_double(B.y);
+                    if (pair_may_collide(pa, swap ? B.x : A.x, swap ? vB : vA, swap ? vA : vB, w.x, w.y, n_c))
+                        need |= 1u << q;
+                }
+            }
+        }
+    }
+    // ---- phase B: the full fp64 rule, only where needed; lanes take their pending pairs one at a time ----
+    while (__any_sync(0xffffffffu, need != 0)) {
+        if (need) {
+            const int q = __ffs(need) - 1;
+            need &= need - 1u;
+            const u32 ea = select_reg<NP>(first, q), eb = select_reg<NP>(second, q);
+            const longlong2 A = st.xv[ea], B = st.xv[eb];
+            const uint2 w = st.uw[ea];
+            const u32 ja = (WORD == 0) ? start + ea : st.idx[ea];
+            const u32 jb = (WORD == 0) ? start + eb : st.idx[eb];
+            zeros += pair_apply(pa, ja, jb, A.x, __longlong_as_double(A.y), B.x, __longlong_as_double(B.y), w.x, w.y, n_c);
+        }
+    }
+    return zeros;
 }
 
-template <int WORD>
+template <int WORD, int RMAX>
 __global__ void __launch_bounds__(CF_BLOCK) k_cell_fused(const FusedArgs a) {
+    __shared__ CellStage<WORD, RMAX> s_stage[CF_WARPS];
     if (a.ctl[CTL_UNSORTED]) return;  // k_cell_bounds refused the input: the step is skipped as a whole
-    const int lane = threadIdx.x & 31;
-    const int c = blockIdx.x * CF_WARPS + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c = blockIdx.x * CF_WARPS + warp;
     if (c >= a.n_cell) return;
     const u32 start = __ldg(a.pair.cell_start + c);
     const u32 n_c = __ldg(a.pair.cell_start + c + 1) - start;
-    if (n_c < 2) {
-        if (n_c == 1 && a.dbg_perm && lane == 0) a.dbg_perm[start] = (int32_t)run_index<WORD>(a, start, 0);
-        return;
+    if (n_c == 0) return;
+    CellStage<WORD, RMAX>& st = s_stage[warp];
+    u32 zeros = 0;
+    if (n_c <= 32) {
+        zeros = warp_cell<WORD, RMAX, 1>(a, st, start, n_c, lane);
+    } else if (RMAX >= 2 && n_c <= 64) {
+        if constexpr (RMAX >= 2) zeros = warp_cell<WORD, RMAX, 2>(a, st, start, n_c, lane);
+    } else if (RMAX >= 4 && n_c <= 128) {
+        if constexpr (RMAX >= 4) zeros = warp_cell<WORD, RMAX, 4>(a, st, start, n_c, lane);
+    } else if (RMAX >= 8 && n_c <= 256) {
+        if constexpr (RMAX >= 8) zeros = warp_cell<WORD, RMAX, 8>(a, st, start, n_c, lane);
+    } else if (lane == 0) {
+        a.sticky[STICKY_BAD_DATA] = 1u;  // unreachable: k_cell_bounds refuses such cells
     }
-    if (n_c <= 32) warp_cell<WORD, 1>(a, start, n_c, lane);
-    else if (n_c <= 64) warp_cell<WORD, 2>(a, start, n_c, lane);
-    else if (n_c <= 128) warp_cell<WORD, 4>(a, start, n_c, lane);
-    else if (n_c <= CELL_FAST_MAX) warp_cell<WORD, 8>(a, start, n_c, lane);
-    else if (lane == 0) a.sticky[STICKY_BAD_DATA] = 1u;  // unreachable: k_cell_bounds refuses such cells
+    // a5, fused: the number of zero multiplicities after the step (sdm_remove_zero_multiplicity reads it)
+    zeros = __reduce_add_sync(0xffffffffu, zeros);
+    if (lane == 0 && zeros) atomicAdd(a.ctl + CTL_ZERO_COUNT, zeros);
 }
 
-// src_kind: 0 = cell_id array itself (CELL_SORTED), 1 = u64 sorted words, 2 = u32 sorted words (HYBRID)
+// src_kind: 0 = cell_id array itself (CELL_SORTED), 1 = u64 sorted words, 2 = u32 sorted words (HYBRID).
+// max_cell = 32 * rmax: the largest cell the fused kernel launched next can hold.
 cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
-                               int idxbits) {
+                               int idxbits, int rmax) {
     const u32 grid = (u32)((n_sd + CB_BLOCK * CB_ITEMS - 1) / (CB_BLOCK * CB_ITEMS));
+    const u32 max_cell = 32u * (u32)rmax;
     LaunchScope scope(ctx, PROF_CELL_BOUNDS);
     Workspace& ws = ctx->ws;
+    const bool vec = (reinterpret_cast<uintptr_t>(src) & 15u) == 0;
+#define SDM_BOUNDS(SRC, VEC, IDXBITS)                                                                       \
+    k_cell_bounds<SRC, VEC><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, IDXBITS, max_cell, \
+                                                                ws.cell_start, ws.ctl, ws.sticky, ctx->dbg_cell_start)
     if (src_kind == 0) {
-        if ((reinterpret_cast<uintptr_t>(src) & 15u) == 0)
-            k_cell_bounds<0><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, 0, (u32)CELL_FAST_MAX,
-                                                                ws.cell_start, ws.ctl, ws.sticky, ctx->dbg_cell_start);
-        else  // misaligned cell_id: the scalar-load instantiation (SRC = 2 reads 4-byte words, idxbits = 0)
-            k_cell_bounds<2><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, 0, (u32)CELL_FAST_MAX,
-                                                                ws.cell_start, ws.ctl, ws.sticky, ctx->dbg_cell_start);
+        if (vec) SDM_BOUNDS(0, true, 0);
+        else SDM_BOUNDS(0, false, 0);
     } else if (src_kind == 1) {
-        k_cell_bounds<1><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, idxbits, (u32)CELL_FAST_MAX,
-                                                            ws.cell_start, ws.ctl, ws.sticky, ctx->dbg_cell_start);
+        if (vec) SDM_BOUNDS(1, true, idxbits);
+        else SDM_BOUNDS(1, false, idxbits);
     } else {
-        k_cell_bounds<2><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, idxbits, (u32)CELL_FAST_MAX,
-                                                            ws.cell_start, ws.ctl, ws.sticky, ctx->dbg_cell_start);
+        if (vec) SDM_BOUNDS(2, true, idxbits);
+        else SDM_BOUNDS(2, false, idxbits);
     }
+#undef SDM_BOUNDS
     return cudaGetLastError();
 }
 
-cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int64_t* xi, double* v,
-                              int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
+template <int WORD>
+static void launch_fused_word(const FusedArgs& a, int rmax, u32 grid, cudaStream_t st) {
+    if (rmax <= 2) k_cell_fused<WORD, 2><<<grid, CF_BLOCK, 0, st>>>(a);
+    else if (rmax <= 4) k_cell_fused<WORD, 4><<<grid, CF_BLOCK, 0, st>>>(a);
+    else k_cell_fused<WORD, 8><<<grid, CF_BLOCK, 0, st>>>(a);
+}
+
+cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int rmax, int64_t* xi,
+                              double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
                               const PhiloxKeys& pk) {
     FusedArgs a;
     a.pair.sorted = nullptr;
@@ -286,6 +407,7 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.pair.single_cell = 0;
     a.pair.dtdV = dtdV;
     a.pair.kp = kp;
+    set_bound_constants(a.pair);
     a.pair.pk = pk;
     a.pair.dbg_gamma = reinterpret_cast<long long*>(ctx->dbg_gamma);
     a.pair.dbg_gamma_clamped = reinterpret_cast<long long*>(ctx->dbg_gamma_clamped);
@@ -298,9 +420,9 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.ctl = ctx->ws.ctl;
     const u32 grid = (u32)((n_cell + CF_WARPS - 1) / CF_WARPS);
     LaunchScope scope(ctx, PROF_CELL_FUSED);
-    if (src_kind == 0) k_cell_fused<0><<<grid, CF_BLOCK, 0, ctx->stream>>>(a);
-    else if (src_kind == 1) k_cell_fused<1><<<grid, CF_BLOCK, 0, ctx->stream>>>(a);
-    else k_cell_fused<2><<<grid, CF_BLOCK, 0, ctx->stream>>>(a);
+    if (src_kind == 0) launch_fused_word<0>(a, rmax, grid, ctx->stream);
+    else if (src_kind == 1) launch_fused_word<1>(a, rmax, grid, ctx->stream);
+    else launch_fused_word<2>(a, rmax, grid, ctx->stream);
     return cudaGetLastError();
 }
 

@@ -103,6 +103,11 @@ struct sdm_ctx {
     // AUTO path selection: verdict of the last general-path step about (cell_id pointer, n_sd, n_cell)
     sdm::Verdict* verdict_host;  // pinned
     cudaEvent_t verdict_event;
+    // zero-multiplicity count left in ctl[CTL_ZERO_COUNT] by the last fused step (SDM_OPT_TRACK_ZEROS)
+    int track_zeros;
+    int zero_hint_valid;
+    const void* zero_hint_xi;
+    int64_t zero_hint_n_sd;
     const void* verdict_cell_ptr;
     int64_t verdict_n_sd;
     int32_t verdict_n_cell;
@@ -151,9 +156,9 @@ cudaError_t launch_cell_sort_pass(sdm_ctx* ctx, int pass, bool narrow, const int
 cudaError_t launch_cell_digit_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
                                    const Plan& plan);
 cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
-                               int idxbits);
-cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int64_t* xi, double* v,
-                              int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
+                               int idxbits, int rmax);
+cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int rmax, int64_t* xi,
+                              double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
                               const PhiloxKeys& pk);
 cudaError_t launch_debug_perm(sdm_ctx* ctx, const u64* sorted, int64_t n_sd, const Plan& plan);
 cudaError_t launch_count_zero(sdm_ctx* ctx, const int64_t* xi, int64_t n_sd);

@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(PAIR_BLOCK) k_pair(const PairArgs a) {
         if (s0 + 2u >= end) return;
         Pf = P1; Pg = a.sorted[s0 + 2u];
     }
-    pair_collide<false>(a, (u32)(Pf & idx_mask), (u32)(Pg & idx_mask), end - start);
+    pair_collide(a, (u32)(Pf & idx_mask), (u32)(Pg & idx_mask), end - start);
 }
 
 __global__ void __launch_bounds__(256) k_debug_perm(const u64* __restrict__ sorted, u32 n_sd, int idxbits,
@@ -81,6 +81,7 @@ cudaError_t launch_pair(sdm_ctx* ctx, const u64* sorted, int64_t* xi, double* v,
     a.single_cell = (n_cell == 1);
     a.dtdV = dtdV;
     a.kp = kp;
+    set_bound_constants(a);
     a.pk = pk;
     a.dbg_gamma = reinterpret_cast<long long*>(ctx->dbg_gamma);
     a.dbg_gamma_clamped = reinterpret_cast<long long*>(ctx->dbg_gamma_clamped);

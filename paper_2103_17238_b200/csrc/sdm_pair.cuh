@@ -3,7 +3,13 @@
 //
 // fp64 discipline: the pair probability and the volume update use __dmul_rn/__dadd_rn in the order
 // ((K * xi_j) * dtdV) * scale and gamma~ * v_j + v_k (R10, R13) -- no FMA contraction.
+//
+// The rule is split in two phases so that a warp can run the cheap one for all of its pairs and the
+// expensive one only where it is needed:
+//   pair_may_collide  exact-or-conservative test "can gamma be non-zero?" (never a false negative)
+//   pair_apply        the whole rule in fp64, exactly as the oracle orders it
 #pragma once
+#include <cmath>
 #include "sdm_internal.h"
 
 namespace sdm {
@@ -18,54 +24,91 @@ struct PairArgs {
     int cshift;  // packed >> cshift = cell_id
     int single_cell;
     double dtdV;
+    float dtdV_up;  // dtdV rounded up to fp32 (bound arithmetic)
+    float Epi_up;   // E * pi rounded up to fp32
     KernelParams kp;
     PhiloxKeys pk;
     long long* dbg_gamma;
     long long* dbg_gamma_clamped;
 };
 
-// Exact early-out for the geometric kernel: an upper bound of the pair probability from a handful of
-// fp32 operations, p_ub >= p (every factor rounded up by far more than its error: K <= E pi (2 r_max)^2
-// max_regime v_t(r_max), since each regime of the fall-speed law is increasing).  When u >= p_ub then
-// p < 1 and not (u < p - floor(p)), i.e. gamma = 0 and nothing changes -- the same result the full fp64
-// evaluation gives, without the two cube roots.  Returns +inf when no bound is available.
-__device__ __forceinline__ double pair_probability_bound(const PairArgs& a, double v_max, long long xj, double scale) {
-    if (a.kp.kind != 1) return __longlong_as_double(0x7FF0000000000000LL);
-    const float vm = __double2float_ru(v_max);
-    if (!(vm > 1e-30f) || !(vm < 1e30f)) return __longlong_as_double(0x7FF0000000000000LL);
-    const float r = __fmul_ru(cbrtf(__fmul_ru(vm, 0.2387325f)), 1.00001f);
-    const float vt = fmaxf(fmaxf(__fmul_ru(1.19e8f, __fmul_ru(r, r)), __fmul_ru(8e3f, r)),
-                           __fmul_ru(2.01e2f, __fsqrt_ru(r)));
-    const float K = __fmul_ru(__fmul_ru(__fmul_ru(4.00001f, __fmul_ru(r, r)), vt), __double2float_ru(a.kp.Epi));
-    return __dmul_ru(__dmul_ru(__dmul_ru(__dmul_ru((double)K, (double)xj), a.dtdV), scale), 1.0001);
+// fp32 constants of the geometric bound, rounded UP on the host (after dtdV and kp are set).
+inline float float_round_up(double x) {
+    float f = (float)x;
+    if ((double)f < x) f = nextafterf(f, INFINITY);
+    return f;
+}
+inline void set_bound_constants(PairArgs& a) {
+    a.dtdV_up = float_round_up(a.dtdV);
+    a.Epi_up = float_round_up(a.kp.Epi);
 }
 
-// HAS_U: the caller already holds the uniform of the first-shuffled member (fused kernel: taken from the
-// Philox block that also gave its permutation key); otherwise it is regenerated here.
-template <bool HAS_U>
-__device__ __forceinline__ void pair_collide(const PairArgs& a, u32 j0, u32 k0, u32 n_c, double u_in = 0.0) {
-    long long xj = a.xi[j0], xk = a.xi[k0];
-    double vj = a.v[j0], vk = a.v[k0];
+// (n_c (n_c - 1) / 2) / floor(n_c / 2) == n_c if odd else n_c - 1   (R9)
+__device__ __forceinline__ u32 pair_scale_int(u32 n_c) { return (n_c & 1u) ? n_c : n_c - 1u; }
+
+// fp32 helpers of the geometric bound.  BOUND_EPS covers every rounding of the fp32 evaluation: the
+// approximate cube root 2^(log2(x)/3) from MUFU.LG2/EX2 (|log2 x| <= 100 inside the guarded range ->
+// relative error < 6e-6), the fp64 -> fp32 conversions and a dozen fp32 roundings (6e-8 each).
+constexpr float BOUND_EPS = 3e-5f;
+
+__device__ __forceinline__ float bound_radius(float v) {  // ~ (3 v / 4 pi)^(1/3), relative error < 1e-5
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(__log2f(v * 0.2387324f) * 0.33333334f));  // MUFU.EX2, 2 ulp
+    return y;
+}
+// R16 in fp32; the fall speed is non-decreasing in r over all three regimes (0.19 -> 0.32 m/s at 40 um,
+// 4.8 -> 4.92 m/s at 600 um), which is what turns radius intervals into fall-speed intervals.
+__device__ __forceinline__ float bound_fall_speed(float r) {
+    if (r < 40e-6f) return 1.19e8f * (r * r);
+    if (r < 600e-6f) return 8e3f * r;
+    return 2.01e2f * sqrtf(r);
+}
+
+// Conservative test: returns false only when gamma = 0 is certain (then the pair changes nothing and,
+// without debug outputs, needs no further work).  xj >= xk, (vj, vk) follow that order.
+//   Golovin: the exact fp64 probability is five operations, so the test is exact:
+//            gamma != 0  <=>  p >= 1  or  u < p            (p < 1 => floor(p) = 0, p - 0 = p)
+//   geometric: an upper bound p_ub >= p from ~30 fp32 operations on radius / fall-speed INTERVALS
+//            [r(1-eps), r(1+eps)]: K <= E pi (r_j+ + r_k+)^2 max(vt_j+ - vt_k-, vt_k+ - vt_j-).
+//            u >= p_ub (compared through a lower bound of u) => p < 1 and not (u < p) => gamma = 0.
+__device__ __forceinline__ bool pair_may_collide(const PairArgs& a, long long xj, double vj, double vk, u32 w2, u32 w3,
+                                                 u32 n_c) {
+    if (a.kp.kind == 0) {
+        const double K = __dmul_rn(a.kp.b, __dadd_rn(vj, vk));
+        const double p = __dmul_rn(__dmul_rn(__dmul_rn(K, (double)xj), a.dtdV), (double)pair_scale_int(n_c));
+        return (p >= 1.0) || (uniform_from_words(w2, w3) < p) || !(p == p);
+    }
+    const float fj = (float)vj, fk = (float)vk;
+    if (!(fj > 1e-30f && fj < 1e30f && fk > 1e-30f && fk < 1e30f)) return true;  // outside the bound's validity
+    const float rj = bound_radius(fj), rk = bound_radius(fk);
+    const float up = 1.0f + BOUND_EPS, dn = 1.0f - BOUND_EPS;
+    const float rj_hi = rj * up, rk_hi = rk * up;
+    const float tj_hi = bound_fall_speed(rj_hi) * up, tj_lo = bound_fall_speed(rj * dn) * dn;
+    const float tk_hi = bound_fall_speed(rk_hi) * up, tk_lo = bound_fall_speed(rk * dn) * dn;
+    const float dvt = fmaxf(tj_hi - tk_lo, tk_hi - tj_lo) * up;
+    const float s = rj_hi + rk_hi;
+    const float K_ub = a.Epi_up * (s * s) * dvt * up;
+    const float p_ub = K_ub * __ll2float_ru(xj) * a.dtdV_up * (float)pair_scale_int(n_c) * up + 1e-30f;
+    const float u_lo = (float)(w3 >> 8) * 0x1.0p-24f;  // exact in fp32, <= u (the low 29 bits are dropped)
+    return !(u_lo >= p_ub);
+}
+
+// The whole rule for one pair, exactly.  (j0, k0) = original indices in shuffled order, (x0, v0) / (x1, v1)
+// their pre-step attributes, (w2, w3) the Philox words of j0's uniform (R2).  Returns the number of
+// super-droplets whose multiplicity became 0 (the split of xi_k = 1, R14).
+__device__ __forceinline__ u32 pair_apply(const PairArgs& a, u32 j0, u32 k0, long long x0, double v0, long long x1,
+                                          double v1, u32 w2, u32 w3, u32 n_c) {
+    long long xj = x0, xk = x1;
+    double vj = v0, vk = v1;
     u32 j = j0, k = k0;
     if (xj < xk) {  // order so that xi_j >= xi_k; ties keep the shuffled order (R8)
-        const long long tx = xj; xj = xk; xk = tx;
-        const double tv = vj; vj = vk; vk = tv;
+        xj = x1; xk = x0;
+        vj = v1; vk = v0;
         j = k0; k = j0;
     }
-    // a dead partner: gamma~ = 0 whatever gamma is (R7); only the debug gamma output needs the probability
-    if (xk == 0 && !a.dbg_gamma) return;
-    double u;
-    if (HAS_U) {
-        u = u_in;
-    } else {
-        const PhiloxOut w = philox4x32_10(a.pk, (u64)j0);  // uniform of the first-shuffled member (R2)
-        u = uniform_from_words(w.w2, w.w3);
-    }
-    // (n_c (n_c - 1) / 2) / floor(n_c / 2) == n_c if odd else n_c - 1   (R9)
-    const double scale = (double)((n_c & 1u) ? n_c : n_c - 1u);
-    if (u >= pair_probability_bound(a, fmax(vj, vk), xj, scale)) return;  // gamma = 0, exactly
+    const double u = uniform_from_words(w2, w3);
     const double K = coalescence_kernel(a.kp, vj, vk);
-    const double p = __dmul_rn(__dmul_rn(__dmul_rn(K, (double)xj), a.dtdV), scale);
+    const double p = __dmul_rn(__dmul_rn(__dmul_rn(K, (double)xj), a.dtdV), (double)pair_scale_int(n_c));
     long long g = 0;
     if (p > 0.0) {
         if (p >= 0x1.0p63) {
@@ -76,6 +119,7 @@ __device__ __forceinline__ void pair_collide(const PairArgs& a, u32 j0, u32 k0, 
         }
     }
     long long gt = 0;
+    u32 new_zeros = 0;
     if (g != 0 && xk != 0) {
         // gamma~ = min(gamma, floor(xi_j / xi_k)); the quotient is >= 1, so gamma == 1 needs no division (R12)
         gt = (g == 1) ? 1 : min(g, xj / xk);
@@ -90,10 +134,26 @@ __device__ __forceinline__ void pair_collide(const PairArgs& a, u32 j0, u32 k0, 
             a.xi[k] = xk - h;
             a.v[j] = vnew;
             a.v[k] = vnew;
+            new_zeros = (h == 0);
         }
     }
     if (a.dbg_gamma) a.dbg_gamma[j0] = g;
     if (a.dbg_gamma_clamped) a.dbg_gamma_clamped[j0] = gt;
+    return new_zeros;
+}
+
+// General pair kernel: gathers the attributes, regenerates j0's Philox block, runs both phases.
+__device__ __forceinline__ void pair_collide(const PairArgs& a, u32 j0, u32 k0, u32 n_c) {
+    const long long x0 = a.xi[j0], x1 = a.xi[k0];
+    const double v0 = a.v[j0], v1 = a.v[k0];
+    // a dead partner: gamma~ = 0 whatever gamma is (R7); only the debug gamma output needs the probability
+    if ((x0 == 0 || x1 == 0) && !a.dbg_gamma) return;
+    const PhiloxOut w = philox4x32_10(a.pk, (u64)j0);  // uniform of the first-shuffled member (R2)
+    const bool swap = x0 < x1;
+    if (!a.dbg_gamma &&
+        !pair_may_collide(a, swap ? x1 : x0, swap ? v1 : v0, swap ? v0 : v1, w.w2, w.w3, n_c))
+        return;
+    pair_apply(a, j0, k0, x0, v0, x1, v1, w.w2, w.w3, n_c);
 }
 
 }  // namespace sdm

@@ -51,7 +51,8 @@ def _assert_vol_close(got, want, what=""):
     assert rel.max(initial=0.0) <= VOL_RTOL, f"{what}: max rel volume error {rel.max()}"
 
 
-def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key_bits=None, expect_last_path=None):
+def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key_bits=None, expect_last_path=None,
+                track_zeros=False):
     """Steps the oracle and the GPU side by side over w.n_steps steps, comparing after every step."""
     sdm = _sdm()
     ow = w.copy()
@@ -61,6 +62,8 @@ def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key
             ctx.set_path(path)
         if narrow_key_bits is not None:
             ctx.set_option(sdm.OPT_NARROW_KEY_BITS, narrow_key_bits)
+        if track_zeros:
+            ctx.set_option(sdm.OPT_TRACK_ZEROS, 1)
         xi, v, cell = _to_dev(w, dev)
         dbg = ctx.debug_outputs(n, w.n_cell) if check_debug else None
         okp, gkp = _okp(w), _gkp(w)
@@ -180,6 +183,34 @@ def test_small_configs_hybrid_path(dev, name, interleave):
                      expect_last_path=sdm.PATH_HYBRID)
     if name == "cfg4s":
         assert st["clamped"] > 0 and st["removed"] > 0
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg3z", "cfg4", "cfg4s"])
+@pytest.mark.parametrize("path", ["general", "cell_sorted", "hybrid"])
+def test_small_configs_without_debug_outputs(dev, name, path):
+    """The launch configuration bench.py times: debug outputs off, so the conservative early-out
+    (pair_may_collide) decides which pairs run the full rule, and the fused kernels count the zeros for
+    the compaction call (SDM_OPT_TRACK_ZEROS).  Same bits as the oracle after every step."""
+    sdm = _sdm()
+    if name == "cfg1" and path != "general":
+        pytest.skip("single cell: general path only")
+    p = {"general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED, "hybrid": sdm.PATH_HYBRID}[path]
+    st = _run_parity(W.small(name, interleave=(path == "hybrid")), dev, path=p, check_debug=False, bit_exact=True,
+                     track_zeros=True)
+    if name in ("cfg3z", "cfg4s"):
+        assert st["removed"] > 0
+
+
+@pytest.mark.parametrize("dV", [400.0, 4.0, 0.04, 4e-4])
+@pytest.mark.parametrize("path", ["general", "cell_sorted"])
+def test_geometric_early_out_is_exact(dev, dV, path):
+    """The fp32 interval bound of the geometric kernel must never hide a collision: cfg3's spectrum with
+    the cell volume scaled so that p runs from << 1 to >> 1, debug outputs off, against the oracle."""
+    sdm = _sdm()
+    w = W.small("cfg3")
+    w.dV = dV
+    p = {"general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED}[path]
+    _run_parity(w, dev, path=p, check_debug=False, bit_exact=True, track_zeros=True)
 
 
 @pytest.mark.parametrize("path", ["cell_sorted", "hybrid"])
