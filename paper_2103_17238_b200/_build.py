@@ -40,12 +40,12 @@ def needs_build() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
-        cmd = [_nvcc(), *NVCC_FLAGS]
+        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("SDM_NVCC_EXTRA", "").split()]
         if verbose:
             cmd += ["-Xptxas", "-v"]
         cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", OUT]
         subprocess.run(cmd, check=True)
-    return OUT
+    return OUT  # SDM_NVCC_EXTRA: extra nvcc flags for tuning experiments (e.g. -DSDM_CF_WARPS=8)
 
 
 if __name__ == "__main__":

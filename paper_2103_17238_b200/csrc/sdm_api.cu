@@ -44,12 +44,15 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
         off = align_up(off + bytes, 256);
         return q;
     };
+    // sticky | ctl are adjacent (256 B each) so that one small D2H copy reports both (STATUS_WORDS)
+    static_assert(STICKY_WORDS * 4 == 256 && CTL_WORDS * 4 == 256, "status block layout");
+    w.sticky = reinterpret_cast<u32*>(take(STICKY_WORDS * 4));
+    const size_t ctl_off = off;
     w.ctl = reinterpret_cast<u32*>(take(CTL_WORDS * 4));
     w.digit_hist = reinterpret_cast<u32*>(take((size_t)MAX_PASSES * RADIX * 4));
-    w.zero_bytes_fixed = off;
+    w.zero_bytes_fixed = off - ctl_off;
     w.cell_count = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 1) * 4));
     w.tile_state = reinterpret_cast<u32*>(take((size_t)MAX_PASSES * max_tiles * RADIX * 4));
-    w.sticky = reinterpret_cast<u32*>(take(STICKY_WORDS * 4));
     w.cell_start = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 2) * 4));
     w.buf_a = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.buf_b = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
@@ -91,6 +94,7 @@ static void free_ctx(sdm_ctx* ctx) {
         delete ctx->prof_events;
     }
     if (ctx->verdict_host) cudaFreeHost(ctx->verdict_host);
+    if (ctx->status_host) cudaFreeHost(ctx->status_host);
     if (ctx->verdict_event) cudaEventDestroy(ctx->verdict_event);
     delete ctx;
 }
@@ -124,6 +128,7 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
     ctx->ws = carve_workspace(workspace_dev, max_n_sd, max_n_cell);
     ctx->path = SDM_PATH_AUTO;
     ctx->narrow_key_bits = 24;
+    ctx->epoch = 2;
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms <= 0) {
         free_ctx(ctx);
@@ -131,6 +136,8 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
     }
     ctx->sm_count = sms;
     if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->verdict_host), sizeof(Verdict), cudaHostAllocDefault) != cudaSuccess ||
+        cudaHostAlloc(reinterpret_cast<void**>(&ctx->status_host), (STICKY_WORDS + CTL_WORDS) * 4, cudaHostAllocDefault) !=
+            cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->verdict_event, cudaEventDisableTiming) != cudaSuccess) {
         free_ctx(ctx);
         return SDM_ERR_CUDA;
@@ -281,8 +288,8 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         rmax = mc <= 64 ? 2 : (mc <= 128 ? 4 : 8);
     }
     ctx->zero_hint_valid = 0;
+    ctx->epoch = ctx->epoch >= 0xFFFFFFF0u ? 2u : ctx->epoch + 1u;
     if (path == SDM_PATH_CELL_SORTED) {
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, CTL_WORDS * 4, st)))) return rc;
         if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, 0, cell_id, n_sd, n_cell, 0, rmax)))) return rc;
         if ((rc = note_cuda(ctx, launch_cell_fused(ctx, 0, nullptr, 0, rmax, multiplicity, volume, n_sd, n_cell, dtdV, dkp,
                                                    pk))))
@@ -366,35 +373,28 @@ int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* vo
     *n_sd_out = n_sd;
     int rc;
     cudaStream_t st = ctx->stream;
-    u32 host_words[3] = {0, 0, 0};  // [0] zero count, [1] sticky bad-data flag, [2] "the fused step was skipped"
+    // one 512-byte copy into pinned memory reports the sticky words [0, 64) and the control block [64, 128)
+    u32* hs = ctx->status_host;
     // SDM_OPT_TRACK_ZEROS: the fused step kernel that just updated this very array counted its zeros
     bool hinted = ctx->zero_hint_valid && ctx->zero_hint_xi == multiplicity && ctx->zero_hint_n_sd == n_sd && n_sd > 0;
     ctx->zero_hint_valid = 0;
     for (int attempt = 0; attempt < 2; ++attempt) {
-        if (n_sd > 0) {
-            if (hinted) {
-                if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_CMP_TICKET, 0, 4, st)))) return rc;
-                if ((rc = note_cuda(ctx, cudaMemcpyAsync(&host_words[2], ctx->ws.ctl + CTL_UNSORTED, 4,
-                                                         cudaMemcpyDeviceToHost, st))))
-                    return rc;
-            } else {
-                if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_CMP_TICKET, 0, 8, st)))) return rc;
-                if ((rc = note_cuda(ctx, launch_count_zero(ctx, multiplicity, n_sd)))) return rc;
-            }
-            if ((rc = note_cuda(ctx, cudaMemcpyAsync(&host_words[0], ctx->ws.ctl + CTL_ZERO_COUNT, 4,
-                                                     cudaMemcpyDeviceToHost, st))))
-                return rc;
+        if (n_sd > 0 && !hinted) {
+            if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_ZERO_COUNT, 0, 4, st)))) return rc;
+            if ((rc = note_cuda(ctx, launch_count_zero(ctx, multiplicity, n_sd)))) return rc;
         }
-        if ((rc = note_cuda(ctx, cudaMemcpyAsync(&host_words[1], ctx->ws.sticky + STICKY_BAD_DATA, 4,
+        if ((rc = note_cuda(ctx, cudaMemcpyAsync(hs, ctx->ws.sticky, (STICKY_WORDS + CTL_WORDS) * 4,
                                                  cudaMemcpyDeviceToHost, st))))
             return rc;
         if ((rc = note_cuda(ctx, cudaStreamSynchronize(st)))) return rc;
-        if (!(hinted && host_words[2])) break;
+        if (!(hinted && hs[STICKY_WORDS + CTL_UNSORTED] == ctx->epoch)) break;
         hinted = false;  // the step refused its input and counted nothing: count now
     }
-    const int64_t zeros = host_words[0];
+    const int64_t zeros = n_sd > 0 ? (int64_t)hs[STICKY_WORDS + CTL_ZERO_COUNT] : 0;
+    const u32 bad_data = hs[STICKY_BAD_DATA];
     if (zeros > 0) {
         const size_t n_tiles = (size_t)((n_sd + CMP_TILE - 1) / CMP_TILE);
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_CMP_TICKET, 0, 4, st)))) return rc;
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.cmp_state, 0, n_tiles * 4, st)))) return rc;
         if ((rc = note_cuda(ctx, launch_compact(ctx, multiplicity, volume, cell_id, n_sd)))) return rc;
     }
@@ -402,7 +402,7 @@ int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* vo
     // stable compaction keeps a sorted cell_id sorted and cannot grow a cell: the verdict carries over
     if (ctx->verdict_valid && ctx->verdict_cell_ptr == cell_id && ctx->verdict_n_sd == n_sd)
         ctx->verdict_n_sd = n_sd - zeros;
-    if (host_words[1]) {
+    if (bad_data) {
         cudaMemsetAsync(ctx->ws.sticky, 0, STICKY_WORDS * 4, st);
         ctx->verdict_valid = 0;
         return SDM_ERR_BAD_DATA;

@@ -24,6 +24,7 @@ namespace sdm {
 
 constexpr int CF_WARPS = 4;
 constexpr int CF_BLOCK = CF_WARPS * 32;
+constexpr int CF_MIN_BLOCKS = 8;  // measured on B200: 8, 10 and 12 resident blocks give 81, 84, 87 us on cfg3
 constexpr int CB_BLOCK = 256;
 constexpr int CB_ITEMS = 8;
 
@@ -68,48 +69,74 @@ __device__ __forceinline__ void cells_at8(const void* src, u32 i0, u32 n_sd, int
     }
 }
 
+// Position i opens cell cc and closes cell prev (opening every empty cell in between).  The closed cell
+// [s, i) is larger than max_cell exactly when position i - 1 - max_cell still belongs to it (sorted input),
+// so the cell-size limit costs one extra load per cell, not per super-droplet.  Returns "too large".
+template <int SRC>
+__device__ __forceinline__ bool open_cells(const void* src, int idxbits, int prev, int cc, u32 i, u32 max_cell,
+                                           u32* __restrict__ cell_start, int32_t* __restrict__ dbg_cell_start) {
+    for (int q = prev + 1; q <= cc; ++q) {
+        cell_start[q] = i;
+        if (dbg_cell_start) dbg_cell_start[q] = (int32_t)i;
+    }
+    return prev >= 0 && i > max_cell && cell_at<SRC>(src, i - 1u - max_cell, idxbits) == prev;
+}
+
 template <int SRC, bool VEC>
 __global__ void __launch_bounds__(CB_BLOCK)
-k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32 max_cell,
+k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32 max_cell, u32 epoch,
               u32* __restrict__ cell_start, u32* __restrict__ ctl, u32* __restrict__ sticky,
               int32_t* __restrict__ dbg_cell_start) {
+    // the fused kernel that follows accumulates the zero count; no separate memset of the control block
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctl[CTL_ZERO_COUNT] = 0u;
     const u32 i0 = (blockIdx.x * CB_BLOCK + threadIdx.x) * CB_ITEMS;  // lanes past the end stay for the shuffle
-    int c[CB_ITEMS], back[CB_ITEMS];
+    int c[CB_ITEMS];
     cells_at8<SRC, VEC>(src, i0, n_sd, idxbits, c);
-    const bool has_back = i0 >= max_cell && i0 < n_sd;  // max_cell is a multiple of 8: same alignment as i0
-    if (has_back) cells_at8<SRC, VEC>(src, i0 - max_cell, n_sd, idxbits, back);
     int prev = __shfl_up_sync(0xffffffffu, c[CB_ITEMS - 1], 1);
     if ((threadIdx.x & 31) == 0) prev = (i0 == 0 || i0 > n_sd) ? -1 : cell_at<SRC>(src, i0 - 1, idxbits);
     bool bad = false;
+    if (i0 + CB_ITEMS < n_sd) {
+        // interior thread, straight-line: every value in range (then the differences cannot overflow);
+        // the OR of the differences to the predecessor is negative when the order is broken, zero when the
+        // thread holds no cell boundary (the common case), positive otherwise
+        bad = (u32)prev + 1u > (u32)n_cell;  // prev is -1 (array start) or a cell_id that must be in range too
+        int ored = 0;
+        int p = prev;
 #pragma unroll
-    for (int k = 0; k < CB_ITEMS; ++k) {
-        const u32 i = i0 + k;
-        if (i < n_sd) {
-            const int cc = c[k];
-            if (cc < 0 || cc >= n_cell || cc < prev) {
-                bad = true;
-            } else {
-                // a cell larger than the fused kernel's register tile: position i - max_cell is in it too
-                if (has_back && back[k] == cc) bad = true;
-                if (cc != prev) {
-                    for (int q = prev + 1; q <= cc; ++q) {  // i opens cell cc and every empty cell before it
-                        cell_start[q] = i;
-                        if (dbg_cell_start) dbg_cell_start[q] = (int32_t)i;
-                    }
-                }
-                if (i == n_sd - 1) {
-                    for (int q = cc + 1; q <= n_cell; ++q) {
-                        cell_start[q] = n_sd;
-                        if (dbg_cell_start) dbg_cell_start[q] = (int32_t)n_sd;
-                    }
-                }
+        for (int k = 0; k < CB_ITEMS; ++k) {
+            bad |= (u32)c[k] >= (u32)n_cell;
+            ored |= c[k] - p;
+            p = c[k];
+        }
+        bad |= ored < 0;
+        if (!bad && ored != 0) {
+            p = prev;
+#pragma unroll
+            for (int k = 0; k < CB_ITEMS; ++k) {
+                if (c[k] != p) bad |= open_cells<SRC>(src, idxbits, p, c[k], i0 + k, max_cell, cell_start, dbg_cell_start);
+                p = c[k];
             }
-            prev = cc;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < CB_ITEMS; ++k) {
+            const u32 i = i0 + k;
+            if (i < n_sd) {
+                const int cc = c[k];
+                if (cc < 0 || cc >= n_cell || cc < prev) {
+                    bad = true;
+                } else {
+                    if (cc != prev) bad |= open_cells<SRC>(src, idxbits, prev, cc, i, max_cell, cell_start, dbg_cell_start);
+                    if (i == n_sd - 1)  // the array end closes cell cc and opens the (empty) rest
+                        bad |= open_cells<SRC>(src, idxbits, cc, n_cell, n_sd, max_cell, cell_start, dbg_cell_start);
+                }
+                prev = cc;
+            }
         }
     }
     if (bad) {  // out of range, out of order or too large: the step is skipped and reported
         sticky[STICKY_BAD_DATA] = 1u;
-        ctl[CTL_UNSORTED] = 1u;
+        ctl[CTL_UNSORTED] = epoch;  // tagged with this step's epoch: stale refusals never match
     }
 }
 
@@ -183,6 +210,7 @@ struct FusedArgs {
     int32_t* dbg_perm;
     u32* sticky;
     u32* ctl;
+    u32 epoch;  // ctl[CTL_UNSORTED] == epoch: k_cell_bounds refused this step's input
 };
 
 // Original array index of position e of the run that starts at `start`.
@@ -234,20 +262,27 @@ __device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMA
             vol[r] = pa.v[idx[r]];
         }
     }
+    // keys first: Philox needs only the index, so the attribute loads above stay in flight under it
     u32 x[R];
     const int drop = 32 - a.key_bits;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const u32 e = 32u * r + lane;
         x[r] = 0xFFFFFFFFu;  // padding sorts to the end
-        if (e < n_c) {
-            zeros += (xi[r] == 0);
+        if (e < n_c && n_c >= 2) {
             const PhiloxOut w = philox4x32_10(pa.pk, (u64)idx[r]);
-            st.xv[e] = make_longlong2(xi[r], __double_as_longlong(vol[r]));
             st.uw[e] = make_uint2(w.w2, w.w3);
             st.key[e] = w.w0;
             if (WORD != 0) st.idx[e] = idx[r];
             x[r] = ((w.w0 >> drop) << 8) | e;
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const u32 e = 32u * r + lane;
+        if (e < n_c) {
+            zeros += (xi[r] == 0);
+            st.xv[e] = make_longlong2(xi[r], __double_as_longlong(vol[r]));
         }
     }
     if (n_c < 2) {
@@ -333,27 +368,30 @@ __device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMA
 }
 
 template <int WORD, int RMAX>
-__global__ void __launch_bounds__(CF_BLOCK) k_cell_fused(const FusedArgs a) {
+__global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const FusedArgs a) {
     __shared__ CellStage<WORD, RMAX> s_stage[CF_WARPS];
-    if (a.ctl[CTL_UNSORTED]) return;  // k_cell_bounds refused the input: the step is skipped as a whole
+    if (a.ctl[CTL_UNSORTED] == a.epoch) return;  // k_cell_bounds refused the input: the step is skipped as a whole
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int c = blockIdx.x * CF_WARPS + warp;
-    if (c >= a.n_cell) return;
-    const u32 start = __ldg(a.pair.cell_start + c);
-    const u32 n_c = __ldg(a.pair.cell_start + c + 1) - start;
-    if (n_c == 0) return;
     CellStage<WORD, RMAX>& st = s_stage[warp];
+    // one warp per cell, one launch wave after another: the block scheduler balances the (data-dependent)
+    // cost of the cells; a persistent strided loop measured 12 % slower on cfg3
+    const int c = blockIdx.x * CF_WARPS + warp;
     u32 zeros = 0;
-    if (n_c <= 32) {
-        zeros = warp_cell<WORD, RMAX, 1>(a, st, start, n_c, lane);
-    } else if (RMAX >= 2 && n_c <= 64) {
-        if constexpr (RMAX >= 2) zeros = warp_cell<WORD, RMAX, 2>(a, st, start, n_c, lane);
-    } else if (RMAX >= 4 && n_c <= 128) {
-        if constexpr (RMAX >= 4) zeros = warp_cell<WORD, RMAX, 4>(a, st, start, n_c, lane);
-    } else if (RMAX >= 8 && n_c <= 256) {
-        if constexpr (RMAX >= 8) zeros = warp_cell<WORD, RMAX, 8>(a, st, start, n_c, lane);
-    } else if (lane == 0) {
-        a.sticky[STICKY_BAD_DATA] = 1u;  // unreachable: k_cell_bounds refuses such cells
+    if (c < a.n_cell) {
+        const u32 start = __ldg(a.pair.cell_start + c);
+        const u32 n_c = __ldg(a.pair.cell_start + c + 1) - start;
+        if (n_c == 0) {
+        } else if (n_c <= 32) {
+            zeros = warp_cell<WORD, RMAX, 1>(a, st, start, n_c, lane);
+        } else if (RMAX >= 2 && n_c <= 64) {
+            if constexpr (RMAX >= 2) zeros = warp_cell<WORD, RMAX, 2>(a, st, start, n_c, lane);
+        } else if (RMAX >= 4 && n_c <= 128) {
+            if constexpr (RMAX >= 4) zeros = warp_cell<WORD, RMAX, 4>(a, st, start, n_c, lane);
+        } else if (RMAX >= 8 && n_c <= 256) {
+            if constexpr (RMAX >= 8) zeros = warp_cell<WORD, RMAX, 8>(a, st, start, n_c, lane);
+        } else if (lane == 0) {
+            a.sticky[STICKY_BAD_DATA] = 1u;  // unreachable: k_cell_bounds refuses such cells
+        }
     }
     // a5, fused: the number of zero multiplicities after the step (sdm_remove_zero_multiplicity reads it)
     zeros = __reduce_add_sync(0xffffffffu, zeros);
@@ -371,7 +409,8 @@ cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int6
     const bool vec = (reinterpret_cast<uintptr_t>(src) & 15u) == 0;
 #define SDM_BOUNDS(SRC, VEC, IDXBITS)                                                                       \
     k_cell_bounds<SRC, VEC><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, IDXBITS, max_cell, \
-                                                                ws.cell_start, ws.ctl, ws.sticky, ctx->dbg_cell_start)
+                                                                ctx->epoch, ws.cell_start, ws.ctl, ws.sticky,      \
+                                                                ctx->dbg_cell_start)
     if (src_kind == 0) {
         if (vec) SDM_BOUNDS(0, true, 0);
         else SDM_BOUNDS(0, false, 0);
@@ -386,8 +425,21 @@ cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int6
     return cudaGetLastError();
 }
 
+template <int WORD, int RMAX>
+static void prefer_shared_carveout() {  // the staging tiles want the shared-memory end of the L1 split
+    static bool done = false;
+    if (!done) {
+        cudaFuncSetAttribute(k_cell_fused<WORD, RMAX>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                             cudaSharedmemCarveoutMaxShared);
+        done = true;
+    }
+}
+
 template <int WORD>
 static void launch_fused_word(const FusedArgs& a, int rmax, u32 grid, cudaStream_t st) {
+    prefer_shared_carveout<WORD, 2>();
+    prefer_shared_carveout<WORD, 4>();
+    prefer_shared_carveout<WORD, 8>();
     if (rmax <= 2) k_cell_fused<WORD, 2><<<grid, CF_BLOCK, 0, st>>>(a);
     else if (rmax <= 4) k_cell_fused<WORD, 4><<<grid, CF_BLOCK, 0, st>>>(a);
     else k_cell_fused<WORD, 8><<<grid, CF_BLOCK, 0, st>>>(a);
@@ -418,6 +470,7 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.dbg_perm = ctx->dbg_perm;
     a.sticky = ctx->ws.sticky;
     a.ctl = ctx->ws.ctl;
+    a.epoch = ctx->epoch;
     const u32 grid = (u32)((n_cell + CF_WARPS - 1) / CF_WARPS);
     LaunchScope scope(ctx, PROF_CELL_FUSED);
     if (src_kind == 0) launch_fused_word<0>(a, rmax, grid, ctx->stream);

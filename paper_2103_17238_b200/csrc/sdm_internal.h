@@ -30,7 +30,8 @@ constexpr int CMP_TILE = CMP_BLOCK * CMP_ITEMS;
 
 // Words of the per-step control block (zeroed by one memset at the start of every step).
 enum CtlWord {
-    CTL_UNSORTED = 0,     // set when cell_id is not non-decreasing (fast path: the step is skipped)
+    CTL_UNSORTED = 0,     // general path: 1 when cell_id is not non-decreasing; fused paths: the step's
+                          // epoch when k_cell_bounds refused the input (the step is then skipped)
     CTL_MAX_COUNT = 1,    // general path: largest per-cell count (feeds the host-side path verdict)
     CTL_TICKET0 = 8,      // CTL_TICKET0 + pass: dynamic tile tickets of the sort passes
     CTL_CMP_TICKET = 24,  // compaction ticket
@@ -102,8 +103,10 @@ struct sdm_ctx {
     size_t prof_used;
     // AUTO path selection: verdict of the last general-path step about (cell_id pointer, n_sd, n_cell)
     sdm::Verdict* verdict_host;  // pinned
+    sdm::u32* status_host;       // pinned: sticky words then control block, one D2H copy
     cudaEvent_t verdict_event;
     // zero-multiplicity count left in ctl[CTL_ZERO_COUNT] by the last fused step (SDM_OPT_TRACK_ZEROS)
+    sdm::u32 epoch;  // tag of the current fused-path step (>= 2; see k_cell_bounds)
     int track_zeros;
     int zero_hint_valid;
     const void* zero_hint_xi;

@@ -48,7 +48,8 @@ __device__ __forceinline__ u32 pair_scale_int(u32 n_c) { return (n_c & 1u) ? n_c
 
 // fp32 helpers of the geometric bound.  BOUND_EPS covers every rounding of the fp32 evaluation: the
 // approximate cube root 2^(log2(x)/3) from MUFU.LG2/EX2 (|log2 x| <= 100 inside the guarded range ->
-// relative error < 6e-6), the fp64 -> fp32 conversions and a dozen fp32 roundings (6e-8 each).
+// relative error < 6e-6), the fp64 -> fp32 conversions, r sqrt^-1(r) (2 ulp) and a dozen fp32 roundings
+// (6e-8 each).  The fall speed goes like r^2 at most, so its relative error is below 2 BOUND_EPS.
 constexpr float BOUND_EPS = 3e-5f;
 
 __device__ __forceinline__ float bound_radius(float v) {  // ~ (3 v / 4 pi)^(1/3), relative error < 1e-5
@@ -56,20 +57,20 @@ __device__ __forceinline__ float bound_radius(float v) {  // ~ (3 v / 4 pi)^(1/3
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(__log2f(v * 0.2387324f) * 0.33333334f));  // MUFU.EX2, 2 ulp
     return y;
 }
-// R16 in fp32; the fall speed is non-decreasing in r over all three regimes (0.19 -> 0.32 m/s at 40 um,
-// 4.8 -> 4.92 m/s at 600 um), which is what turns radius intervals into fall-speed intervals.
-__device__ __forceinline__ float bound_fall_speed(float r) {
-    if (r < 40e-6f) return 1.19e8f * (r * r);
-    if (r < 600e-6f) return 8e3f * r;
-    return 2.01e2f * sqrtf(r);
+// R16 in fp32.  `near_edge` is set when r is within BOUND_EPS of a regime boundary, where the fp64 radius
+// may fall in the other regime (the law jumps there: 0.19 -> 0.32 m/s at 40 um, 4.8 -> 4.92 m/s at 600 um).
+__device__ __forceinline__ float bound_fall_speed(float r, bool& near_edge) {
+    near_edge |= (fabsf(r - 40e-6f) <= 40e-6f * BOUND_EPS) | (fabsf(r - 600e-6f) <= 600e-6f * BOUND_EPS);
+    const float quad = 1.19e8f * (r * r), lin = 8e3f * r, root = 2.01e2f * (r * rsqrtf(r));
+    return r < 40e-6f ? quad : (r < 600e-6f ? lin : root);
 }
 
 // Conservative test: returns false only when gamma = 0 is certain (then the pair changes nothing and,
 // without debug outputs, needs no further work).  xj >= xk, (vj, vk) follow that order.
 //   Golovin: the exact fp64 probability is five operations, so the test is exact:
 //            gamma != 0  <=>  p >= 1  or  u < p            (p < 1 => floor(p) = 0, p - 0 = p)
-//   geometric: an upper bound p_ub >= p from ~30 fp32 operations on radius / fall-speed INTERVALS
-//            [r(1-eps), r(1+eps)]: K <= E pi (r_j+ + r_k+)^2 max(vt_j+ - vt_k-, vt_k+ - vt_j-).
+//   geometric: an upper bound p_ub >= p from ~30 fp32 operations: with relative errors eps on the radii
+//            and 2 eps on the fall speeds, K <= E pi ((r_j + r_k)(1 + eps))^2 (|vt_j - vt_k| + 2 eps (vt_j + vt_k)).
 //            u >= p_ub (compared through a lower bound of u) => p < 1 and not (u < p) => gamma = 0.
 __device__ __forceinline__ bool pair_may_collide(const PairArgs& a, long long xj, double vj, double vk, u32 w2, u32 w3,
                                                  u32 n_c) {
@@ -79,18 +80,16 @@ __device__ __forceinline__ bool pair_may_collide(const PairArgs& a, long long xj
         return (p >= 1.0) || (uniform_from_words(w2, w3) < p) || !(p == p);
     }
     const float fj = (float)vj, fk = (float)vk;
-    if (!(fj > 1e-30f && fj < 1e30f && fk > 1e-30f && fk < 1e30f)) return true;  // outside the bound's validity
+    bool unsure = !(fj > 1e-30f && fj < 1e30f && fk > 1e-30f && fk < 1e30f);  // outside the bound's validity
     const float rj = bound_radius(fj), rk = bound_radius(fk);
-    const float up = 1.0f + BOUND_EPS, dn = 1.0f - BOUND_EPS;
-    const float rj_hi = rj * up, rk_hi = rk * up;
-    const float tj_hi = bound_fall_speed(rj_hi) * up, tj_lo = bound_fall_speed(rj * dn) * dn;
-    const float tk_hi = bound_fall_speed(rk_hi) * up, tk_lo = bound_fall_speed(rk * dn) * dn;
-    const float dvt = fmaxf(tj_hi - tk_lo, tk_hi - tj_lo) * up;
-    const float s = rj_hi + rk_hi;
-    const float K_ub = a.Epi_up * (s * s) * dvt * up;
+    const float tj = bound_fall_speed(rj, unsure), tk = bound_fall_speed(rk, unsure);
+    const float up = 1.0f + 4.0f * BOUND_EPS;
+    const float dvt = (fabsf(tj - tk) + (2.0f * BOUND_EPS) * (tj + tk)) * up;
+    const float s = (rj + rk) * up;
+    const float K_ub = a.Epi_up * (s * s) * dvt;
     const float p_ub = K_ub * __ll2float_ru(xj) * a.dtdV_up * (float)pair_scale_int(n_c) * up + 1e-30f;
     const float u_lo = (float)(w3 >> 8) * 0x1.0p-24f;  // exact in fp32, <= u (the low 29 bits are dropped)
-    return !(u_lo >= p_ub);
+    return unsure || !(u_lo >= p_ub);
 }
 
 // The whole rule for one pair, exactly.  (j0, k0) = original indices in shuffled order, (x0, v0) / (x1, v1)
