@@ -57,6 +57,8 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     w.buf_a = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.buf_b = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.cmp_state = reinterpret_cast<u32*>(take(cmp_tiles * 4));
+    w.scan_state_bytes = ((size_t)max_n_cell / 4096 + 2) * 8;
+    w.scan_state = reinterpret_cast<u64*>(take(w.scan_state_bytes));
     w.total_bytes = off;
     return w;
 }
@@ -143,7 +145,8 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
         return SDM_ERR_CUDA;
     }
     if (cudaMemsetAsync(ctx->ws.sticky, 0, STICKY_WORDS * 4, ctx->stream) != cudaSuccess ||
-        cudaMemsetAsync(ctx->ws.ctl, 0, CTL_WORDS * 4, ctx->stream) != cudaSuccess) {
+        cudaMemsetAsync(ctx->ws.ctl, 0, CTL_WORDS * 4, ctx->stream) != cudaSuccess ||
+        cudaMemsetAsync(ctx->ws.scan_state, 0, ctx->ws.scan_state_bytes, ctx->stream) != cudaSuccess) {
         free_ctx(ctx);
         return SDM_ERR_CUDA;
     }
@@ -268,6 +271,11 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
     dkp.Epi = kp->E * 3.141592653589793;
     const double dtdV = dt / dV;
 
+    // one epoch per step tags the device-side flags and scan states of this step (no per-step memsets of them)
+    if (++ctx->epoch >= (1u << 30)) {
+        ctx->epoch = 2;
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.scan_state, 0, ws.scan_state_bytes, st)))) return rc;
+    }
     // ---- path selection (include/sdm.h, sdm_path) ----
     int path = SDM_PATH_GENERAL;
     if (n_cell > 1) {
@@ -288,7 +296,6 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         rmax = mc <= 64 ? 2 : (mc <= 128 ? 4 : 8);
     }
     ctx->zero_hint_valid = 0;
-    ctx->epoch = ctx->epoch >= 0xFFFFFFF0u ? 2u : ctx->epoch + 1u;
     if (path == SDM_PATH_CELL_SORTED) {
         if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, 0, cell_id, n_sd, n_cell, 0, rmax)))) return rc;
         if ((rc = note_cuda(ctx, launch_cell_fused(ctx, 0, nullptr, 0, rmax, multiplicity, volume, n_sd, n_cell, dtdV, dkp,

@@ -2,7 +2,7 @@
 // the composite sort key (cell_id << 32 | key), the per-cell histogram and its exclusive scan.
 //
 //   k_keys_hist  reads cell_id (4 B/SD), writes sortkey u64 (8 B/SD)            -> HBM bound, 12 B/SD
-//   k_cell_scan  one CTA, chained warp-shuffle scan over the n_cell counts       -> latency bound
+//   k_cell_scan  one CTA per slab of 4096 counts, decoupled look-back over slab totals -> latency bound
 #include "sdm_internal.h"
 
 namespace sdm {
@@ -87,22 +87,30 @@ k_keys_hist(const int32_t* __restrict__ cell_id, long long n_sd, int n_cell, int
     if (unsorted) ctl[CTL_UNSORTED] = 1u;
 }
 
-// Exclusive scan of the per-cell counts -> cell_start[0..n_cell]; one CTA of 1024 threads walks the
-// array in coalesced slabs of 4096 counts, carrying the running total (chained warp-shuffle scans).
+// Exclusive scan of the per-cell counts -> cell_start[0..n_cell].  Slabs of 4096 counts, one CTA of 1024
+// threads per slab (at most one CTA per SM, so every CTA of a round is resident), chained by a decoupled
+// look-back over 64-bit slab states {epoch << 2 | kind, value}: kind 1 = slab total, 2 = inclusive prefix.
+// The epoch tag (one per step) makes stale states of earlier steps invisible without a memset.
 constexpr int SCAN_BLOCK = 1024;
+constexpr int SCAN_SLAB = SCAN_BLOCK * 4;
+
+__device__ __forceinline__ u64 ld_relaxed_u64(const u64* p) {
+    u64 v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_u64(u64* p, u64 v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
 
 __global__ void __launch_bounds__(SCAN_BLOCK)
 k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, int n_cell, u32 n_sd_total,
-            int32_t* __restrict__ dbg_cell_start, u32* __restrict__ ctl) {
+            int32_t* __restrict__ dbg_cell_start, u32* __restrict__ ctl, u64* __restrict__ slab_state, u32 epoch) {
     __shared__ u32 s_warp[32];
     __shared__ u32 s_carry;
-    __shared__ u32 s_max;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) { s_carry = 0; s_max = 0; }
-    u32 my_max = 0;
-    __syncthreads();
     if (n_cell == 1) {  // box model: the single cell holds every super-droplet
-        if (tid == 0) {
+        if (tid == 0 && blockIdx.x == 0) {
             cell_start[0] = 0;
             cell_start[1] = n_sd_total;
             if (dbg_cell_start) { dbg_cell_start[0] = 0; dbg_cell_start[1] = (int32_t)n_sd_total; }
@@ -110,8 +118,11 @@ k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, in
         }
         return;
     }
-    for (int base = 0; base < n_cell; base += SCAN_BLOCK * 4) {
-        const int c0 = base + tid * 4;
+    const int n_slabs = (n_cell + SCAN_SLAB - 1) / SCAN_SLAB;
+    const u64 tag_total = ((u64)epoch << 2 | 1ull) << 32, tag_prefix = ((u64)epoch << 2 | 2ull) << 32;
+    u32 my_max = 0;
+    for (int slab = blockIdx.x; slab < n_slabs; slab += gridDim.x) {
+        const int c0 = slab * SCAN_SLAB + tid * 4;
         u32 x[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) x[j] = (c0 + j < n_cell) ? cell_count[c0 + j] : 0u;
@@ -126,7 +137,7 @@ k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, in
         if (lane == 31) s_warp[warp] = incl;
         __syncthreads();
         if (warp == 0) {
-            u32 w = s_warp[lane];
+            const u32 w = s_warp[lane];
             u32 wi = w;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -134,10 +145,30 @@ k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, in
                 if (lane >= o) wi += y;
             }
             s_warp[lane] = wi - w;  // exclusive warp offsets
+            const u32 total = __shfl_sync(0xffffffffu, wi, 31);
+            if (lane == 0 && slab != 0) st_relaxed_u64(slab_state + slab, tag_total | total);
+            // look-back, a window of 32 predecessors at a time (lane l inspects slab j - l)
+            u32 excl = 0;
+            for (int j = slab - 1; j >= 0; j -= 32) {
+                const int q = j - lane;
+                u64 st = tag_prefix;  // before slab 0: prefix 0
+                if (q >= 0) {
+                    do st = ld_relaxed_u64(slab_state + q);
+                    while ((u32)(st >> 34) != epoch);
+                }
+                const bool is_prefix = ((st >> 32) & 3ull) == 2ull;
+                const u32 pm = __ballot_sync(0xffffffffu, is_prefix);
+                const int first = pm ? __ffs(pm) - 1 : 32;
+                excl += __reduce_add_sync(0xffffffffu, lane <= first ? (u32)st : 0u);
+                if (pm) break;
+            }
+            if (lane == 0) {
+                st_relaxed_u64(slab_state + slab, tag_prefix | (u64)(excl + total));
+                s_carry = excl;
+            }
         }
         __syncthreads();
-        const u32 carry = s_carry;
-        u32 run = carry + s_warp[warp] + (incl - tsum);
+        u32 run = s_carry + s_warp[warp] + (incl - tsum);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             if (c0 + j < n_cell) {
@@ -146,17 +177,13 @@ k_cell_scan(const u32* __restrict__ cell_count, u32* __restrict__ cell_start, in
             }
             run += x[j];
         }
-        __syncthreads();
-        if (tid == SCAN_BLOCK - 1) s_carry = run;  // inclusive total through this slab
-        __syncthreads();
+        __syncthreads();  // s_warp / s_carry are rewritten by the next slab
     }
     my_max = __reduce_max_sync(0xffffffffu, my_max);
-    if (lane == 0) atomicMax(&s_max, my_max);
-    __syncthreads();
-    if (tid == 0) {
+    if (lane == 0 && my_max) atomicMax(&ctl[CTL_MAX_COUNT], my_max);
+    if (tid == 0 && blockIdx.x == 0) {
         cell_start[n_cell] = n_sd_total;
         if (dbg_cell_start) dbg_cell_start[n_cell] = (int32_t)n_sd_total;
-        ctl[CTL_MAX_COUNT] = s_max;
     }
 }
 
@@ -234,8 +261,10 @@ cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd,
 
 cudaError_t launch_cell_scan(sdm_ctx* ctx, int32_t n_cell, int64_t n_sd) {
     LaunchScope scope(ctx, PROF_CELL_SCAN);
-    k_cell_scan<<<1, SCAN_BLOCK, 0, ctx->stream>>>(ctx->ws.cell_count, ctx->ws.cell_start, n_cell, (u32)n_sd,
-                                                   ctx->dbg_cell_start, ctx->ws.ctl);
+    const int n_slabs = (n_cell + SCAN_SLAB - 1) / SCAN_SLAB;
+    const int grid = n_slabs < ctx->sm_count ? n_slabs : ctx->sm_count;  // all CTAs of a round resident (look-back)
+    k_cell_scan<<<grid, SCAN_BLOCK, 0, ctx->stream>>>(ctx->ws.cell_count, ctx->ws.cell_start, n_cell, (u32)n_sd,
+                                                      ctx->dbg_cell_start, ctx->ws.ctl, ctx->ws.scan_state, ctx->epoch);
     return cudaGetLastError();
 }
 

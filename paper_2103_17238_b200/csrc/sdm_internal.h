@@ -54,6 +54,8 @@ struct Workspace {
     u64* buf_a;       // max_n_sd
     u64* buf_b;       // max_n_sd
     u32* cmp_state;   // max compaction tiles
+    u64* scan_state;  // k_cell_scan slab states (epoch-tagged; zeroed at init)
+    size_t scan_state_bytes;
     size_t total_bytes;
 };
 

@@ -14,9 +14,9 @@
 // Stability (required: ties between equal keys must keep index order, R4): within a tile
 // the elements are ranked warp by warp in load order -- warp w owns the contiguous slab
 // [w*32*ITEMS, (w+1)*32*ITEMS), round k covers 32 consecutive elements.  The peers of a lane (lanes of
-// the same round with the same digit) come from eight ballots, one per digit bit: fixed-latency work
-// that pipelines across the 16 rounds, unlike MATCH.ANY, whose cost grows with the number of distinct
-// digits in the warp (profiles/r1a_README.md).  Ranks follow (warp, round, lane) = memory order.
+// the same round with the same digit) are gathered as a lane mask by one shared-memory atomic OR per
+// element (MATCH.ANY costs grow with the number of distinct digits in the warp, eight ballots per round
+// cost ~45 instructions per element: profiles/).  Ranks follow (warp, round, lane) = memory order.
 #include "sdm_internal.h"
 
 namespace sdm {
@@ -74,7 +74,10 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(ticket, 1u);
 #pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w) s_whist[w][tid] = 0;
+    for (int w = 0; w < SORT_WARPS; ++w) {
+        s_whist[w][tid] = 0;
+        reinterpret_cast<u32*>(s_stage)[w * RADIX + tid] = 0;  // the lane-mask table of the ranking phase
+    }
     __syncthreads();
     const u32 tile = s_tile;
     const u32 base = tile * (u32)SORT_TILE;
@@ -102,32 +105,40 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
         item[k] = x;
     }
 
-    // ---- peers of every element inside its round: 8 ballots per round, all rounds independent ----
-    u32 info[SORT_ITEMS];  // [4:0] lanes before me with my digit, [13:8] lanes with my digit (1..32)
+    // ---- stable ranks inside the warp, round by round (32 consecutive elements each) ----
+    // The peers of a lane (lanes of the round with the same digit) are collected in a per-warp table of
+    // lane masks: one shared-memory atomic OR per element instead of eight ballots and their selects; the
+    // first peer then advances the warp's running digit counter and clears the mask for the next round.
+    // The table aliases the staging buffer, which is not written before every warp has finished ranking.
+    u32 (*s_mask)[RADIX] = reinterpret_cast<u32 (*)[RADIX]>(s_stage);
+    u32 info[SORT_ITEMS];  // [23:16] digit, [15:0] rank among this warp's elements with that digit
     const u32 lt = lanemask_lt();
+    const u32 me = 1u << lane;
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
         const u32 d = (u32)(item[k] >> dshift) & 0xFFu;
-        u32 peers = 0xffffffffu;
-#pragma unroll
-        for (int b = 0; b < RADIX_BITS; ++b) {
-            const bool bit = (d >> b) & 1u;
-            const u32 m = __ballot_sync(0xffffffffu, bit);
-            peers &= bit ? m : ~m;
+        u32 peers, old;
+        if (__all_sync(0xffffffffu, d == __shfl_sync(0xffffffffu, d, 0))) {
+            // one digit in the whole round (cell digits of an already grouped array): no table traffic,
+            // and none of the 32-way same-address serialisation the atomic would see
+            peers = 0xffffffffu;
+            old = s_whist[warp][d];
+            __syncwarp();
+            if (lane == 0) s_whist[warp][d] = old + 32u;
+        } else {
+            atomicOr(&s_mask[warp][d], me);
+            __syncwarp();
+            peers = s_mask[warp][d];
+            old = s_whist[warp][d];
+            __syncwarp();
+            if ((peers & lt) == 0) {
+                s_whist[warp][d] = old + __popc(peers);
+                s_mask[warp][d] = 0u;
+            }
         }
-        info[k] = __popc(peers & lt) | (__popc(peers) << 8);
-    }
-
-    // ---- running per-warp digit counters: every lane reads the counter, the first peer advances it ----
-#pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) {
-        const u32 d = (u32)(item[k] >> dshift) & 0xFFu;
-        const u32 pre = info[k] & 0xFFu;
-        const u32 old = s_whist[warp][d];
         __syncwarp();
-        if (pre == 0) s_whist[warp][d] = old + (info[k] >> 8);
-        __syncwarp();
-        info[k] = old + pre;  // rank among this warp's elements with digit d
+        const u32 pre = __popc(peers & lt);
+        info[k] = (d << 16) | (old + pre);
     }
     __syncthreads();
 
@@ -150,10 +161,7 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
 
     // ---- stage in shared memory in sorted order ----
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) {
-        const u32 d = (u32)(item[k] >> dshift) & 0xFFu;
-        s_stage[s_whist[warp][d] + info[k]] = item[k];
-    }
+    for (int k = 0; k < SORT_ITEMS; ++k) s_stage[s_whist[warp][info[k] >> 16] + (info[k] & 0xFFFFu)] = item[k];
 
     // ---- decoupled look-back: global position of this tile's first element of digit d ----
     u32 gexcl;
