@@ -309,10 +309,13 @@ def run_ours(args):
     for k in kernels.values():
         k["share_of_kernel_time"] = k["ms_total"] / tot_ms
     dom = max(kernels, key=lambda nm: kernels[nm]["ms_total"]) if kernels else None
-    traffic = None
+    traffic = None  # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
     try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
-        traffic = tj.get(args.workload, {}).get(dom)
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == args.workload and row["kernel"] == dom:
+                    traffic = float(row["dram_bytes_per_launch"])
     except Exception:
         pass
     roofline = None
