@@ -188,6 +188,17 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def aggregate_over_ranks(elapsed_ms: float, units: float, dist, dev):
+    """Whole-job figures: the slowest rank's device time and the units all ranks processed."""
+    import torch
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)
+    tot = torch.tensor([units], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(tot.item())
+
+
 # ------------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
@@ -220,6 +231,8 @@ def run_ours(args):
     if args.path:
         ctx.set_path({"auto": sdm.PATH_AUTO, "general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED,
                       "hybrid": sdm.PATH_HYBRID}[args.path])
+    if world > 1:  # rank r holds entries [r n0, (r+1) n0) of a world-times larger domain (no collective)
+        ctx.set_option(sdm.OPT_INDEX_BASE, rank * n0)
     if not args.no_track_zeros:
         ctx.set_option(sdm.OPT_TRACK_ZEROS, 1)  # a5 fused into a4 (include/sdm.h): bench never writes xi in between
     stream = torch.cuda.current_stream(dev)
@@ -272,13 +285,8 @@ def run_ours(args):
     assert ctx.poll_error() == 0
     last_path = ctx.last_path()
 
-    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)
-    tot = torch.tensor([float(sd_steps)], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    max_ms = float(t.item())
-    value = float(tot.item()) / (max_ms * 1e-3)
+    max_ms, total_units = aggregate_over_ranks(elapsed_ms, float(sd_steps), dist, dev)
+    value = total_units / (max_ms * 1e-3)
 
     # ---- per-kernel timing pass: the same K steps again with an event pair around every launch ----
     ctx.profile_enable(True)

@@ -146,8 +146,13 @@ int sdm_set_path(sdm_ctx* ctx, int path);
  * of scanning the array again.  Contract: between the two calls the caller does not write the
  * multiplicity array (if it does, it sets the option again, which drops the stored count).  The GENERAL
  * path, a refused step and any other call order fall back to the counting kernel; results are identical.
+ * SDM_OPT_INDEX_BASE (>= 0, default 0): the Philox counter of array entry i becomes index_base + i.  A rank
+ * that holds entries [index_base, index_base + n_sd) of a larger array (whole cells only: cells are
+ * independent within a step) then produces exactly the bits the unsharded step produces
+ * for them -- multi-GPU runs shard by contiguous cell ranges with no collective.  Applies to
+ * sdm_coalescence_step and sdm_coalescence_step_host; the caller updates it after a compaction.
  * Returns INVALID_ARG for an unknown option or value. */
-enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1 };
+enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1, SDM_OPT_INDEX_BASE = 2 };
 int sdm_set_option(sdm_ctx* ctx, int option, int64_t value);
 
 /* Which path the most recent sdm_coalescence_step took (an sdm_path value other than AUTO), or 0 if

@@ -63,6 +63,10 @@ _lib.oracle_coalescence_step.argtypes = [
     _i64p, _f64p, _i32p, C.c_int64, C.c_int32, C.c_double, C.c_double, C.POINTER(KernelParams),
     C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.oracle_coalescence_step.restype = C.c_int
+_lib.oracle_coalescence_step_shard.argtypes = [
+    _i64p, _f64p, _i32p, C.c_int64, C.c_int32, C.c_double, C.c_double, C.POINTER(KernelParams),
+    C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.oracle_coalescence_step_shard.restype = C.c_int
 _lib.oracle_remove_zero_multiplicity.argtypes = [_i64p, _f64p, _i32p, C.c_int64]
 _lib.oracle_remove_zero_multiplicity.restype = C.c_int64
 _lib.oracle_cell_stats.argtypes = [_i64p, _f64p, _i32p, C.c_int64, C.c_int32, _i32p, _i64p, _f64p, _f64p]
@@ -139,8 +143,9 @@ def pair_update(xi_j: int, xi_k: int, v_j: float, v_k: float, g: int):
     return int(gt), int(a.value), int(b.value), float(c.value), float(d.value)
 
 
-def coalescence_step(xi, v, cell_id, n_cell, dt, dV, kp, seed, step, n_sd=None, debug=False):
-    """One step, in place.  With debug=True returns dict(perm, gamma, gamma_clamped, cell_start)."""
+def coalescence_step(xi, v, cell_id, n_cell, dt, dV, kp, seed, step, n_sd=None, debug=False, index_base=0):
+    """One step, in place.  With debug=True returns dict(perm, gamma, gamma_clamped, cell_start).
+    index_base: Philox counter of entry i is index_base + i (a shard of a larger array, R34)."""
     n = int(len(xi) if n_sd is None else n_sd)
     out = None
     ptrs = [None, None, None, None]
@@ -148,7 +153,8 @@ def coalescence_step(xi, v, cell_id, n_cell, dt, dV, kp, seed, step, n_sd=None, 
         out = dict(perm=np.zeros(n, np.int32), gamma=np.zeros(n, np.int64),
                    gamma_clamped=np.zeros(n, np.int64), cell_start=np.zeros(n_cell + 1, np.int32))
         ptrs = [out[k].ctypes.data for k in ("perm", "gamma", "gamma_clamped", "cell_start")]
-    rc = _lib.oracle_coalescence_step(xi, v, cell_id, n, n_cell, dt, dV, C.byref(kp), seed, step, *ptrs)
+    rc = _lib.oracle_coalescence_step_shard(xi, v, cell_id, n, n_cell, dt, dV, C.byref(kp), seed, step, int(index_base),
+                                            *ptrs)
     if rc != 0:
         raise ValueError(f"oracle_coalescence_step failed: {rc}")
     return out

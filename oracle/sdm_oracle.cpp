@@ -166,10 +166,14 @@ int64_t oracle_pair_update(int64_t* xi_j, int64_t* xi_k, double* v_j, double* v_
 //   cell_start_out[c]     = exclusive scan of per-cell counts, length n_cell+1
 // Returns 0, or -1 (invalid argument), -4 (bad data: cell_id out of range).
 // ---------------------------------------------------------------------------
-int oracle_coalescence_step(int64_t* xi, double* v, const int32_t* cell_id, int64_t n_sd,
-                            int32_t n_cell, double dt, double dV, const oracle_kernel_params* kp,
-                            uint64_t seed, uint64_t step, int32_t* perm_out, int64_t* gamma_out,
-                            int64_t* gamma_clamped_out, int32_t* cell_start_out) {
+//
+// index_base (reading R34): the Philox counter of array entry i is index_base + i, so a
+// shard that holds entries [index_base, index_base + n_sd) of a larger array (whole cells only) draws
+// the numbers the unsharded step draws for them.  oracle_coalescence_step is index_base = 0.
+int oracle_coalescence_step_shard(int64_t* xi, double* v, const int32_t* cell_id, int64_t n_sd,
+                                  int32_t n_cell, double dt, double dV, const oracle_kernel_params* kp,
+                                  uint64_t seed, uint64_t step, uint64_t index_base, int32_t* perm_out,
+                                  int64_t* gamma_out, int64_t* gamma_clamped_out, int32_t* cell_start_out) {
     if (n_sd < 0 || n_cell < 1 || !(dt > 0.0) || !(dV > 0.0) || kp == nullptr) return -1;
     const int64_t N = n_sd;
     for (int64_t i = 0; i < N; ++i)
@@ -178,7 +182,7 @@ int oracle_coalescence_step(int64_t* xi, double* v, const int32_t* cell_id, int6
     // O1: one Philox block per super-droplet
     std::vector<uint32_t> key(N);
     std::vector<double> u(N);
-    for (int64_t i = 0; i < N; ++i) oracle_sd_random(seed, step, (uint64_t)i, &key[i], &u[i]);
+    for (int64_t i = 0; i < N; ++i) oracle_sd_random(seed, step, index_base + (uint64_t)i, &key[i], &u[i]);
 
     // O2: stable sort of indices by (cell_id << 32) | key, ascending (R4, R5)
     std::vector<uint64_t> sortkey(N);
@@ -259,6 +263,14 @@ int oracle_cell_stats(const int64_t* xi, const double* v, const int32_t* cell_id
         if (sum_xi_v2) sum_xi_v2[c] += (x * v[i]) * v[i];
     }
     return 0;
+}
+
+int oracle_coalescence_step(int64_t* xi, double* v, const int32_t* cell_id, int64_t n_sd,
+                            int32_t n_cell, double dt, double dV, const oracle_kernel_params* kp,
+                            uint64_t seed, uint64_t step, int32_t* perm_out, int64_t* gamma_out,
+                            int64_t* gamma_clamped_out, int32_t* cell_start_out) {
+    return oracle_coalescence_step_shard(xi, v, cell_id, n_sd, n_cell, dt, dV, kp, seed, step, 0, perm_out,
+                                         gamma_out, gamma_clamped_out, cell_start_out);
 }
 
 // Exact total of xi*v for integer-valued volumes (R22), in 128-bit integers; returned as hi/lo.

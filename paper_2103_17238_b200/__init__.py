@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     PATH_HYBRID,
     OPT_NARROW_KEY_BITS,
     OPT_TRACK_ZEROS,
+    OPT_INDEX_BASE,
     KernelParams,
     SDMContext,
     SDMError,
@@ -27,6 +28,6 @@ from .binding import (  # noqa: F401
 
 __all__ = [
     "SDMContext", "SDMError", "KernelParams", "golovin", "geometric", "GOLOVIN", "GEOMETRIC",
-    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "OPT_NARROW_KEY_BITS", "OPT_TRACK_ZEROS", "workspace_bytes", "host_staging_bytes",
+    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "OPT_NARROW_KEY_BITS", "OPT_TRACK_ZEROS", "OPT_INDEX_BASE", "workspace_bytes", "host_staging_bytes",
     "load_library", "library_path",
 ]

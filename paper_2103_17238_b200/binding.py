@@ -20,6 +20,7 @@ PATH_CELL_SORTED = 2
 PATH_HYBRID = 3
 OPT_NARROW_KEY_BITS = 0
 OPT_TRACK_ZEROS = 1
+OPT_INDEX_BASE = 2
 
 SDM_OK = 0
 

@@ -204,6 +204,10 @@ int sdm_set_option(sdm_ctx* ctx, int option, int64_t value) {
         ctx->narrow_key_bits = (int)value;
         return SDM_OK;
     }
+    if (option == SDM_OPT_INDEX_BASE && value >= 0) {
+        ctx->index_base = (u64)value;
+        return SDM_OK;
+    }
     if (option == SDM_OPT_TRACK_ZEROS && (value == 0 || value == 1)) {
         ctx->track_zeros = (int)value;
         ctx->zero_hint_valid = 0;
@@ -264,7 +268,7 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_gamma, 0, (size_t)n_sd * 8, st)))) return rc;
     if (ctx->dbg_gamma_clamped)
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_gamma_clamped, 0, (size_t)n_sd * 8, st)))) return rc;
-    const PhiloxKeys pk = make_philox_keys(seed, step);
+    const PhiloxKeys pk = make_philox_keys(seed, step, ctx->index_base);
     KernelParams dkp;
     dkp.kind = kp->kind;
     dkp.b = kp->b;

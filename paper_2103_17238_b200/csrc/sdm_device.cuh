@@ -20,9 +20,10 @@ struct PhiloxKeys {
     u32 k0[10];
     u32 k1[10];
     u32 step_lo, step_hi;
+    u64 index_base;  // counter of array entry i is index_base + i (SDM_OPT_INDEX_BASE; R34)
 };
 
-__host__ __device__ inline PhiloxKeys make_philox_keys(u64 seed, u64 step) {
+__host__ __device__ inline PhiloxKeys make_philox_keys(u64 seed, u64 step, u64 index_base = 0) {
     PhiloxKeys pk;
     u32 a = (u32)seed, b = (u32)(seed >> 32);
     for (int r = 0; r < 10; ++r) {
@@ -33,6 +34,7 @@ __host__ __device__ inline PhiloxKeys make_philox_keys(u64 seed, u64 step) {
     }
     pk.step_lo = (u32)step;
     pk.step_hi = (u32)(step >> 32);
+    pk.index_base = index_base;
     return pk;
 }
 
@@ -41,6 +43,7 @@ struct PhiloxOut {
 };
 
 __device__ __forceinline__ PhiloxOut philox4x32_10(const PhiloxKeys& pk, u64 i) {
+    i += pk.index_base;
     u32 c0 = (u32)i, c1 = (u32)(i >> 32), c2 = pk.step_lo, c3 = pk.step_hi;
 #pragma unroll
     for (int r = 0; r < 10; ++r) {

@@ -109,6 +109,7 @@ struct sdm_ctx {
     cudaEvent_t verdict_event;
     // zero-multiplicity count left in ctl[CTL_ZERO_COUNT] by the last fused step (SDM_OPT_TRACK_ZEROS)
     sdm::u32 epoch;  // tag of the current fused-path step (>= 2; see k_cell_bounds)
+    sdm::u64 index_base;  // SDM_OPT_INDEX_BASE
     int track_zeros;
     int zero_hint_valid;
     const void* zero_hint_xi;

@@ -169,3 +169,33 @@ def small(name: str, interleave: bool = False) -> Workload:
     if name == "cfg4s":
         return cfg4(n_cell=401, n_steps=30, interleave=interleave, stress=True)
     raise KeyError(name)
+
+
+@dataclasses.dataclass
+class Shard:
+    """One rank's part of a cell-major workload: whole cells [cell_lo, cell_hi), array entries
+    [index_base, index_base + work.n_sd).  `work.cell_id` is rebased to start at 0."""
+    work: Workload
+    rank: int
+    world: int
+    cell_lo: int
+    cell_hi: int
+    index_base: int
+
+
+def shard(w: Workload, rank: int, world: int) -> Shard:
+    """Splits a multi-cell, cell-major workload into `world` contiguous cell ranges (cells are
+    independent within a step, so ranks exchange nothing).  Pure index bookkeeping: no method arithmetic."""
+    if not (0 <= rank < world):
+        raise ValueError("rank outside [0, world)")
+    if w.n_cell < world:
+        raise ValueError("fewer cells than ranks: single-cell boxes do not shard (replicas only)")
+    if np.any(np.diff(w.cell_id) < 0):
+        raise ValueError("shard() needs cell-major order (non-decreasing cell_id)")
+    cell_lo = (w.n_cell * rank) // world
+    cell_hi = (w.n_cell * (rank + 1)) // world
+    lo = int(np.searchsorted(w.cell_id, cell_lo, side="left"))
+    hi = int(np.searchsorted(w.cell_id, cell_hi, side="left"))
+    work = dataclasses.replace(w, xi=w.xi[lo:hi].copy(), v=w.v[lo:hi].copy(),
+                               cell_id=(w.cell_id[lo:hi] - cell_lo).astype(np.int32), n_cell=cell_hi - cell_lo)
+    return Shard(work, rank, world, cell_lo, cell_hi, lo)

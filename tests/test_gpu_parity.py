@@ -547,3 +547,33 @@ def test_cfg0_long_run_matches_oracle(dev):
         assert ctx.poll_error() == 0
     assert np.array_equal(xi.cpu().numpy(), ow.xi)
     assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v.view(np.int64))
+
+
+# ------------------------------------------------------------------------------------------- multi-GPU plan
+@pytest.mark.parametrize("name", ["cfg3", "cfg4s"])
+@pytest.mark.parametrize("path", ["general", "cell_sorted"])
+def test_shards_with_index_base_reproduce_the_unsharded_step(dev, name, path):
+    """contiguous cell ranges stepped separately with SDM_OPT_INDEX_BASE = first array entry of the
+    shard give exactly the bits of the unsharded step (here: two shards one after the other on one GPU, each
+    against the unsharded ORACLE result)."""
+    sdm = _sdm()
+    w = W.small(name)
+    ow = w.copy()
+    okp = _okp(w)
+    n_steps = 3
+    for s in range(n_steps):
+        oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, okp, w.seed, s)
+    p = {"general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED}[path]
+    for rank in range(2):
+        sh = W.shard(w, rank, 2)
+        sw = sh.work
+        with sdm.SDMContext(sw.n_sd, sw.n_cell, device=dev) as ctx:
+            ctx.set_path(p)
+            ctx.set_option(sdm.OPT_INDEX_BASE, sh.index_base)
+            xi, v, cell = _to_dev(sw, dev)
+            for s in range(n_steps):
+                ctx.coalescence_step(xi, v, cell, sw.n_cell, sw.dt, sw.dV, _gkp(sw), sw.seed, s)
+            assert ctx.poll_error() == 0
+            lo, n = sh.index_base, sw.n_sd
+            assert np.array_equal(xi.cpu().numpy(), ow.xi[lo:lo + n])
+            assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v[lo:lo + n].view(np.int64))
