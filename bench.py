@@ -75,6 +75,8 @@ def algorithmic_bytes(n_cell: int, n_pass: int):
         "cell_scan": 0, "compact": 20, "cell_stats": 20, "other": 0,
         "cell_bounds": 4,                            # read cell_id
         "cell_fused": 32,                            # read xi,v 16 + write xi,v 16 (keys regenerated)
+        "cell_digit_hist": 4,                        # read cell_id
+        "tie_repair": 8,                             # read the sorted words (rewrites only tied runs)
         "_step_total": (4 if n_cell > 1 else 0) + 8 + 16 * n_pass + 40,
     }
 

@@ -151,8 +151,13 @@ int sdm_set_path(sdm_ctx* ctx, int path);
  * independent within a step) then produces exactly the bits the unsharded step produces
  * for them -- multi-GPU runs shard by contiguous cell ranges with no collective.  Applies to
  * sdm_coalescence_step and sdm_coalescence_step_host; the caller updates it after a compaction.
+ * SDM_OPT_SKIP_KEY_DIGITS (-1 = automatic (default), 0..3): number of low 8-bit digits of the Philox key the
+ * GENERAL path's LSD passes leave unsorted.  With few super-droplets per cell the top key digits already
+ * order almost every neighbour; the runs that still tie are then put in exact (key, index) order by a
+ * repair kernel, so the permutation -- and every result -- is the same for every value (tests force 3).
+ * Automatic: sorted key bits = log2(n_sd / n_cell) + 8, rounded up to whole digits.
  * Returns INVALID_ARG for an unknown option or value. */
-enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1, SDM_OPT_INDEX_BASE = 2 };
+enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1, SDM_OPT_INDEX_BASE = 2, SDM_OPT_SKIP_KEY_DIGITS = 3 };
 int sdm_set_option(sdm_ctx* ctx, int option, int64_t value);
 
 /* Which path the most recent sdm_coalescence_step took (an sdm_path value other than AUTO), or 0 if
@@ -185,7 +190,7 @@ int64_t sdm_launch_count(sdm_ctx* ctx);
  * host) since the last read, and resets the accumulation. */
 enum { SDM_PROF_KEYS_HIST = 0, SDM_PROF_CELL_SCAN, SDM_PROF_RADIX_PASS, SDM_PROF_PAIR, SDM_PROF_COUNT_ZERO,
        SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CELL_BOUNDS, SDM_PROF_CELL_FUSED,
-       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_CLASSES };
+       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_TIE_REPAIR, SDM_PROF_CLASSES };
 int sdm_profile_enable(sdm_ctx* ctx, int on);
 int sdm_profile_read(sdm_ctx* ctx, double* ms_out /* host */, int64_t* launches_out /* host */);
 

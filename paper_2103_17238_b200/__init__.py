@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     OPT_NARROW_KEY_BITS,
     OPT_TRACK_ZEROS,
     OPT_INDEX_BASE,
+    OPT_SKIP_KEY_DIGITS,
     KernelParams,
     SDMContext,
     SDMError,
@@ -28,6 +29,6 @@ from .binding import (  # noqa: F401
 
 __all__ = [
     "SDMContext", "SDMError", "KernelParams", "golovin", "geometric", "GOLOVIN", "GEOMETRIC",
-    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "OPT_NARROW_KEY_BITS", "OPT_TRACK_ZEROS", "OPT_INDEX_BASE", "workspace_bytes", "host_staging_bytes",
+    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "OPT_NARROW_KEY_BITS", "OPT_TRACK_ZEROS", "OPT_INDEX_BASE", "OPT_SKIP_KEY_DIGITS", "workspace_bytes", "host_staging_bytes",
     "load_library", "library_path",
 ]

@@ -21,6 +21,7 @@ PATH_HYBRID = 3
 OPT_NARROW_KEY_BITS = 0
 OPT_TRACK_ZEROS = 1
 OPT_INDEX_BASE = 2
+OPT_SKIP_KEY_DIGITS = 3
 
 SDM_OK = 0
 
@@ -33,7 +34,7 @@ EXPORTS = [
 ]
 
 PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
-                "cell_bounds", "cell_fused", "cell_digit_hist"]
+                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair"]
 
 
 class SDMError(RuntimeError):

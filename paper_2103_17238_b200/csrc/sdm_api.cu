@@ -18,11 +18,22 @@ static inline int bits_for(uint64_t max_value) {  // bits needed to represent ma
     return b;
 }
 
-Plan make_plan(int64_t n_sd, int32_t n_cell) {
+// Key digits the LSD passes sort: with m super-droplets per cell on average, the top kb = log2(m) + 8 key bits
+// (rounded up to whole digits) already separate all but ~m / 2^kb <= 2^-8 of the neighbours inside a cell; the
+// remaining ties are put in exact (key, index) order by k_tie_repair, so the result does not depend on `skip`.
+Plan make_plan(int64_t n_sd, int32_t n_cell, int skip_key_digits) {
     Plan p;
     p.cbits = bits_for((uint64_t)(n_cell - 1));
     p.idxbits = bits_for((uint64_t)(n_sd > 1 ? n_sd - 1 : 1));
-    p.n_pass = 4 + (p.cbits + 7) / 8;
+    if (skip_key_digits < 0) {
+        const uint64_t m = (uint64_t)((n_sd + n_cell - 1) / n_cell);
+        int kb = ((bits_for(m > 1 ? m : 1) + 8 + 7) / 8) * 8;
+        if (kb > 32) kb = 32;
+        skip_key_digits = (32 - kb) / 8;
+    }
+    p.skip = skip_key_digits > 3 ? 3 : skip_key_digits;
+    p.n_cpass = (p.cbits + 7) / 8;
+    p.n_pass = (4 - p.skip) + p.n_cpass;
     p.n_tiles = (int)((n_sd + SORT_TILE - 1) / SORT_TILE);
     return p;
 }
@@ -130,6 +141,7 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
     ctx->ws = carve_workspace(workspace_dev, max_n_sd, max_n_cell);
     ctx->path = SDM_PATH_AUTO;
     ctx->narrow_key_bits = 24;
+    ctx->skip_key_digits = -1;
     ctx->epoch = 2;
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms <= 0) {
@@ -204,6 +216,10 @@ int sdm_set_option(sdm_ctx* ctx, int option, int64_t value) {
         ctx->narrow_key_bits = (int)value;
         return SDM_OK;
     }
+    if (option == SDM_OPT_SKIP_KEY_DIGITS && value >= -1 && value <= 3) {
+        ctx->skip_key_digits = (int)value;
+        return SDM_OK;
+    }
     if (option == SDM_OPT_INDEX_BASE && value >= 0) {
         ctx->index_base = (u64)value;
         return SDM_OK;
@@ -253,7 +269,7 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
     if (n_sd > 0 && (!aligned16(multiplicity) || !aligned16(volume))) return SDM_ERR_INVALID_ARG;
     if (ctx->cuda_error) return SDM_ERR_CUDA;
     if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
-    const Plan plan = make_plan(n_sd, n_cell);
+    const Plan plan = make_plan(n_sd, n_cell, ctx->skip_key_digits);
     if (!plan_fits(plan)) return SDM_ERR_CAPACITY;
     cudaStream_t st = ctx->stream;
     Workspace& ws = ctx->ws;
@@ -310,7 +326,7 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         return SDM_OK;
     }
     if (path == SDM_PATH_HYBRID) {
-        const int n_cpass = plan.n_pass - 4;
+        const int n_cpass = plan.n_cpass;
         const bool narrow = plan.cbits + plan.idxbits <= 32 && plan.cbits + 12 <= 32;
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
         if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)n_cpass * plan.n_tiles * RADIX * 4, st))))
@@ -351,6 +367,8 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         if ((rc = note_cuda(ctx, launch_sort_pass(ctx, pass, in, out, n_sd, plan)))) return rc;
         u64* t = in; in = out; out = t;
     }
+    if (plan.skip > 0)  // exact (key, index) order inside the runs the skipped digits left tied
+        if ((rc = note_cuda(ctx, launch_tie_repair(ctx, in, n_sd, plan, pk)))) return rc;
     const u64* sorted = in;
     if (ctx->dbg_perm)
         if ((rc = note_cuda(ctx, launch_debug_perm(ctx, sorted, n_sd, plan)))) return rc;

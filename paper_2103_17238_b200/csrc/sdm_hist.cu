@@ -13,7 +13,7 @@ constexpr int SMEM_CELLS = 2048;      // cell histograms this small are built in
 
 template <bool HAS_CELLS>
 __global__ void __launch_bounds__(HIST_BLOCK)
-k_keys_hist(const int32_t* __restrict__ cell_id, long long n_sd, int n_cell, int n_cpass,
+k_keys_hist(const int32_t* __restrict__ cell_id, long long n_sd, int n_cell, int n_cpass, int skip,
             PhiloxKeys pk, u64* __restrict__ sortkey, u32* __restrict__ digit_hist,
             u32* __restrict__ cell_count, u32* __restrict__ ctl, u32* __restrict__ sticky) {
     __shared__ u32 s_hist[MAX_PASSES][RADIX];
@@ -55,9 +55,9 @@ k_keys_hist(const int32_t* __restrict__ cell_id, long long n_sd, int n_cell, int
             if (valid) {
                 const u32 key = philox_perm_key(pk, (u64)i);
                 sortkey[i] = ((u64)(u32)cc << 32) | (u64)key;
-                atomicAdd(&s_hist[0][key & 0xFF], 1u);
-                atomicAdd(&s_hist[1][(key >> 8) & 0xFF], 1u);
-                atomicAdd(&s_hist[2][(key >> 16) & 0xFF], 1u);
+                if (skip < 1) atomicAdd(&s_hist[0][key & 0xFF], 1u);  // skipped digits are never sorted on
+                if (skip < 2) atomicAdd(&s_hist[1][(key >> 8) & 0xFF], 1u);
+                if (skip < 3) atomicAdd(&s_hist[2][(key >> 16) & 0xFF], 1u);
                 atomicAdd(&s_hist[3][key >> 24], 1u);
                 if (HAS_CELLS) {
                     // warp-aggregated: one leader per distinct cell in this warp round
@@ -235,7 +235,7 @@ cudaError_t launch_cell_digit_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t
     if (grid < 1) grid = 1;
     const int vec_ok = (reinterpret_cast<uintptr_t>(cell_id) & 15u) == 0;
     LaunchScope scope(ctx, PROF_CELL_DIGIT_HIST);
-    k_cell_digit_hist<<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, (u32)n_sd, n_cell, plan.n_pass - 4, vec_ok,
+    k_cell_digit_hist<<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, (u32)n_sd, n_cell, plan.n_cpass, vec_ok,
                                                             ctx->ws.digit_hist, ctx->ws.sticky);
     return cudaGetLastError();
 }
@@ -246,14 +246,14 @@ cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd,
     long long n_chunks = (n_sd + chunk - 1) / chunk;
     int grid = (int)(n_chunks < (long long)ctx->sm_count * 8 ? n_chunks : (long long)ctx->sm_count * 8);
     if (grid < 1) grid = 1;
-    const int n_cpass = plan.n_pass - 4;
+    const int n_cpass = plan.n_cpass;
     LaunchScope scope(ctx, PROF_KEYS_HIST);
     if (n_cell > 1)
-        k_keys_hist<true><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, pk, sortkey_out,
+        k_keys_hist<true><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, plan.skip, pk, sortkey_out,
                                                                  ctx->ws.digit_hist, ctx->ws.cell_count,
                                                                  ctx->ws.ctl, ctx->ws.sticky);
     else
-        k_keys_hist<false><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, pk, sortkey_out,
+        k_keys_hist<false><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, plan.skip, pk, sortkey_out,
                                                                   ctx->ws.digit_hist, ctx->ws.cell_count,
                                                                   ctx->ws.ctl, ctx->ws.sticky);
     return cudaGetLastError();

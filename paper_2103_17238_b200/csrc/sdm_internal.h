@@ -62,7 +62,9 @@ struct Workspace {
 struct Plan {  // per-step derived quantities
     int cbits;     // bits of (n_cell - 1)
     int idxbits;   // bits of (n_sd - 1), at least 1
-    int n_pass;    // 4 + ceil(cbits / 8)
+    int skip;      // low key digits NOT sorted by the LSD passes (0..3); ties on them are repaired exactly afterwards
+    int n_cpass;   // ceil(cbits / 8) cell-id digits
+    int n_pass;    // (4 - skip) + n_cpass
     int n_tiles;   // ceil(n_sd / SORT_TILE)
 };
 
@@ -71,7 +73,7 @@ struct Plan {  // per-step derived quantities
 namespace sdm {
 // Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
 enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
-                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_CLASSES };
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_CLASSES };
 // What the last general-path step learned about the cell_id array (pinned host memory, written by an
 // asynchronous copy; valid once `verdict_event` has completed).
 struct Verdict { u32 unsorted; u32 max_count; };
@@ -98,6 +100,7 @@ struct sdm_ctx {
     void* staging;
     size_t staging_bytes;
     int sm_count;
+    int skip_key_digits;  // SDM_OPT_SKIP_KEY_DIGITS (-1 = automatic)
     int narrow_key_bits;  // key bits kept in the fused kernel's 32-bit sort word (SDM_OPT_NARROW_KEY_BITS)
     // optional per-launch CUDA-event timing (sdm_profile_enable)
     int profiling;
@@ -146,7 +149,7 @@ struct LaunchScope {
 };
 
 Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell);
-Plan make_plan(int64_t n_sd, int32_t n_cell);
+Plan make_plan(int64_t n_sd, int32_t n_cell, int skip_key_digits /* -1 = choose from n_sd / n_cell */);
 
 // Launchers (each enqueues on ctx->stream and bumps ctx->launches).  Return cudaError_t.
 cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
@@ -166,6 +169,7 @@ cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int6
 cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int rmax, int64_t* xi,
                               double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
                               const PhiloxKeys& pk);
+cudaError_t launch_tie_repair(sdm_ctx* ctx, u64* sorted, int64_t n_sd, const Plan& plan, const PhiloxKeys& pk);
 cudaError_t launch_debug_perm(sdm_ctx* ctx, const u64* sorted, int64_t n_sd, const Plan& plan);
 cudaError_t launch_count_zero(sdm_ctx* ctx, const int64_t* xi, int64_t n_sd);
 cudaError_t launch_compact(sdm_ctx* ctx, int64_t* xi, double* v, int32_t* cell_id, int64_t n_sd);

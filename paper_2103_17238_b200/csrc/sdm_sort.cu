@@ -82,7 +82,8 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
     const u32 tile = s_tile;
     const u32 base = tile * (u32)SORT_TILE;
     const u32 n_valid = min((u32)SORT_TILE, n_sd - base);
-    const int dshift = (MODE == MODE_LATER) ? shift : SORT_TILE_BITS;  // where the digit sits in the staged word
+    // where the digit sits in the staged word (first passes stage `word << 12 | tile-local index`)
+    const int dshift = (MODE == MODE_LATER) ? shift : SORT_TILE_BITS + shift;
 
     // ---- load (warp-striped: round k of warp w = 32 consecutive elements) ----
     TW item[SORT_ITEMS];
@@ -202,21 +203,97 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
     }
 }
 
-// General path (north_star (b)): pass 0 reads the 8-byte sort keys, later passes the packed words.
+// General path (north_star (b)): pass 0 reads the 8-byte sort keys, later passes the packed words.  Executed
+// pass p sorts digit q = plan.skip + p of (cell_id << 32 | key); the skipped low key digits are left to
+// k_tie_repair.
 cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, int64_t n_sd,
                              const Plan& plan) {
+    const int q = plan.skip + pass;
     u32* ticket = ctx->ws.ctl + CTL_TICKET0 + pass;
     u32* state = ctx->ws.tile_state + (size_t)pass * (size_t)plan.n_tiles * RADIX;
-    const u32* ghist = ctx->ws.digit_hist + pass * RADIX;
+    const u32* ghist = ctx->ws.digit_hist + q * RADIX;
     LaunchScope scope(ctx, PROF_RADIX_PASS);
     if (pass == 0) {
         k_radix_pass<u64, u64, MODE_KEY_FIRST><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(
-            in, out, (u32)n_sd, 0, plan.idxbits, 0, ghist, ticket, state);
+            in, out, (u32)n_sd, 8 * q, plan.idxbits, 0, ghist, ticket, state);
     } else {
-        const int shift = plan.idxbits + 8 * (pass - 1);
+        const int shift = plan.idxbits + 8 * (q - 1);
         k_radix_pass<u64, u64, MODE_LATER><<<plan.n_tiles, SORT_BLOCK, 0, ctx->stream>>>(
             in, out, (u32)n_sd, shift, plan.idxbits, 0, ghist, ticket, state);
     }
+    return cudaGetLastError();
+}
+
+// Exact order inside the runs of equal sorted digits.  After the passes the words are ordered by
+// (cell_id, key >> 8 skip); members of a run that ties on that are still in index order (LSD stability).
+// The thread at a run's first position sorts the run by (full Philox key, index) -- the order the
+// remaining passes would have produced.  Runs are disjoint, so the repair is race-free and in place;
+// with kb sorted key bits a super-droplet sits in such a run with probability ~ n_c / 2^kb.
+__device__ __noinline__ void repair_run(u64* __restrict__ sorted, u32 s, u32 n_sd, int idxbits, int tshift,
+                                        const PhiloxKeys* __restrict__ pkp /* the kernel's __grid_constant__ parameter */) {
+    const PhiloxKeys& pk = *pkp;
+    const u64 tag = sorted[s] >> tshift;
+    u32 e = s + 2;
+    while (e < n_sd && (sorted[e] >> tshift) == tag) ++e;
+    const u64 idx_mask = (1ull << idxbits) - 1ull;
+    for (u32 a = s + 1; a < e; ++a) {  // insertion sort by (key, index)
+        const u64 wa = sorted[a];
+        const u64 ia = wa & idx_mask;
+        const u64 ka = ((u64)philox_perm_key(pk, ia) << 32) | ia;
+        u32 b = a;
+        while (b > s) {
+            const u64 wb = sorted[b - 1];
+            const u64 ib = wb & idx_mask;
+            const u64 kb = ((u64)philox_perm_key(pk, ib) << 32) | ib;
+            if (kb < ka) break;
+            sorted[b] = wb;
+            --b;
+        }
+        sorted[b] = wa;
+    }
+}
+
+constexpr int TR_ITEMS = 4;
+
+__global__ void __launch_bounds__(256)
+k_tie_repair(u64* __restrict__ sorted, u32 n_sd, int idxbits, int tshift, const __grid_constant__ PhiloxKeys pk) {
+    const u64 none = ~0ull;  // a tag no real word has (tshift >= 1): stands in where the array ends
+    const u32 stride = gridDim.x * 256u * TR_ITEMS;
+    for (u32 s0 = (blockIdx.x * 256u + threadIdx.x) * TR_ITEMS; s0 < n_sd; s0 += stride) {
+        // tags of positions s0 - 1 .. s0 + TR_ITEMS
+        u64 t[TR_ITEMS + 2];
+        if (s0 + TR_ITEMS <= n_sd) {
+            const ulonglong2 p = *reinterpret_cast<const ulonglong2*>(sorted + s0);
+            const ulonglong2 q = *reinterpret_cast<const ulonglong2*>(sorted + s0 + 2);
+            t[1] = p.x >> tshift; t[2] = p.y >> tshift; t[3] = q.x >> tshift; t[4] = q.y >> tshift;
+        } else {
+#pragma unroll
+            for (int k = 0; k < TR_ITEMS; ++k) t[1 + k] = (s0 + k < n_sd) ? (sorted[s0 + k] >> tshift) : none;
+        }
+        t[0] = s0 > 0 ? (sorted[s0 - 1] >> tshift) : none;
+        t[TR_ITEMS + 1] = (s0 + TR_ITEMS < n_sd) ? (sorted[s0 + TR_ITEMS] >> tshift) : none;
+        // a run starts where the tag differs from the predecessor's and equals the successor's; its first
+        // position repairs it (runs are disjoint: a run reaching into another thread's positions does not
+        // start there, and its members keep their common tag while they are being permuted)
+        u32 starts = 0;
+#pragma unroll
+        for (int k = 0; k < TR_ITEMS; ++k)
+            if (t[1 + k] != none && t[1 + k] != t[k] && t[1 + k] == t[2 + k]) starts |= 1u << k;
+        while (starts) {
+            const int k = __ffs(starts) - 1;
+            starts &= starts - 1u;
+            repair_run(sorted, s0 + k, n_sd, idxbits, tshift, &pk);
+        }
+    }
+}
+
+cudaError_t launch_tie_repair(sdm_ctx* ctx, u64* sorted, int64_t n_sd, const Plan& plan, const PhiloxKeys& pk) {
+    LaunchScope scope(ctx, PROF_TIE_REPAIR);
+    // the words hold (sortkey >> 8) above the index: sorted key bit 8 skip sits at idxbits + 8 (skip - 1)
+    const u32 need = (u32)((n_sd + 256 * TR_ITEMS - 1) / (256 * TR_ITEMS));
+    const u32 resident = (u32)ctx->sm_count * 8u;
+    k_tie_repair<<<need < resident ? need : resident, 256, 0, ctx->stream>>>(sorted, (u32)n_sd, plan.idxbits,
+                                                                           plan.idxbits + 8 * (plan.skip - 1), pk);
     return cudaGetLastError();
 }
 

@@ -52,7 +52,7 @@ def _assert_vol_close(got, want, what=""):
 
 
 def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key_bits=None, expect_last_path=None,
-                track_zeros=False):
+                track_zeros=False, skip_key_digits=None):
     """Steps the oracle and the GPU side by side over w.n_steps steps, comparing after every step."""
     sdm = _sdm()
     ow = w.copy()
@@ -64,6 +64,8 @@ def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key
             ctx.set_option(sdm.OPT_NARROW_KEY_BITS, narrow_key_bits)
         if track_zeros:
             ctx.set_option(sdm.OPT_TRACK_ZEROS, 1)
+        if skip_key_digits is not None:
+            ctx.set_option(sdm.OPT_SKIP_KEY_DIGITS, skip_key_digits)
         xi, v, cell = _to_dev(w, dev)
         dbg = ctx.debug_outputs(n, w.n_cell) if check_debug else None
         okp, gkp = _okp(w), _gkp(w)
@@ -151,6 +153,19 @@ def test_small_configs_general_path(dev, name):
         assert st["clamped"] > 0 and st["removed"] > 0       # large gamma, clamp, split->0, compaction
     if name == "cfg3z":
         assert st["removed"] > 0
+
+
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg3", "cfg4s"])
+@pytest.mark.parametrize("skip", [0, 1, 3])
+def test_general_path_skipped_key_digits_are_repaired_exactly(dev, name, skip):
+    """SDM_OPT_SKIP_KEY_DIGITS: the LSD passes sort only the top (4 - skip) key digits and k_tie_repair orders the
+    tied runs by (key, index); the permutation, every gamma and the state stay those of the oracle.  skip = 3 leaves
+    8 sorted key bits: in the single-cell configs every super-droplet sits in a long tied run."""
+    sdm = _sdm()
+    w = W.small(name, interleave=(name in ("cfg3", "cfg4s")))
+    if name in ("cfg0", "cfg1"):
+        w = W.cfg0(n_sd=3001, n_steps=4) if name == "cfg0" else W.cfg1(n_sd=5003, n_steps=3)
+    _run_parity(w, dev, path=sdm.PATH_GENERAL, bit_exact=True, skip_key_digits=skip)
 
 
 @pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg3z", "cfg4", "cfg4s"])
