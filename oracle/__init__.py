@@ -71,6 +71,8 @@ _lib.oracle_remove_zero_multiplicity.argtypes = [_i64p, _f64p, _i32p, C.c_int64]
 _lib.oracle_remove_zero_multiplicity.restype = C.c_int64
 _lib.oracle_cell_stats.argtypes = [_i64p, _f64p, _i32p, C.c_int64, C.c_int32, _i32p, _i64p, _f64p, _f64p]
 _lib.oracle_cell_stats.restype = C.c_int
+_lib.oracle_volume_spectrum.argtypes = [_i64p, _f64p, C.c_int64, _f64p, C.c_int32, _i64p, _i64p, _f64p]
+_lib.oracle_volume_spectrum.restype = C.c_int
 _lib.oracle_total_xi_v_int128.argtypes = [_i64p, _f64p, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_uint64)]
 _lib.oracle_total_xi_v_int128.restype = None
 _lib.oracle_run.argtypes = [_i64p, _f64p, _i32p, C.c_int64, C.c_int32, C.c_double, C.c_double,
@@ -175,6 +177,20 @@ def cell_stats(xi, v, cell_id, n_cell, n_sd=None):
     if rc != 0:
         raise ValueError(f"oracle_cell_stats failed: {rc}")
     return count, sum_xi, sum_xi_v, sum_xi_v2
+
+
+def volume_spectrum(xi, v, volume_edges, n_sd=None):
+    """O7: per-bin (count, sum xi, sum xi*v) over bins edges[b] <= v < edges[b+1] of VOLUME edges."""
+    n = int(len(xi) if n_sd is None else n_sd)
+    edges = np.ascontiguousarray(volume_edges, np.float64)
+    nb = len(edges) - 1
+    count = np.zeros(max(nb, 0), np.int64)
+    sum_xi = np.zeros(max(nb, 0), np.int64)
+    sum_xi_v = np.zeros(max(nb, 0), np.float64)
+    rc = _lib.oracle_volume_spectrum(xi, v, n, edges, len(edges), count, sum_xi, sum_xi_v)
+    if rc != 0:
+        raise ValueError(f"oracle_volume_spectrum failed: {rc}")
+    return count, sum_xi, sum_xi_v
 
 
 def total_xi_v_exact(xi, v, n_sd=None) -> int:

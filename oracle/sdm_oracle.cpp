@@ -19,6 +19,8 @@
 //   pair/p/gamma ........ brute-force 2- and 3-SD cells, binomial frequencies
 //   update/clamp/split .. hand cases, exact integer-volume conservation
 //   whole box run ....... Golovin analytic Smoluchowski solution
+//   volume spectrum ..... hand case with values on the edges, numpy.histogram on random data,
+//                         closed-form bin masses of the exponential spectrum
 //   geometric kernel .... hand values; det_cbrt vs libm cbrt.  Whole-run statistics
 //                         with the geometric kernel: PARITY UNPINNED beyond invariants.
 #include <algorithm>
@@ -271,6 +273,42 @@ int oracle_coalescence_step(int64_t* xi, double* v, const int32_t* cell_id, int6
                             int64_t* gamma_clamped_out, int32_t* cell_start_out) {
     return oracle_coalescence_step_shard(xi, v, cell_id, n_sd, n_cell, dt, dV, kp, seed, step, 0, perm_out,
                                          gamma_out, gamma_clamped_out, cell_start_out);
+}
+
+// ---------------------------------------------------------------------------
+// O7  Volume spectrum (the paper's ParticlesVolumeSpectrum(radius_bins_edges)
+// product).  The paper is silent on the product's normalisation; reading R35: the raw
+// per-bin sums.  Bin b holds the entries with edges[b] <= v < edges[b+1] (edges strictly ascending
+// VOLUMES: the caller converts its radius edges once, so no cube root enters the bin decision);
+// entries outside [edges[0], edges[n_edges-1]) are not counted.
+//   count[b]    number of array entries in the bin (whatever their multiplicity)
+//   sum_xi[b]   sum of multiplicities            (exact)
+//   sum_xi_v[b] sum of double(xi) * v, in index order
+// Returns 0, or -1 (invalid argument: fewer than 2 edges, edges not strictly ascending / not finite).
+// ---------------------------------------------------------------------------
+int oracle_volume_spectrum(const int64_t* xi, const double* v, int64_t n_sd, const double* edges,
+                           int32_t n_edges, int64_t* count, int64_t* sum_xi, double* sum_xi_v) {
+    if (n_sd < 0 || n_edges < 2) return -1;
+    for (int32_t e = 0; e < n_edges; ++e) {
+        if (!std::isfinite(edges[e])) return -1;
+        if (e > 0 && !(edges[e] > edges[e - 1])) return -1;
+    }
+    const int32_t n_bins = n_edges - 1;
+    for (int32_t b = 0; b < n_bins; ++b) {
+        if (count) count[b] = 0;
+        if (sum_xi) sum_xi[b] = 0;
+        if (sum_xi_v) sum_xi_v[b] = 0.0;
+    }
+    for (int64_t i = 0; i < n_sd; ++i) {
+        const double x = v[i];
+        if (!(x >= edges[0]) || !(x < edges[n_bins])) continue;  // outside (NaN included)
+        int32_t b = 0;
+        while (!(x < edges[b + 1])) ++b;  // linear scan: the first bin whose upper edge exceeds v
+        if (count) count[b] += 1;
+        if (sum_xi) sum_xi[b] += xi[i];
+        if (sum_xi_v) sum_xi_v[b] += (double)xi[i] * x;
+    }
+    return 0;
 }
 
 // Exact total of xi*v for integer-valued volumes (R22), in 128-bit integers; returned as hi/lo.
