@@ -372,6 +372,35 @@ def run_ours(args):
                "h2d_bytes_per_step": 20 * n0, "d2h_bytes_per_step": 16 * n0 + 8, "steps": e_steps,
                "api": "sdm_coalescence_step_host (pinned host buffers, compaction included)"}
 
+    # ---- product call outside the step: the volume spectrum on 31 log bins over the state ----
+    products = None
+    try:
+        import numpy as np
+        vpos = w.v[w.v > 0]
+        edges = np.exp(np.linspace(np.log(vpos.min() * 0.999), np.log(vpos.max() * 1.001), 32))
+        ctx.volume_spectrum(xi, v, edges, n_sd=n_prof)
+        torch.cuda.synchronize(dev)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+        for a, b in evs:
+            a.record(stream)
+            ctx.volume_spectrum(xi, v, edges, n_sd=n_prof)
+            b.record(stream)
+        torch.cuda.synchronize(dev)
+        ms = statistics.median(a.elapsed_time(b) for a, b in evs)
+        ctx.profile_enable(True)
+        ctx.profile_read()
+        for _ in range(5):
+            ctx.volume_spectrum(xi, v, edges, n_sd=n_prof)
+        kms, kcnt = ctx.profile_read()["volume_spectrum"]
+        ctx.profile_enable(False)
+        kms = kms / max(kcnt, 1)
+        gbs = 16.0 * n_prof / (kms * 1e-3) / 1e9
+        products = {"volume_spectrum": {"ms_per_call": ms, "kernel_ms": kms, "algorithmic_bytes_per_sd": 16,
+                                        "kernel_gbs": gbs, "kernel_frac": gbs / peak, "bins": 31,
+                                        "note": "call = 3 memsets + edge upload + kernel; CUDA events"}}
+    except Exception as e:  # the product is not part of the timed step
+        products = {"volume_spectrum": {"error": str(e)}}
+
     # ---- CPU baseline: the oracle on a bounded sample (rank 0, N=1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -393,7 +422,7 @@ def run_ours(args):
                                                     "north_star_bytes_per_sd_step": ns_bytes,
                                                     "north_star_equivalent_gbs": ns_gbs,
                                                     "north_star_equivalent_frac": ns_gbs / peak},
-            "kernels": kernels, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "kernels": kernels, "products": products, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
             "ms_per_step_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
         }
         print(json.dumps(line), flush=True)

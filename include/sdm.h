@@ -123,6 +123,18 @@ int sdm_cell_stats(sdm_ctx* ctx, const int64_t* multiplicity, const double* volu
                    const int32_t* cell_id, int64_t n_sd, int32_t n_cell, int32_t* count,
                    int64_t* sum_xi, double* sum_xi_v, double* sum_xi_v2);
 
+/* Volume spectrum (the paper's ParticlesVolumeSpectrum(radius_bins_edges) product,
+ * PAPER.md:68-76; the normalisation is not in the paper -- reading R35: the raw per-bin sums).  Bin b holds the
+ * array entries with volume_edges[b] <= volume < volume_edges[b+1]; entries outside [edges[0], edges[n-1]) are
+ * not counted.  volume_edges: HOST array of n_edges (2..1025) finite, strictly ascending VOLUMES [m^3] -- the
+ * caller converts its radius edges once (4/3 pi r^3), so no cube root enters the bin decision.  Outputs: DEVICE
+ * arrays of n_edges - 1 entries, each nullable: count (entries in the bin, whatever their multiplicity), sum_xi
+ * (exact), sum_xi_v (fp64, accumulated in an unspecified order: compare at 1e-12 relative).  Asynchronous.
+ * INVALID_ARG for bad edges or sizes. */
+int sdm_volume_spectrum(sdm_ctx* ctx, const int64_t* multiplicity, const double* volume, int64_t n_sd,
+                        const double* volume_edges /* host */, int32_t n_edges, int64_t* count, int64_t* sum_xi,
+                        double* sum_xi_v);
+
 /* Parity instrumentation (off by default; never on in timed runs).  Registers device arrays that
  * every later sdm_coalescence_step fills; pass NULL to switch an output off again.
  *   perm_out[s]           int32[n_sd]  original index at shuffled position s
@@ -190,7 +202,7 @@ int64_t sdm_launch_count(sdm_ctx* ctx);
  * host) since the last read, and resets the accumulation. */
 enum { SDM_PROF_KEYS_HIST = 0, SDM_PROF_CELL_SCAN, SDM_PROF_RADIX_PASS, SDM_PROF_PAIR, SDM_PROF_COUNT_ZERO,
        SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CELL_BOUNDS, SDM_PROF_CELL_FUSED,
-       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_TIE_REPAIR, SDM_PROF_CLASSES };
+       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_TIE_REPAIR, SDM_PROF_SPECTRUM, SDM_PROF_CLASSES };
 int sdm_profile_enable(sdm_ctx* ctx, int on);
 int sdm_profile_read(sdm_ctx* ctx, double* ms_out /* host */, int64_t* launches_out /* host */);
 

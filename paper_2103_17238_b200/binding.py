@@ -30,11 +30,11 @@ EXPORTS = [
     "sdm_cell_stats", "sdm_debug_outputs", "sdm_set_path", "sdm_last_path", "sdm_host_staging_bytes",
     "sdm_bind_host_staging", "sdm_coalescence_step_host", "sdm_poll_error", "sdm_launch_count",
     "sdm_philox_fill", "sdm_kernel_eval", "sdm_strerror", "sdm_destroy", "sdm_profile_enable",
-    "sdm_profile_read", "sdm_set_option",
+    "sdm_profile_read", "sdm_set_option", "sdm_volume_spectrum",
 ]
 
 PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
-                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair"]
+                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum"]
 
 
 class SDMError(RuntimeError):
@@ -102,6 +102,8 @@ def load_library():
     lib.sdm_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
     lib.sdm_profile_read.restype = C.c_int
     lib.sdm_coalescence_step_host.restype = C.c_int
+    lib.sdm_volume_spectrum.argtypes = [vp, vp, vp, i64, C.POINTER(C.c_double), i32, vp, vp, vp]
+    lib.sdm_volume_spectrum.restype = C.c_int
     lib.sdm_poll_error.argtypes = [vp]
     lib.sdm_poll_error.restype = C.c_int
     lib.sdm_launch_count.argtypes = [vp]
@@ -248,6 +250,21 @@ class SDMContext:
 
     def set_path(self, path: int):
         _check(self._lib.sdm_set_path(self._h, int(path)), "sdm_set_path")
+
+    def volume_spectrum(self, multiplicity, volume, volume_edges, n_sd=None):
+        """sdm_volume_spectrum: (count int64[nb], sum_xi int64[nb], sum_xi_v float64[nb]) device tensors."""
+        t = self._torch
+        n = int(multiplicity.shape[0] if n_sd is None else n_sd)
+        edges = [float(e) for e in volume_edges]
+        arr = (C.c_double * len(edges))(*edges)
+        nb = max(len(edges) - 1, 0)
+        count = t.empty(nb, dtype=t.int64, device=self.device)
+        sum_xi = t.empty(nb, dtype=t.int64, device=self.device)
+        sum_xi_v = t.empty(nb, dtype=t.float64, device=self.device)
+        rc = self._lib.sdm_volume_spectrum(self._h, _ptr(multiplicity, t.int64), _ptr(volume, t.float64), n, arr,
+                                           len(edges), count.data_ptr(), sum_xi.data_ptr(), sum_xi_v.data_ptr())
+        _check(rc, "sdm_volume_spectrum")
+        return count, sum_xi, sum_xi_v
 
     def set_option(self, option: int, value: int):
         _check(self._lib.sdm_set_option(self._h, int(option), int(value)), "sdm_set_option")

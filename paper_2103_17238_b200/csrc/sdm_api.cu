@@ -68,6 +68,7 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     w.buf_a = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.buf_b = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.cmp_state = reinterpret_cast<u32*>(take(cmp_tiles * 4));
+    w.spec_edges = reinterpret_cast<double*>(take((size_t)SPECTRUM_MAX_EDGES * 8));
     w.scan_state_bytes = ((size_t)max_n_cell / 4096 + 2) * 8;
     w.scan_state = reinterpret_cast<u64*>(take(w.scan_state_bytes));
     w.total_bytes = off;
@@ -235,6 +236,33 @@ int sdm_set_option(sdm_ctx* ctx, int option, int64_t value) {
 int sdm_last_path(sdm_ctx* ctx) { return ctx ? ctx->last_path : 0; }
 
 int64_t sdm_launch_count(sdm_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int sdm_volume_spectrum(sdm_ctx* ctx, const int64_t* multiplicity, const double* volume, int64_t n_sd,
+                        const double* volume_edges, int32_t n_edges, int64_t* count, int64_t* sum_xi,
+                        double* sum_xi_v) {
+    if (!ctx || !volume_edges || n_sd < 0 || n_edges < 2 || n_edges > SPECTRUM_MAX_EDGES) return SDM_ERR_INVALID_ARG;
+    if (n_sd > 0 && (!multiplicity || !volume)) return SDM_ERR_INVALID_ARG;
+    if (n_sd > 0 && (!aligned16(multiplicity) || !aligned16(volume))) return SDM_ERR_INVALID_ARG;
+    for (int32_t e = 0; e < n_edges; ++e) {
+        if (!std::isfinite(volume_edges[e])) return SDM_ERR_INVALID_ARG;
+        if (e > 0 && !(volume_edges[e] > volume_edges[e - 1])) return SDM_ERR_INVALID_ARG;
+    }
+    if (ctx->cuda_error) return SDM_ERR_CUDA;
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
+    cudaStream_t st = ctx->stream;
+    const size_t nb = (size_t)(n_edges - 1);
+    int rc;
+    if (count && (rc = note_cuda(ctx, cudaMemsetAsync(count, 0, nb * 8, st)))) return rc;
+    if (sum_xi && (rc = note_cuda(ctx, cudaMemsetAsync(sum_xi, 0, nb * 8, st)))) return rc;
+    if (sum_xi_v && (rc = note_cuda(ctx, cudaMemsetAsync(sum_xi_v, 0, nb * 8, st)))) return rc;
+    if (n_sd == 0) return SDM_OK;
+    // the edges are pageable host memory: this copy is staged before the call returns
+    if ((rc = note_cuda(ctx, cudaMemcpyAsync(ctx->ws.spec_edges, volume_edges, (size_t)n_edges * 8,
+                                             cudaMemcpyHostToDevice, st))))
+        return rc;
+    return note_cuda(ctx, launch_volume_spectrum(ctx, multiplicity, volume, n_sd, ctx->ws.spec_edges, n_edges, count,
+                                                 sum_xi, sum_xi_v));
+}
 
 int sdm_debug_outputs(sdm_ctx* ctx, int32_t* perm_out, int64_t* gamma_out, int64_t* gamma_clamped_out,
                       int32_t* cell_start_out) {

@@ -23,6 +23,9 @@ constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
 // Largest cell the register-resident per-cell sort of the fast path handles (one warp, 8 keys per lane).
 constexpr int CELL_FAST_MAX = 256;
 
+// Largest number of bin edges sdm_volume_spectrum accepts (edges + per-bin sums live in shared memory).
+constexpr int SPECTRUM_MAX_EDGES = 1025;
+
 // Compaction tile.
 constexpr int CMP_BLOCK = 256;
 constexpr int CMP_ITEMS = 8;
@@ -54,6 +57,7 @@ struct Workspace {
     u64* buf_a;       // max_n_sd
     u64* buf_b;       // max_n_sd
     u32* cmp_state;   // max compaction tiles
+    double* spec_edges;  // SPECTRUM_MAX_EDGES volume edges of sdm_volume_spectrum
     u64* scan_state;  // k_cell_scan slab states (epoch-tagged; zeroed at init)
     size_t scan_state_bytes;
     size_t total_bytes;
@@ -73,7 +77,7 @@ struct Plan {  // per-step derived quantities
 namespace sdm {
 // Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
 enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
-                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_CLASSES };
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_CLASSES };
 // What the last general-path step learned about the cell_id array (pinned host memory, written by an
 // asynchronous copy; valid once `verdict_event` has completed).
 struct Verdict { u32 unsorted; u32 max_count; };
@@ -176,6 +180,9 @@ cudaError_t launch_compact(sdm_ctx* ctx, int64_t* xi, double* v, int32_t* cell_i
 cudaError_t launch_cell_stats(sdm_ctx* ctx, const int64_t* xi, const double* v, const int32_t* cell_id,
                               int64_t n_sd, int32_t n_cell, int32_t* count, int64_t* sum_xi,
                               double* sum_xi_v, double* sum_xi_v2);
+cudaError_t launch_volume_spectrum(sdm_ctx* ctx, const int64_t* xi, const double* v, int64_t n_sd,
+                                   const double* edges_dev, int32_t n_edges, int64_t* count, int64_t* sum_xi,
+                                   double* sum_xi_v);
 cudaError_t launch_philox_fill(sdm_ctx* ctx, const PhiloxKeys& pk, u64 i0, int64_t n, u32* key_out,
                                double* u_out);
 cudaError_t launch_kernel_eval(sdm_ctx* ctx, const KernelParams& kp, const double* vj, const double* vk,

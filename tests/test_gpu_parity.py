@@ -592,3 +592,53 @@ def test_shards_with_index_base_reproduce_the_unsharded_step(dev, name, path):
             lo, n = sh.index_base, sw.n_sd
             assert np.array_equal(xi.cpu().numpy(), ow.xi[lo:lo + n])
             assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v[lo:lo + n].view(np.int64))
+
+
+# ------------------------------------------------------------------------------------------- NEXT-2: spectrum
+def _paper_volume_edges():
+    return 4.0 / 3.0 * np.pi * np.logspace(np.log10(10e-6), np.log10(5e-3), 32) ** 3
+
+
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg3", "cfg4"])
+def test_volume_spectrum_against_oracle(dev, name):
+    """sdm_volume_spectrum on the paper's 31 bins: counts and sum xi exact, sum xi v within 1e-12 relative."""
+    sdm = _sdm()
+    w = W.small(name)
+    edges = _paper_volume_edges()
+    if name in ("cfg3", "cfg4"):                     # their spectra sit below 10 um: bins that actually fill
+        edges = np.exp(np.linspace(np.log(w.v[w.v > 0].min() * 0.5), np.log(w.v.max() * 0.9), 40))
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        kp = _gkp(w)
+        for s in range(3):
+            ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, w.seed, s)
+        got = [t.cpu().numpy() for t in ctx.volume_spectrum(xi, v, edges)]
+        hx, hv = xi.cpu().numpy(), v.cpu().numpy()
+    want = oracle.volume_spectrum(hx, hv, edges)
+    assert want[0].sum() > 0.5 * w.n_sd
+    assert np.array_equal(got[0], want[0])
+    assert np.array_equal(got[1], want[1])
+    assert np.allclose(got[2], want[2], rtol=VOL_RTOL, atol=0.0)
+
+
+def test_volume_spectrum_edges_and_degenerate_inputs(dev):
+    sdm = _sdm()
+    edges = np.array([1.0, 2.0, 4.0, 8.0])
+    v = np.array([0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 7.9, 8.0, 9.0, np.nan])
+    xi = np.array([100, 1, 2, 3, 4, 5, 6, 700, 800, 900], np.int64)
+    with sdm.SDMContext(1024, 1, device=dev) as ctx:
+        got = [t.cpu().numpy() for t in ctx.volume_spectrum(torch.from_numpy(xi).to(dev), torch.from_numpy(v).to(dev), edges)]
+        assert got[0].tolist() == [2, 2, 2] and got[1].tolist() == [3, 7, 11]
+        assert got[2].tolist() == [1 * 1.0 + 2 * 1.5, 3 * 2.0 + 4 * 3.0, 5 * 4.0 + 6 * 7.9]
+        # all in one bin (one 32-lane group per warp), ragged length, two edges only
+        n = 1000 + 7
+        xi1 = torch.full((n,), 3, dtype=torch.int64, device=dev)
+        v1 = torch.full((n,), 1.25, dtype=torch.float64, device=dev)
+        c, sx, sv = ctx.volume_spectrum(xi1, v1, [1.0, 2.0])
+        assert c.item() == n and sx.item() == 3 * n and sv.item() == 3 * n * 1.25
+        # empty input, and bad edges
+        c, sx, sv = ctx.volume_spectrum(xi1, v1, edges, n_sd=0)
+        assert c.sum().item() == 0
+        for bad in ([1.0], [2.0, 1.0], [1.0, float("inf")], list(range(1, 1028))):
+            with pytest.raises(sdm.SDMError):
+                ctx.volume_spectrum(xi1, v1, bad)
