@@ -642,3 +642,35 @@ def test_volume_spectrum_edges_and_degenerate_inputs(dev):
         for bad in ([1.0], [2.0, 1.0], [1.0, float("inf")], list(range(1, 1028))):
             with pytest.raises(sdm.SDMError):
                 ctx.volume_spectrum(xi1, v1, bad)
+
+
+# ------------------------------------------------------------------------------------------- races / path equality
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_full_size_paths_agree_and_repeat(dev, name):
+    """BASELINE.json sizes: the three paths give the same bits, and running a path twice from the same state
+    gives the same bits again (a race in the look-back, the rank tables, the tie repair or the fused kernel's
+    staging would show up as a difference between runs or paths).  The oracle comparison at these sizes is
+    test_full_size_configs_two_steps; this one needs no CPU time, so it runs more steps."""
+    sdm = _sdm()
+    w = FULL[name]()
+    n, n_steps = w.n_sd, 4
+    kp = _gkp(w)
+    results = []
+    with sdm.SDMContext(n, w.n_cell, device=dev) as ctx:
+        ctx.set_option(sdm.OPT_TRACK_ZEROS, 1)
+        for path in (sdm.PATH_GENERAL, sdm.PATH_CELL_SORTED, sdm.PATH_HYBRID, sdm.PATH_GENERAL, sdm.PATH_CELL_SORTED):
+            ctx.set_path(path)
+            xi, v, cell = _to_dev(w, dev)
+            m = n
+            for s in range(n_steps):
+                ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, w.seed, s, n_sd=m)
+                if w.compact_every:
+                    m = ctx.remove_zero_multiplicity(xi, v, cell, n_sd=m)
+            assert ctx.poll_error() == 0
+            results.append((m, xi[:m].clone(), v[:m].clone()))
+    m0, xi0, v0 = results[0]
+    assert int((xi0 != torch.from_numpy(w.xi[:m0]).to(dev)).sum()) > 0        # something did collide
+    for m, xi, v in results[1:]:
+        assert m == m0
+        assert torch.equal(xi, xi0)
+        assert torch.equal(v.view(torch.int64), v0.view(torch.int64))
