@@ -210,6 +210,16 @@ k_cell_digit_hist(const int32_t* __restrict__ cell_id, u32 n_sd, int n_cell, int
 #pragma unroll
             for (int k = 0; k < CDH_ITEMS; ++k) c[k] = (i0 + k < n_sd) ? __ldg(cell_id + i0 + k) : -1;
         }
+        // grouped input (whole warp inside one cell): one add of 32 x CDH_ITEMS per digit instead of 128
+        // same-address atomics, which shared memory would serialise
+        const bool full = i0 + CDH_ITEMS <= n_sd;
+        const bool same = full && c[0] == c[1] && c[0] == c[2] && c[0] == c[3] && (u32)c[0] < (u32)n_cell;
+        const int c_first = __shfl_sync(0xffffffffu, c[0], 0);  // every lane takes part, whatever `same` says
+        if (__all_sync(0xffffffffu, same && c[0] == c_first)) {
+            if ((tid & 31) == 0)
+                for (int q = 0; q < n_cpass; ++q) atomicAdd(&s_hist[q][((u32)c[0] >> (8 * q)) & 0xFFu], 32u * CDH_ITEMS);
+            continue;
+        }
 #pragma unroll
         for (int k = 0; k < CDH_ITEMS; ++k) {
             if (i0 + k < n_sd) {
