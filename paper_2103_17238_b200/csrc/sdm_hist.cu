@@ -13,7 +13,7 @@ constexpr int SMEM_CELLS = 2048;      // cell histograms this small are built in
 
 template <bool HAS_CELLS>
 __global__ void __launch_bounds__(HIST_BLOCK)
-k_keys_hist(const int32_t* __restrict__ cell_id, long long n_sd, int n_cell, int n_cpass, int skip,
+k_keys_hist(const int32_t* __restrict__ cell_id, u32 n_sd /* < 2^30 */, int n_cell, int n_cpass, int skip,
             PhiloxKeys pk, u64* __restrict__ sortkey, u32* __restrict__ digit_hist,
             u32* __restrict__ cell_count, u32* __restrict__ ctl, u32* __restrict__ sticky) {
     __shared__ u32 s_hist[MAX_PASSES][RADIX];
@@ -27,21 +27,21 @@ k_keys_hist(const int32_t* __restrict__ cell_id, long long n_sd, int n_cell, int
         for (int q = tid; q < n_cell; q += HIST_BLOCK) s_cells[q] = 0;
     __syncthreads();
 
-    const long long chunk = (long long)HIST_BLOCK * HIST_ROUNDS;
-    const long long n_chunks = (n_sd + chunk - 1) / chunk;
+    const u32 chunk = HIST_BLOCK * HIST_ROUNDS;
+    const u32 n_chunks = (n_sd + chunk - 1) / chunk;
     bool bad = false, unsorted = false;
-    for (long long ch = blockIdx.x; ch < n_chunks; ch += gridDim.x) {
-        const long long base = ch * chunk;
+    for (u32 ch = blockIdx.x; ch < n_chunks; ch += gridDim.x) {
+        const u32 base = ch * chunk;
         int c[HIST_ROUNDS];
 #pragma unroll
         for (int r = 0; r < HIST_ROUNDS; ++r) {
-            const long long i = base + (long long)r * HIST_BLOCK + tid;
+            const u32 i = base + (u32)r * HIST_BLOCK + tid;
             c[r] = 0;
             if (HAS_CELLS && i < n_sd) c[r] = __ldg(cell_id + i);
         }
 #pragma unroll
         for (int r = 0; r < HIST_ROUNDS; ++r) {
-            const long long i = base + (long long)r * HIST_BLOCK + tid;
+            const u32 i = base + (u32)r * HIST_BLOCK + tid;
             const bool valid = i < n_sd;
             int cc = c[r];
             if (HAS_CELLS) {
@@ -259,11 +259,11 @@ cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd,
     const int n_cpass = plan.n_cpass;
     LaunchScope scope(ctx, PROF_KEYS_HIST);
     if (n_cell > 1)
-        k_keys_hist<true><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, plan.skip, pk, sortkey_out,
+        k_keys_hist<true><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, (u32)n_sd, n_cell, n_cpass, plan.skip, pk, sortkey_out,
                                                                  ctx->ws.digit_hist, ctx->ws.cell_count,
                                                                  ctx->ws.ctl, ctx->ws.sticky);
     else
-        k_keys_hist<false><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, n_sd, n_cell, n_cpass, plan.skip, pk, sortkey_out,
+        k_keys_hist<false><<<grid, HIST_BLOCK, 0, ctx->stream>>>(cell_id, (u32)n_sd, n_cell, n_cpass, plan.skip, pk, sortkey_out,
                                                                   ctx->ws.digit_hist, ctx->ws.cell_count,
                                                                   ctx->ws.ctl, ctx->ws.sticky);
     return cudaGetLastError();
