@@ -32,12 +32,16 @@ k_keys_hist(const int32_t* __restrict__ cell_id, u32 n_sd /* < 2^30 */, int n_ce
     bool bad = false, unsorted = false;
     for (u32 ch = blockIdx.x; ch < n_chunks; ch += gridDim.x) {
         const u32 base = ch * chunk;
-        int c[HIST_ROUNDS];
+        int c[HIST_ROUNDS], c_before[HIST_ROUNDS];  // c_before: lane 0's predecessor, loaded with the rest (no dependent load later)
 #pragma unroll
         for (int r = 0; r < HIST_ROUNDS; ++r) {
             const u32 i = base + (u32)r * HIST_BLOCK + tid;
             c[r] = 0;
-            if (HAS_CELLS && i < n_sd) c[r] = __ldg(cell_id + i);
+            c_before[r] = -1;
+            if (HAS_CELLS && i < n_sd) {
+                c[r] = __ldg(cell_id + i);
+                if (lane == 0 && i > 0) c_before[r] = __ldg(cell_id + i - 1);
+            }
         }
 #pragma unroll
         for (int r = 0; r < HIST_ROUNDS; ++r) {
@@ -48,7 +52,7 @@ k_keys_hist(const int32_t* __restrict__ cell_id, u32 n_sd /* < 2^30 */, int n_ce
                 if (valid && (cc < 0 || cc >= n_cell)) { bad = true; cc = cc < 0 ? 0 : n_cell - 1; }
                 // cell_id non-decreasing?  (selects the cell-sorted fast path)
                 int prev = __shfl_up_sync(0xffffffffu, cc, 1);
-                if (lane == 0) prev = (valid && i > 0) ? __ldg(cell_id + i - 1) : cc;
+                if (lane == 0) prev = c_before[r];  // -1 at the array start and past its end: never > cc
                 if (valid && prev > cc) unsorted = true;
             }
             const u32 active = __ballot_sync(0xffffffffu, valid);
