@@ -319,6 +319,7 @@ def run_ours(args):
     for k in kernels.values():
         k["share_of_kernel_time"] = k["ms_total"] / tot_ms
     dom = max(kernels, key=lambda nm: kernels[nm]["ms_total"]) if kernels else None
+    warp_inst = None
     traffic = None  # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
     try:
         import csv
@@ -326,6 +327,8 @@ def run_ours(args):
             for row in csv.DictReader(f):
                 if row["workload"] == args.workload and row["kernel"] == dom:
                     traffic = float(row["dram_bytes_per_launch"])
+                    if row.get("warp_instructions_per_launch"):
+                        warp_inst = float(row["warp_instructions_per_launch"])
     except Exception:
         pass
     roofline = None
@@ -334,6 +337,17 @@ def run_ours(args):
                     "frac": kernels[dom]["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
                     "ms_per_launch": kernels[dom]["ms_per_launch"], "launches": kernels[dom]["launches"],
                     "algorithmic_bytes_per_launch": kernels[dom]["algorithmic_bytes_per_launch"]}
+    # second view of the dominant kernel: issue slots.  peak = SMs x 4 schedulers x 1 warp instruction / clock at the
+    # sampled SM clock (B300_MICROARCH.md: one issue per SMSP per clock; ALU and FMA pipes each take one per 2 clocks);
+    # achieved = warp instructions per launch (ncu, profiles/traffic.csv) / measured launch time
+    roofline_alu = None
+    if dom and warp_inst:
+        sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+        n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_issue = n_sm * 4 * sm_mhz * 1e6 / 1e9   # G warp-instructions / s
+        ach = warp_inst / (kernels[dom]["ms_per_launch"] * 1e-3) / 1e9
+        roofline_alu = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": peak_issue, "unit": "G warp-inst/s",
+                        "frac": ach / peak_issue, "warp_instructions_per_launch": warp_inst}
     # bytes the executed path must move per SD-step = sum of its kernels' algorithmic bytes; next to it the
     # figure SURVEY 8(d) quotes for north_star's own pass structure (general LSD path + separate zero scan)
     step_bytes = sum(ab.get(nm, 0) * k["launches"] for nm, k in kernels.items()) / max(min(args.steps, block), 1)
@@ -417,7 +431,7 @@ def run_ours(args):
             "config": workload_config(w, args.workload, {"parallelism": f"independent shards x{world} (no collective)",
                                                          "path": {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid"}.get(last_path, str(last_path)),
                                                          "track_zeros": not args.no_track_zeros}),
-            "roofline": roofline, "step_roofline": {"algorithmic_bytes_per_sd_step": step_bytes, "gbs": step_gbs,
+            "roofline": roofline, "roofline_alu": roofline_alu, "step_roofline": {"algorithmic_bytes_per_sd_step": step_bytes, "gbs": step_gbs,
                                                     "frac": step_gbs / peak, "peak": peak,
                                                     "north_star_bytes_per_sd_step": ns_bytes,
                                                     "north_star_equivalent_gbs": ns_gbs,
