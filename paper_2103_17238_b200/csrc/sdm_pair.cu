@@ -15,7 +15,7 @@
 
 namespace sdm {
 
-constexpr int PAIR_BLOCK = 256;
+constexpr int PAIR_BLOCK = 128;
 
 __global__ void __launch_bounds__(PAIR_BLOCK) k_pair(const PairArgs a) {
     const u32 t = blockIdx.x * PAIR_BLOCK + threadIdx.x;
