@@ -20,9 +20,11 @@
  *  - Errors: every entry point returns an sdm_status (0 = SDM_OK, negative = error).  Nothing is
  *    printed, nothing throws.  Misuse visible on the host -> SDM_ERR_INVALID_ARG / SDM_ERR_CAPACITY
  *    before any kernel is launched.  Data errors only visible on the device (cell_id outside
- *    [0, n_cell), multiplicity < 0) set a sticky flag reported by sdm_poll_error() and by the next
- *    synchronising call as SDM_ERR_BAD_DATA; the step stays memory-safe but its output is then
- *    unspecified.
+ *    [0, n_cell); an input that an explicitly chosen CELL_SORTED / HYBRID path cannot take) set a sticky
+ *    flag reported by sdm_poll_error() and by the next synchronising call as SDM_ERR_BAD_DATA; the step
+ *    stays memory-safe but its output is then unspecified.  Multiplicities are NOT range-checked: a
+ *    negative multiplicity or a negative / non-finite volume is the caller's responsibility (the oracle does
+ *    not define them either).
  *  - There is no CPU fallback: without a CUDA device sdm_init() returns SDM_ERR_CUDA.
  */
 #ifndef SDM_B200_H_
@@ -58,21 +60,24 @@ typedef struct {
     double E; /* geometric collision efficiency, >= 0 (configs use 1.0) */
 } sdm_kernel_params;
 
-/* Path selection for sdm_coalescence_step (sdm_set_path).  Every path produces the same bits.
+/* Path selection for sdm_coalescence_step / sdm_coalescence_steps (sdm_set_path).  Every path produces the same bits.
  *   GENERAL      global stable LSD radix sort of (cell_id, Philox key): north_star (b).  Any input.
  *   CELL_SORTED  per-cell register-resident sort fused with the pair kernel.  Legal
  *                only when cell_id is non-decreasing and no cell holds more than 256 super-droplets.
  *   HYBRID       LSD radix passes over the cell_id digits only (grouping the indices by cell), then the same
  *                fused per-cell sort + pair kernel, gathering through the sorted indices.  Any order of
  *                cell_id; legal when n_cell > 1 and no cell holds more than 256 super-droplets.
- *                CELL_SORTED and HYBRID verify their preconditions on the device BEFORE anything is updated:
- *                on a violation the step is NOT applied and the sticky SDM_ERR_BAD_DATA flag is set.
- *   AUTO         (default) the first step on a given (cell_id pointer, n_sd, n_cell) takes GENERAL, which
- *                also records whether the array is sorted and its largest cell; later steps on the same
- *                triple take CELL_SORTED or HYBRID when that verdict allows it.  If cell_id was then
- *                modified in place so that the verdict no longer holds, the device check above catches it
- *                (step skipped, SDM_ERR_BAD_DATA at the next poll, verdict reset).  Calling sdm_set_path()
- *                -- with any value -- also resets the verdict: do so after rewriting cell_id in place. */
+ *                An explicitly chosen CELL_SORTED or HYBRID verifies its precondition on the device BEFORE anything
+ *                is updated: on a violation (the caller's error) the step is NOT applied and the sticky
+ *                SDM_ERR_BAD_DATA flag is set.  Both stay fully asynchronous.
+ *   AUTO         (default) never refuses valid input.  Every step first analyses cell_id on the device (one
+ *                streaming read: range, order, largest cell) and the host waits for that verdict -- a few
+ *                microseconds, through a mapped status word, without draining work enqueued behind it -- before
+ *                it enqueues either the fused kernel (CELL_SORTED when the array is non-decreasing, HYBRID when the
+ *                previous GENERAL step on the same array saw small cells in any order) or the GENERAL path.  So
+ *                cell_id may be rewritten in place between steps (a displacement step does exactly that): the
+ *                next step simply takes the path that fits.  sdm_coalescence_steps pays the analysis once per
+ *                call instead of once per step.  sdm_set_path() forgets what was learned. */
 typedef enum { SDM_PATH_AUTO = 0, SDM_PATH_GENERAL = 1, SDM_PATH_CELL_SORTED = 2, SDM_PATH_HYBRID = 3 } sdm_path;
 
 /* Bytes of device workspace sdm_init() needs for problems up to (max_n_sd, max_n_cell).
@@ -106,6 +111,24 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
 int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, const int32_t* cell_id,
                          int64_t n_sd, int32_t n_cell, double dt, double dV,
                          const sdm_kernel_params* kp, uint64_t seed, uint64_t step);
+
+/* The time loop on the device ("API in brief": the Particulator "control[s] time-stepping"; the
+ * loop itself is in the snippet that PAPER.md:80-84 announces and omits, so its statement is SURVEY 8(c)
+ * `oracle_run`): exactly
+ *     for s in 0 .. n_steps-1:
+ *         sdm_coalescence_step(..., n_sd, ..., seed, step0 + s)
+ *         if compact_every > 0 and (s + 1) % compact_every == 0:
+ *             sdm_remove_zero_multiplicity(..., n_sd, &n_sd)
+ * with the same bits as that sequence of calls, but enqueued without a host round trip per step: the path is chosen
+ * once per call (see sdm_path), cell boundaries -- cell_id cannot change during the call -- are computed once, and a
+ * due compaction costs nothing while no multiplicity is 0: every fused step counts the zeros it leaves behind, and
+ * only a non-zero count at a due step halts the run on the device until the host has compacted.  cell_id is written
+ * only by a compaction.  *n_sd_out (host) receives the final number of super-droplets; the call synchronises the
+ * stream once, at its end, and then also reports a pending SDM_ERR_BAD_DATA.  n_steps == 0 and n_sd == 0 are no-ops.
+ * Errors: as sdm_coalescence_step, plus INVALID_ARG for n_steps < 0, compact_every < 0 or a null n_sd_out. */
+int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, int32_t* cell_id, int64_t n_sd,
+                          int32_t n_cell, double dt, double dV, const sdm_kernel_params* kp, uint64_t seed,
+                          uint64_t step0, int64_t n_steps, int64_t compact_every, int64_t* n_sd_out /* host */);
 
 /* Stable stream compaction (north_star (d)): removes every entry whose
  * multiplicity is 0 from (multiplicity, volume, cell_id), in place; survivors keep their relative
@@ -172,8 +195,8 @@ int sdm_set_path(sdm_ctx* ctx, int path);
 enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1, SDM_OPT_INDEX_BASE = 2, SDM_OPT_SKIP_KEY_DIGITS = 3 };
 int sdm_set_option(sdm_ctx* ctx, int option, int64_t value);
 
-/* Which path the most recent sdm_coalescence_step took (an sdm_path value other than AUTO), or 0 if
- * none ran yet.  Synchronises the stream when the decision was taken on the device. */
+/* Which path the most recent step took (an sdm_path value other than AUTO), or 0 if none ran yet.  Host-side
+ * bookkeeping: does not touch the stream. */
 int sdm_last_path(sdm_ctx* ctx);
 
 /* End-to-end variant with HOST buffers (bench.py `e2e`): copies multiplicity, volume and cell_id to the

@@ -26,7 +26,7 @@ OPT_SKIP_KEY_DIGITS = 3
 SDM_OK = 0
 
 EXPORTS = [
-    "sdm_workspace_bytes", "sdm_init", "sdm_coalescence_step", "sdm_remove_zero_multiplicity",
+    "sdm_workspace_bytes", "sdm_init", "sdm_coalescence_step", "sdm_coalescence_steps", "sdm_remove_zero_multiplicity",
     "sdm_cell_stats", "sdm_debug_outputs", "sdm_set_path", "sdm_last_path", "sdm_host_staging_bytes",
     "sdm_bind_host_staging", "sdm_coalescence_step_host", "sdm_poll_error", "sdm_launch_count",
     "sdm_philox_fill", "sdm_kernel_eval", "sdm_strerror", "sdm_destroy", "sdm_profile_enable",
@@ -79,6 +79,8 @@ def load_library():
     lib.sdm_init.restype = C.c_int
     lib.sdm_coalescence_step.argtypes = [vp, vp, vp, vp, i64, i32, dbl, dbl, kpp, u64, u64]
     lib.sdm_coalescence_step.restype = C.c_int
+    lib.sdm_coalescence_steps.argtypes = [vp, vp, vp, vp, i64, i32, dbl, dbl, kpp, u64, u64, i64, i64, C.POINTER(i64)]
+    lib.sdm_coalescence_steps.restype = C.c_int
     lib.sdm_remove_zero_multiplicity.argtypes = [vp, vp, vp, vp, i64, C.POINTER(i64)]
     lib.sdm_remove_zero_multiplicity.restype = C.c_int
     lib.sdm_cell_stats.argtypes = [vp, vp, vp, vp, i64, i32, vp, vp, vp, vp]
@@ -208,6 +210,19 @@ class SDMContext:
                                             _ptr(cell_id, t.int32), n, int(n_cell), float(dt), float(dV),
                                             C.byref(kp), int(seed), int(step))
         _check(rc, "sdm_coalescence_step")
+
+    def coalescence_steps(self, multiplicity, volume, cell_id, n_cell, dt, dV, kp, seed, step0, n_steps,
+                          compact_every=0, n_sd=None) -> int:
+        """sdm_coalescence_steps: n_steps steps (+ a compaction every `compact_every` steps) in one call; returns
+        the final number of super-droplets."""
+        t = self._torch
+        n = int(multiplicity.shape[0] if n_sd is None else n_sd)
+        out = C.c_int64(n)
+        rc = self._lib.sdm_coalescence_steps(self._h, _ptr(multiplicity, t.int64), _ptr(volume, t.float64),
+                                             _ptr(cell_id, t.int32), n, int(n_cell), float(dt), float(dV), C.byref(kp),
+                                             int(seed), int(step0), int(n_steps), int(compact_every), C.byref(out))
+        _check(rc, "sdm_coalescence_steps")
+        return int(out.value)
 
     def remove_zero_multiplicity(self, multiplicity, volume, cell_id, n_sd=None) -> int:
         t = self._torch

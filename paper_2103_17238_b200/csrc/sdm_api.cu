@@ -1,6 +1,7 @@
 // The C ABI of libsdm_b200.so (include/sdm.h): argument validation, workspace carving and the
 // launch sequence of one coalescence step.  No device memory is allocated here; everything is
 // enqueued on the caller's stream.
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -71,6 +72,7 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     w.spec_edges = reinterpret_cast<double*>(take((size_t)SPECTRUM_MAX_EDGES * 8));
     w.scan_state_bytes = ((size_t)max_n_cell / 4096 + 2) * 8;
     w.scan_state = reinterpret_cast<u64*>(take(w.scan_state_bytes));
+    w.run = reinterpret_cast<u32*>(take(RUN_WORDS * 4));
     w.total_bytes = off;
     return w;
 }
@@ -109,7 +111,10 @@ static void free_ctx(sdm_ctx* ctx) {
     }
     if (ctx->verdict_host) cudaFreeHost(ctx->verdict_host);
     if (ctx->status_host) cudaFreeHost(ctx->status_host);
+    if (ctx->mapped) cudaFreeHost(const_cast<u32*>(ctx->mapped));
     if (ctx->verdict_event) cudaEventDestroy(ctx->verdict_event);
+    for (cudaEvent_t e : ctx->chunk_event)
+        if (e) cudaEventDestroy(e);
     delete ctx;
 }
 
@@ -153,11 +158,18 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
     if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->verdict_host), sizeof(Verdict), cudaHostAllocDefault) != cudaSuccess ||
         cudaHostAlloc(reinterpret_cast<void**>(&ctx->status_host), (STICKY_WORDS + CTL_WORDS) * 4, cudaHostAllocDefault) !=
             cudaSuccess ||
-        cudaEventCreateWithFlags(&ctx->verdict_event, cudaEventDisableTiming) != cudaSuccess) {
+        cudaHostAlloc(reinterpret_cast<void**>(const_cast<u32**>(&ctx->mapped)), MAPPED_WORDS * 4,
+                      cudaHostAllocMapped | cudaHostAllocPortable) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->verdict_event, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->chunk_event[0], cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->chunk_event[1], cudaEventDisableTiming) != cudaSuccess ||
+        init_cell_fused(ctx) != cudaSuccess || init_volume_spectrum(ctx) != cudaSuccess) {
         free_ctx(ctx);
         return SDM_ERR_CUDA;
     }
+    for (int q = 0; q < MAPPED_WORDS; ++q) ctx->mapped[q] = 0u;
     if (cudaMemsetAsync(ctx->ws.sticky, 0, STICKY_WORDS * 4, ctx->stream) != cudaSuccess ||
+        cudaMemsetAsync(ctx->ws.run, 0, RUN_WORDS * 4, ctx->stream) != cudaSuccess ||
         cudaMemsetAsync(ctx->ws.ctl, 0, CTL_WORDS * 4, ctx->stream) != cudaSuccess ||
         cudaMemsetAsync(ctx->ws.scan_state, 0, ctx->ws.scan_state_bytes, ctx->stream) != cudaSuccess) {
         free_ctx(ctx);
@@ -199,7 +211,7 @@ const char* sdm_strerror(int status) {
         case SDM_ERR_INVALID_ARG: return "invalid argument";
         case SDM_ERR_CAPACITY: return "problem larger than the context capacity (or workspace too small)";
         case SDM_ERR_CUDA: return "CUDA error";
-        case SDM_ERR_BAD_DATA: return "bad data on device (cell_id out of range or negative multiplicity)";
+        case SDM_ERR_BAD_DATA: return "bad data on device (cell_id out of range, or an input the explicitly chosen path cannot take)";
         default: return "unknown status";
     }
 }
@@ -289,6 +301,213 @@ static int validate_step(sdm_ctx* ctx, const void* xi, const void* v, const void
     return SDM_OK;
 }
 
+namespace {
+
+// What one step works on: the caller's arrays and the per-call constants (everything but the step index).
+struct StepArgs {
+    int64_t* xi;
+    double* v;
+    const int32_t* cell_id;
+    int64_t n_sd;
+    int32_t n_cell;
+    double dtdV;
+    KernelParams dkp;
+    uint64_t seed;
+};
+
+StepArgs make_step_args(int64_t* xi, double* v, const int32_t* cell_id, int64_t n_sd, int32_t n_cell, double dt,
+                        double dV, const sdm_kernel_params* kp, uint64_t seed) {
+    StepArgs A;
+    A.xi = xi; A.v = v; A.cell_id = cell_id; A.n_sd = n_sd; A.n_cell = n_cell;
+    A.dtdV = dt / dV;
+    A.dkp.kind = kp->kind;
+    A.dkp.b = kp->b;
+    A.dkp.Epi = kp->E * 3.141592653589793;
+    A.seed = seed;
+    return A;
+}
+
+// one epoch per step (and per analysis) tags the device-side flags and scan states (no per-step memsets of them)
+int next_epoch(sdm_ctx* ctx) {
+    if (++ctx->epoch >= (1u << 30)) {
+        ctx->epoch = 2;
+        return note_cuda(ctx, cudaMemsetAsync(ctx->ws.scan_state, 0, ctx->ws.scan_state_bytes, ctx->stream));
+    }
+    return SDM_OK;
+}
+
+int clear_debug_gammas(sdm_ctx* ctx, int64_t n_sd) {
+    int rc;
+    if (ctx->dbg_gamma)
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_gamma, 0, (size_t)n_sd * 8, ctx->stream)))) return rc;
+    if (ctx->dbg_gamma_clamped)
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_gamma_clamped, 0, (size_t)n_sd * 8, ctx->stream)))) return rc;
+    return SDM_OK;
+}
+
+// GENERAL path, north_star (b) literally: keys + histograms, cell scan, LSD radix passes, tie repair, pairs.
+int enqueue_general_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
+    int rc;
+    const Plan plan = make_plan(A.n_sd, A.n_cell, ctx->skip_key_digits);
+    if (!plan_fits(plan)) return SDM_ERR_CAPACITY;
+    cudaStream_t st = ctx->stream;
+    Workspace& ws = ctx->ws;
+    if ((rc = clear_debug_gammas(ctx, A.n_sd))) return rc;
+    if ((rc = next_epoch(ctx))) return rc;
+    const PhiloxKeys pk = make_philox_keys(A.seed, step, ctx->index_base);
+    ctx->zero_hint_valid = 0;
+    // zero the per-step control block, the digit histograms, the cell counts and the look-back states
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
+    if (A.n_cell > 1)
+        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.cell_count, 0, ((size_t)A.n_cell + 1) * 4, st)))) return rc;
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)plan.n_pass * plan.n_tiles * RADIX * 4, st))))
+        return rc;
+    // a1 + a2: keys, digit histograms, cell histogram; then the cell scan
+    if ((rc = note_cuda(ctx, launch_keys_hist(ctx, A.cell_id, A.n_sd, A.n_cell, plan, pk, ws.buf_b)))) return rc;
+    if ((rc = note_cuda(ctx, launch_cell_scan(ctx, A.n_cell, A.n_sd)))) return rc;
+    // a3: LSD radix passes, ping-pong between buf_b and buf_a
+    u64* in = ws.buf_b;
+    u64* out = ws.buf_a;
+    for (int pass = 0; pass < plan.n_pass; ++pass) {
+        if ((rc = note_cuda(ctx, launch_sort_pass(ctx, pass, in, out, A.n_sd, plan)))) return rc;
+        u64* t = in; in = out; out = t;
+    }
+    if (plan.skip > 0)  // exact (key, index) order inside the runs the skipped digits left tied
+        if ((rc = note_cuda(ctx, launch_tie_repair(ctx, in, A.n_sd, plan, pk)))) return rc;
+    const u64* sorted = in;
+    if (ctx->dbg_perm)
+        if ((rc = note_cuda(ctx, launch_debug_perm(ctx, sorted, A.n_sd, plan)))) return rc;
+    // a4: pairs
+    if ((rc = note_cuda(ctx, launch_pair(ctx, sorted, A.xi, A.v, A.n_sd, A.n_cell, plan, A.dtdV, A.dkp, pk)))) return rc;
+    ctx->last_path = SDM_PATH_GENERAL;
+    // what this step learned about cell_id is AUTO's hint for the next one (asynchronous copy)
+    ctx->verdict_valid = 0;
+    if (A.n_cell > 1) {
+        if ((rc = note_cuda(ctx, cudaMemcpyAsync(ctx->verdict_host, ws.ctl + CTL_UNSORTED, sizeof(Verdict),
+                                                 cudaMemcpyDeviceToHost, st))))
+            return rc;
+        if ((rc = note_cuda(ctx, cudaEventRecord(ctx->verdict_event, st)))) return rc;
+        ctx->verdict_cell_ptr = A.cell_id;
+        ctx->verdict_n_sd = A.n_sd;
+        ctx->verdict_n_cell = A.n_cell;
+        ctx->verdict_valid = 1;
+    }
+    return SDM_OK;
+}
+
+// The index runs of the fused kernel: CELL_SORTED reads the arrays directly (kind 0); HYBRID gathers through the
+// words `run_idx` (kind 1: u64, kind 2: u32) that LSD passes over the cell_id digits alone have grouped by cell.
+struct FusedSource {
+    int kind;
+    const void* run_idx;
+    int idxbits;
+};
+
+// cell boundaries straight from cell_id (CELL_SORTED)
+int enqueue_sorted_prepare(sdm_ctx* ctx, const StepArgs& A, int rmax, bool strict, FusedSource* src) {
+    int rc;
+    if ((rc = next_epoch(ctx))) return rc;
+    src->kind = 0; src->run_idx = nullptr; src->idxbits = 0;
+    return note_cuda(ctx, launch_cell_bounds(ctx, 0, A.cell_id, A.n_sd, A.n_cell, 0, rmax, strict));
+}
+
+// cell-digit LSD passes + cell boundaries of the grouped words (HYBRID)
+int enqueue_hybrid_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, int rmax, bool strict, FusedSource* src) {
+    int rc;
+    cudaStream_t st = ctx->stream;
+    Workspace& ws = ctx->ws;
+    if ((rc = next_epoch(ctx))) return rc;
+    const int n_cpass = plan.n_cpass;
+    const bool narrow = plan.cbits + plan.idxbits <= 32 && plan.cbits + 12 <= 32;
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)n_cpass * plan.n_tiles * RADIX * 4, st))))
+        return rc;
+    if ((rc = note_cuda(ctx, launch_cell_digit_hist(ctx, A.cell_id, A.n_sd, A.n_cell, plan)))) return rc;
+    void* in = nullptr;
+    void* out = ws.buf_a;
+    for (int pass = 0; pass < n_cpass; ++pass) {
+        if ((rc = note_cuda(ctx, launch_cell_sort_pass(ctx, pass, narrow, A.cell_id, in, out, A.n_sd, A.n_cell, plan))))
+            return rc;
+        in = out;
+        out = (out == (void*)ws.buf_a) ? (void*)ws.buf_b : (void*)ws.buf_a;
+    }
+    src->kind = narrow ? 2 : 1;
+    src->run_idx = in;
+    src->idxbits = plan.idxbits;
+    return note_cuda(ctx, launch_cell_bounds(ctx, src->kind, in, A.n_sd, A.n_cell, plan.idxbits, rmax, strict));
+}
+
+int enqueue_fused_step(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, int rmax, uint64_t step,
+                       const StepLinks& links, bool bump_epoch) {
+    int rc;
+    if ((rc = clear_debug_gammas(ctx, A.n_sd))) return rc;
+    if (bump_epoch && (rc = next_epoch(ctx))) return rc;
+    const PhiloxKeys pk = make_philox_keys(A.seed, step, ctx->index_base);
+    if ((rc = note_cuda(ctx, launch_cell_fused(ctx, src.kind, src.run_idx, src.idxbits, rmax, A.xi, A.v, A.n_sd,
+                                               A.n_cell, A.dtdV, A.dkp, pk, links))))
+        return rc;
+    ctx->last_path = src.kind == 0 ? SDM_PATH_CELL_SORTED : SDM_PATH_HYBRID;
+    return SDM_OK;
+}
+
+// Waits, WITHOUT draining the stream behind it, until k_cell_bounds of `epoch` has published its verdict in the
+// mapped status block; *cls = worst cell-size class (3 = the fused kernel cannot take this input).
+int wait_verdict(sdm_ctx* ctx, u32 epoch, u32* cls) {
+    volatile u32* m = ctx->mapped;
+    for (unsigned long spin = 1;; ++spin) {
+        if (m[MAPPED_VERDICT_EPOCH] == epoch) break;
+        if ((spin & 0xFFFu) == 0) {  // the stream ran dry without a verdict: a launch failed
+            const cudaError_t q = cudaStreamQuery(ctx->stream);
+            if (q == cudaErrorNotReady) { (void)cudaGetLastError(); continue; }
+            if (q != cudaSuccess) return note_cuda(ctx, q);
+            if (m[MAPPED_VERDICT_EPOCH] == epoch) break;
+            return note_cuda(ctx, cudaErrorUnknown);
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    *cls = m[MAPPED_VERDICT_CLASS];
+    return SDM_OK;
+}
+
+int rmax_of_class(u32 cls) { return cls == 0 ? 2 : (cls == 1 ? 4 : 8); }
+
+// AUTO's hint: what the last GENERAL step on this very (cell_id pointer, n_sd, n_cell) saw.  Waits for its
+// asynchronous copy (AUTO waits for the analysis enqueued behind it anyway).  Returns false when there is none.
+bool auto_hint(sdm_ctx* ctx, const StepArgs& A, Verdict* hint) {
+    if (!(ctx->verdict_valid && ctx->verdict_cell_ptr == A.cell_id && ctx->verdict_n_sd == A.n_sd &&
+          ctx->verdict_n_cell == A.n_cell))
+        return false;
+    if (note_cuda(ctx, cudaEventSynchronize(ctx->verdict_event)) != SDM_OK) return false;
+    *hint = *ctx->verdict_host;
+    return true;
+}
+
+// AUTO: analyses cell_id on the device, waits for the verdict and prepares the fused kernel's input when it fits.
+// *fits = false: take the GENERAL path (nothing was updated).  The analysis never raises SDM_ERR_BAD_DATA by itself.
+int auto_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, bool* fits, FusedSource* src, int* rmax) {
+    *fits = false;
+    if (A.n_cell <= 1) return SDM_OK;
+    Verdict hint;
+    const bool have_hint = auto_hint(ctx, A, &hint);
+    if (have_hint && hint.max_count > (u32)CELL_FAST_MAX) return SDM_OK;
+    int rc;
+    u32 cls = 3;
+    if (!have_hint || !hint.unsorted) {
+        if ((rc = enqueue_sorted_prepare(ctx, A, CELL_FAST_MAX / 32, false, src))) return rc;
+        if ((rc = wait_verdict(ctx, ctx->epoch, &cls))) return rc;
+    } else if (hybrid_fits(plan)) {
+        if ((rc = enqueue_hybrid_prepare(ctx, A, plan, CELL_FAST_MAX / 32, false, src))) return rc;
+        if ((rc = wait_verdict(ctx, ctx->epoch, &cls))) return rc;
+    }
+    if (cls <= 2) {
+        *fits = true;
+        *rmax = rmax_of_class(cls);
+    }
+    return SDM_OK;
+}
+
+}  // namespace
+
 int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, const int32_t* cell_id,
                          int64_t n_sd, int32_t n_cell, double dt, double dV, const sdm_kernel_params* kp,
                          uint64_t seed, uint64_t step) {
@@ -299,125 +518,48 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
     if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
     const Plan plan = make_plan(n_sd, n_cell, ctx->skip_key_digits);
     if (!plan_fits(plan)) return SDM_ERR_CAPACITY;
-    cudaStream_t st = ctx->stream;
-    Workspace& ws = ctx->ws;
-
     if (n_sd == 0) {  // legal no-op; the debug cell_start is still defined (all zeros)
         if (ctx->dbg_cell_start)
-            if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_cell_start, 0, ((size_t)n_cell + 1) * 4, st)))) return rc;
-        return SDM_OK;
-    }
-
-    if (ctx->dbg_gamma)
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_gamma, 0, (size_t)n_sd * 8, st)))) return rc;
-    if (ctx->dbg_gamma_clamped)
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_gamma_clamped, 0, (size_t)n_sd * 8, st)))) return rc;
-    const PhiloxKeys pk = make_philox_keys(seed, step, ctx->index_base);
-    KernelParams dkp;
-    dkp.kind = kp->kind;
-    dkp.b = kp->b;
-    dkp.Epi = kp->E * 3.141592653589793;
-    const double dtdV = dt / dV;
-
-    // one epoch per step tags the device-side flags and scan states of this step (no per-step memsets of them)
-    if (++ctx->epoch >= (1u << 30)) {
-        ctx->epoch = 2;
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.scan_state, 0, ws.scan_state_bytes, st)))) return rc;
-    }
-    // ---- path selection (include/sdm.h, sdm_path) ----
-    int path = SDM_PATH_GENERAL;
-    if (n_cell > 1) {
-        if (ctx->path == SDM_PATH_CELL_SORTED || ctx->path == SDM_PATH_HYBRID) {
-            path = ctx->path;
-        } else if (ctx->path == SDM_PATH_AUTO && ctx->verdict_valid && ctx->verdict_cell_ptr == cell_id &&
-                   ctx->verdict_n_sd == n_sd && ctx->verdict_n_cell == n_cell &&
-                   cudaEventQuery(ctx->verdict_event) == cudaSuccess) {
-            if (ctx->verdict_host->max_count <= (u32)CELL_FAST_MAX)
-                path = ctx->verdict_host->unsorted ? SDM_PATH_HYBRID : SDM_PATH_CELL_SORTED;
-        }
-    }
-    if (path == SDM_PATH_HYBRID && !hybrid_fits(plan)) path = SDM_PATH_GENERAL;
-    // register tile of the fused kernel: 32 * rmax >= the largest cell (known from the verdict under AUTO)
-    int rmax = CELL_FAST_MAX / 32;
-    if (ctx->path == SDM_PATH_AUTO && path != SDM_PATH_GENERAL) {
-        const u32 mc = ctx->verdict_host->max_count;
-        rmax = mc <= 64 ? 2 : (mc <= 128 ? 4 : 8);
-    }
-    ctx->zero_hint_valid = 0;
-    if (path == SDM_PATH_CELL_SORTED) {
-        if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, 0, cell_id, n_sd, n_cell, 0, rmax)))) return rc;
-        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, 0, nullptr, 0, rmax, multiplicity, volume, n_sd, n_cell, dtdV, dkp,
-                                                   pk))))
-            return rc;
-        ctx->last_path = SDM_PATH_CELL_SORTED;
-        note_zero_hint(ctx, multiplicity, n_sd);
-        return SDM_OK;
-    }
-    if (path == SDM_PATH_HYBRID) {
-        const int n_cpass = plan.n_cpass;
-        const bool narrow = plan.cbits + plan.idxbits <= 32 && plan.cbits + 12 <= 32;
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)n_cpass * plan.n_tiles * RADIX * 4, st))))
-            return rc;
-        if ((rc = note_cuda(ctx, launch_cell_digit_hist(ctx, cell_id, n_sd, n_cell, plan)))) return rc;
-        void* in = nullptr;
-        void* out = ws.buf_a;
-        for (int pass = 0; pass < n_cpass; ++pass) {
-            if ((rc = note_cuda(ctx, launch_cell_sort_pass(ctx, pass, narrow, cell_id, in, out, n_sd, n_cell, plan))))
+            if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->dbg_cell_start, 0, ((size_t)n_cell + 1) * 4, ctx->stream))))
                 return rc;
-            in = out;
-            out = (out == (void*)ws.buf_a) ? (void*)ws.buf_b : (void*)ws.buf_a;
-        }
-        const int kind = narrow ? 2 : 1;
-        if ((rc = note_cuda(ctx, launch_cell_bounds(ctx, kind, in, n_sd, n_cell, plan.idxbits, rmax)))) return rc;
-        if ((rc = note_cuda(ctx, launch_cell_fused(ctx, kind, in, plan.idxbits, rmax, multiplicity, volume, n_sd, n_cell,
-                                                   dtdV, dkp, pk))))
-            return rc;
-        ctx->last_path = SDM_PATH_HYBRID;
-        note_zero_hint(ctx, multiplicity, n_sd);
         return SDM_OK;
     }
-
-    // zero the per-step control block, the digit histograms, the cell counts and the look-back states
-    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
-    if (n_cell > 1)
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.cell_count, 0, ((size_t)n_cell + 1) * 4, st)))) return rc;
-    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)plan.n_pass * plan.n_tiles * RADIX * 4, st))))
-        return rc;
-
-    // a1 + a2: keys, digit histograms, cell histogram; then the cell scan
-    if ((rc = note_cuda(ctx, launch_keys_hist(ctx, cell_id, n_sd, n_cell, plan, pk, ws.buf_b)))) return rc;
-    if ((rc = note_cuda(ctx, launch_cell_scan(ctx, n_cell, n_sd)))) return rc;
-    // a3: LSD radix passes, ping-pong between buf_b and buf_a
-    u64* in = ws.buf_b;
-    u64* out = ws.buf_a;
-    for (int pass = 0; pass < plan.n_pass; ++pass) {
-        if ((rc = note_cuda(ctx, launch_sort_pass(ctx, pass, in, out, n_sd, plan)))) return rc;
-        u64* t = in; in = out; out = t;
+    const StepArgs A = make_step_args(multiplicity, volume, cell_id, n_sd, n_cell, dt, dV, kp, seed);
+    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u};
+    ctx->zero_hint_valid = 0;
+    // ---- path selection (include/sdm.h, sdm_path) ----
+    FusedSource src;
+    int rmax = CELL_FAST_MAX / 32;
+    bool fused = false;
+    if (n_cell > 1 && ctx->path == SDM_PATH_CELL_SORTED) {
+        if ((rc = enqueue_sorted_prepare(ctx, A, rmax, true, &src))) return rc;
+        fused = true;
+    } else if (n_cell > 1 && ctx->path == SDM_PATH_HYBRID && hybrid_fits(plan)) {
+        if ((rc = enqueue_hybrid_prepare(ctx, A, plan, rmax, true, &src))) return rc;
+        fused = true;
+    } else if (ctx->path == SDM_PATH_AUTO) {
+        if ((rc = auto_prepare(ctx, A, plan, &fused, &src, &rmax))) return rc;
     }
-    if (plan.skip > 0)  // exact (key, index) order inside the runs the skipped digits left tied
-        if ((rc = note_cuda(ctx, launch_tie_repair(ctx, in, n_sd, plan, pk)))) return rc;
-    const u64* sorted = in;
-    if (ctx->dbg_perm)
-        if ((rc = note_cuda(ctx, launch_debug_perm(ctx, sorted, n_sd, plan)))) return rc;
-    // a4: pairs
-    if ((rc = note_cuda(ctx, launch_pair(ctx, sorted, multiplicity, volume, n_sd, n_cell, plan, dtdV, dkp, pk))))
-        return rc;
-    ctx->last_path = SDM_PATH_GENERAL;
-    // what this step learned about cell_id feeds AUTO's choice for the next one (asynchronous copy)
-    ctx->verdict_valid = 0;
-    if (n_cell > 1 && ctx->path == SDM_PATH_AUTO) {
-        if ((rc = note_cuda(ctx, cudaMemcpyAsync(ctx->verdict_host, ws.ctl + CTL_UNSORTED, sizeof(Verdict),
-                                                 cudaMemcpyDeviceToHost, st))))
-            return rc;
-        if ((rc = note_cuda(ctx, cudaEventRecord(ctx->verdict_event, st)))) return rc;
-        ctx->verdict_cell_ptr = cell_id;
-        ctx->verdict_n_sd = n_sd;
-        ctx->verdict_n_cell = n_cell;
-        ctx->verdict_valid = 1;
-    }
+    if (!fused) return enqueue_general_step(ctx, A, step);
+    if ((rc = enqueue_fused_step(ctx, A, src, rmax, step, no_links, false))) return rc;
+    note_zero_hint(ctx, multiplicity, n_sd);
     return SDM_OK;
 }
+
+// ---- sdm_remove_zero_multiplicity and its parts ----
+namespace {
+
+// Enqueues the in-place compaction of a known number of zeros (> 0).
+int enqueue_compact(sdm_ctx* ctx, int64_t* xi, double* v, int32_t* cell_id, int64_t n_sd) {
+    int rc;
+    cudaStream_t st = ctx->stream;
+    const size_t n_tiles = (size_t)((n_sd + CMP_TILE - 1) / CMP_TILE);
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_CMP_TICKET, 0, 4, st)))) return rc;
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.cmp_state, 0, n_tiles * 4, st)))) return rc;
+    return note_cuda(ctx, launch_compact(ctx, xi, v, cell_id, n_sd));
+}
+
+}  // namespace
 
 int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* volume, int32_t* cell_id,
                                  int64_t n_sd, int64_t* n_sd_out) {
@@ -449,14 +591,10 @@ int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* vo
     }
     const int64_t zeros = n_sd > 0 ? (int64_t)hs[STICKY_WORDS + CTL_ZERO_COUNT] : 0;
     const u32 bad_data = hs[STICKY_BAD_DATA];
-    if (zeros > 0) {
-        const size_t n_tiles = (size_t)((n_sd + CMP_TILE - 1) / CMP_TILE);
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.ctl + CTL_CMP_TICKET, 0, 4, st)))) return rc;
-        if ((rc = note_cuda(ctx, cudaMemsetAsync(ctx->ws.cmp_state, 0, n_tiles * 4, st)))) return rc;
-        if ((rc = note_cuda(ctx, launch_compact(ctx, multiplicity, volume, cell_id, n_sd)))) return rc;
-    }
+    if (zeros > 0)
+        if ((rc = enqueue_compact(ctx, multiplicity, volume, cell_id, n_sd))) return rc;
     *n_sd_out = n_sd - zeros;
-    // stable compaction keeps a sorted cell_id sorted and cannot grow a cell: the verdict carries over
+    // stable compaction keeps a sorted cell_id sorted and cannot grow a cell: AUTO's hint carries over
     if (ctx->verdict_valid && ctx->verdict_cell_ptr == cell_id && ctx->verdict_n_sd == n_sd)
         ctx->verdict_n_sd = n_sd - zeros;
     if (bad_data) {
@@ -465,6 +603,164 @@ int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* vo
         return SDM_ERR_BAD_DATA;
     }
     return SDM_OK;
+}
+
+// ---- sdm_coalescence_steps: the time loop on the device ----
+namespace {
+
+constexpr int64_t RUN_CHUNK = 64;  // fused steps enqueued between two looks at the halt word
+
+// Reads and clears the sticky data-error flag after the stream has been drained.
+int finish_run(sdm_ctx* ctx) {
+    int rc;
+    u32 bad = 0;
+    if ((rc = note_cuda(ctx, cudaMemcpyAsync(&bad, ctx->ws.sticky + STICKY_BAD_DATA, 4, cudaMemcpyDeviceToHost,
+                                             ctx->stream))))
+        return rc;
+    if ((rc = note_cuda(ctx, cudaStreamSynchronize(ctx->stream)))) return rc;
+    if (bad) {
+        cudaMemsetAsync(ctx->ws.sticky, 0, STICKY_WORDS * 4, ctx->stream);
+        ctx->verdict_valid = 0;
+        return SDM_ERR_BAD_DATA;
+    }
+    return SDM_OK;
+}
+
+// Fused steps [*s, n_steps) of the run, enqueued chunk by chunk with no host synchronisation in between.  Each step
+// counts the zero multiplicities it leaves behind (slot s mod 3 of the run block); the step after a due
+// compaction looks at that count first and, when it is not 0, HALTS the run: it and every later step already
+// enqueued exit without touching the state, and the host -- which watches the mapped halt word from one chunk
+// behind -- compacts and resumes from the halted step.  Returns with *s = first step not yet applied,
+// *halt_zeros > 0 when a compaction of that many zeros is due before step *s (stream drained), else 0.
+int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, int rmax, uint64_t step0, int64_t* s,
+                    int64_t n_steps, int64_t compact_every, int64_t* halt_zeros) {
+    int rc;
+    cudaStream_t st = ctx->stream;
+    u32* run = ctx->ws.run;
+    *halt_zeros = 0;
+    const int64_t s_begin = *s;
+    ctx->mapped[MAPPED_HALT] = 0u;
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(run + RUN_HALT, 0, 4 * 4, st)))) return rc;  // halt word + three zero slots
+    int64_t enq = s_begin;  // steps enqueued so far
+    int n_chunks = 0;
+    bool halted = false;
+    while (enq < n_steps && !halted) {
+        const int64_t c_end = (n_steps - enq > RUN_CHUNK) ? enq + RUN_CHUNK : n_steps;
+        for (; enq < c_end; ++enq) {
+            StepLinks links;
+            links.zc_accum = run + RUN_ZC0 + (enq % 3);
+            links.zc_clear = run + RUN_ZC0 + ((enq + 1) % 3);
+            const bool due_before = compact_every > 0 && enq > s_begin && (enq % compact_every) == 0;
+            links.zc_check = due_before ? run + RUN_ZC0 + ((enq - 1) % 3) : nullptr;
+            links.halt_tag = (u32)(enq - s_begin) + 1u;
+            if ((rc = enqueue_fused_step(ctx, A, src, rmax, step0 + (uint64_t)enq, links, true))) return rc;
+        }
+        if ((rc = note_cuda(ctx, cudaEventRecord(ctx->chunk_event[n_chunks & 1], st)))) return rc;
+        ++n_chunks;
+        if (n_chunks >= 2) {  // one chunk stays queued behind the one that is running
+            if ((rc = note_cuda(ctx, cudaEventSynchronize(ctx->chunk_event[n_chunks & 1])))) return rc;
+            halted = ctx->mapped[MAPPED_HALT] != 0u;
+        }
+    }
+    if ((rc = note_cuda(ctx, cudaStreamSynchronize(st)))) return rc;
+    std::atomic_thread_fence(std::memory_order_acquire);
+    const u32 tag = ctx->mapped[MAPPED_HALT];
+    if (tag != 0u) {  // steps before s_begin + tag - 1 were applied; that one and all later ones were not
+        *s = s_begin + (int64_t)tag - 1;
+        *halt_zeros = (int64_t)ctx->mapped[MAPPED_ZEROS];
+        return SDM_OK;
+    }
+    *s = n_steps;
+    // a compaction due after the last step: its count sits in that step's slot
+    if (compact_every > 0 && n_steps > s_begin && (n_steps % compact_every) == 0) {
+        u32 z = 0;
+        if ((rc = note_cuda(ctx, cudaMemcpy(&z, run + RUN_ZC0 + ((n_steps - 1) % 3), 4, cudaMemcpyDeviceToHost)))) return rc;
+        *halt_zeros = (int64_t)z;
+    }
+    return SDM_OK;
+}
+
+}  // namespace
+
+int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, int32_t* cell_id, int64_t n_sd,
+                          int32_t n_cell, double dt, double dV, const sdm_kernel_params* kp, uint64_t seed,
+                          uint64_t step0, int64_t n_steps, int64_t compact_every, int64_t* n_sd_out) {
+    int rc = validate_step(ctx, multiplicity, volume, cell_id, n_sd, n_cell, dt, dV, kp);
+    if (rc != SDM_OK) return rc;
+    if (!n_sd_out || n_steps < 0 || compact_every < 0) return SDM_ERR_INVALID_ARG;
+    if (n_sd > 0 && (!aligned16(multiplicity) || !aligned16(volume))) return SDM_ERR_INVALID_ARG;
+    if (ctx->cuda_error) return SDM_ERR_CUDA;
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
+    *n_sd_out = n_sd;
+    ctx->zero_hint_valid = 0;
+    int64_t n = n_sd;
+    int64_t s = 0;
+    bool general_only = (n_cell <= 1) || ctx->path == SDM_PATH_GENERAL;
+    while (s < n_steps && n > 0) {
+        const StepArgs A = make_step_args(multiplicity, volume, cell_id, n, n_cell, dt, dV, kp, seed);
+        const Plan plan = make_plan(n, n_cell, ctx->skip_key_digits);
+        if (!plan_fits(plan)) return SDM_ERR_CAPACITY;
+        FusedSource src;
+        int rmax = CELL_FAST_MAX / 32;
+        bool fused = false;
+        if (!general_only) {
+            if (ctx->path == SDM_PATH_AUTO) {
+                if ((rc = auto_prepare(ctx, A, plan, &fused, &src, &rmax))) return rc;
+            } else {  // explicit CELL_SORTED / HYBRID: an input that does not fit is the caller's error
+                const bool hybrid = ctx->path == SDM_PATH_HYBRID;
+                if (hybrid && !hybrid_fits(plan)) {
+                    general_only = true;
+                    continue;
+                }
+                if ((rc = hybrid ? enqueue_hybrid_prepare(ctx, A, plan, rmax, true, &src)
+                                 : enqueue_sorted_prepare(ctx, A, rmax, true, &src)))
+                    return rc;
+                u32 cls = 3;
+                if ((rc = wait_verdict(ctx, ctx->epoch, &cls))) return rc;
+                if (cls > 2) {
+                    *n_sd_out = n;
+                    rc = finish_run(ctx);
+                    return rc != SDM_OK ? rc : SDM_ERR_BAD_DATA;
+                }
+                rmax = rmax_of_class(cls);
+                fused = true;
+            }
+        }
+        int64_t zeros = 0;
+        if (fused) {
+            if ((rc = run_fused_steps(ctx, A, src, rmax, step0, &s, n_steps, compact_every, &zeros))) return rc;
+            if (zeros > 0) {
+                if ((rc = enqueue_compact(ctx, multiplicity, volume, cell_id, n))) return rc;
+                n -= zeros;
+            }
+        } else {
+            // GENERAL steps; under AUTO the first one also tells whether the fused kernel could take this array
+            // (cells of at most 256 super-droplets), and the loop comes back to try
+            bool retry_fused = false;
+            while (s < n_steps && !retry_fused) {
+                if ((rc = enqueue_general_step(ctx, A, step0 + (uint64_t)s))) return rc;
+                ++s;
+                if (!general_only) {
+                    Verdict hint;
+                    if (auto_hint(ctx, A, &hint) && hint.max_count <= (u32)CELL_FAST_MAX && hint.unsorted &&
+                        hybrid_fits(plan))
+                        retry_fused = true;
+                    else
+                        general_only = true;
+                }
+                if (compact_every > 0 && (s % compact_every) == 0) {
+                    int64_t n_new = n;
+                    if ((rc = sdm_remove_zero_multiplicity(ctx, multiplicity, volume, cell_id, n, &n_new))) return rc;
+                    if (n_new != n) {
+                        n = n_new;
+                        break;  // the arrays shrank: new plan
+                    }
+                }
+            }
+        }
+    }
+    *n_sd_out = n;
+    return finish_run(ctx);
 }
 
 int sdm_cell_stats(sdm_ctx* ctx, const int64_t* multiplicity, const double* volume, const int32_t* cell_id,
@@ -537,6 +833,8 @@ int sdm_coalescence_step_host(sdm_ctx* ctx, int64_t* multiplicity_host, double* 
     if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_xi, multiplicity_host, (size_t)n_sd * 8, cudaMemcpyHostToDevice, st)))) return rc;
     if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_v, volume_host, (size_t)n_sd * 8, cudaMemcpyHostToDevice, st)))) return rc;
     if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_c, cell_id_host, (size_t)n_sd * 4, cudaMemcpyHostToDevice, st)))) return rc;
+    // the staging area is refilled by every call: what AUTO learned about the previous contents does not carry over
+    ctx->verdict_valid = 0;
     rc = sdm_coalescence_step(ctx, d_xi, d_v, d_c, n_sd, n_cell, dt, dV, kp, seed, step);
     if (rc != SDM_OK) return rc;
     int64_t n_out = n_sd;
@@ -549,7 +847,8 @@ int sdm_coalescence_step_host(sdm_ctx* ctx, int64_t* multiplicity_host, double* 
     }
     if ((rc = note_cuda(ctx, cudaMemcpyAsync(multiplicity_host, d_xi, (size_t)n_out * 8, cudaMemcpyDeviceToHost, st)))) return rc;
     if ((rc = note_cuda(ctx, cudaMemcpyAsync(volume_host, d_v, (size_t)n_out * 8, cudaMemcpyDeviceToHost, st)))) return rc;
-    return note_cuda(ctx, cudaStreamSynchronize(st));
+    // this call synchronises anyway: report a data error of its own step now, not at some later poll
+    return finish_run(ctx);
 }
 
 int sdm_philox_fill(sdm_ctx* ctx, uint64_t seed, uint64_t step, uint64_t i0, int64_t n, uint32_t* key_out,

@@ -8,9 +8,11 @@
 // (cell_id << 32 | key) and the oracle's std::stable_sort produce, so the output is bit-identical,
 // at 36-48 B/SD of HBM traffic instead of 148.
 //
-//   k_cell_bounds<SRC>  reads the cell of every position once: verifies range, order and the cell-size
-//                       limit, writes cell_start[0..n_cell].  Any violation sets CTL_SKIP: the fused
-//                       kernel then does nothing (the state is never half-updated).
+//   k_cell_bounds<SRC>  reads the cell of every position once: verifies range and order, finds the largest
+//                       cell's size class, writes cell_start[0..n_cell] and publishes the verdict (device flag
+//                       for the fused kernel, mapped host word for AUTO's path choice).  When the input does
+//                       not fit the fused kernel launched next, that kernel does nothing (the state is never
+//                       half-updated).
 //   k_cell_fused<W>     one warp per cell, n_c <= 32 R, R in {1,2,4,8}.  Sort word = 32 bits:
 //                       (top 24 bits of the Philox key) << 8 | position-in-run, sorted by an
 //                       all-ascending bitonic network (IMNMX + SHFL, 2 instructions per compare).
@@ -22,17 +24,25 @@
 
 namespace sdm {
 
-constexpr int CF_WARPS = 4;
+#ifndef SDM_CF_WARPS
+#define SDM_CF_WARPS 4
+#endif
+#ifndef SDM_CF_MIN_BLOCKS
+#define SDM_CF_MIN_BLOCKS 9
+#endif
+constexpr int CF_WARPS = SDM_CF_WARPS;  // tuning constants (profiles/): -DSDM_CF_WARPS / -DSDM_CF_MIN_BLOCKS via SDM_NVCC_EXTRA
 constexpr int CF_BLOCK = CF_WARPS * 32;
-constexpr int CF_MIN_BLOCKS = 8;  // measured on B200: 8, 10 and 12 resident blocks give 81, 84, 87 us on cfg3
+constexpr int CF_MIN_BLOCKS = SDM_CF_MIN_BLOCKS;
 constexpr int CB_BLOCK = 256;
-constexpr int CB_ITEMS = 8;
+constexpr int CB_K = 4;                         // quads (4 positions, one 16-byte load for int32 sources) per thread and iteration
+constexpr int CB_CHUNK = CB_BLOCK * CB_K * 4;   // positions per block and iteration
 
 // ---------------------------------------------------------------------------------------------
 // Cell boundaries of an array whose cells are contiguous.  SRC = 0: cell_id int32[n];
 // SRC = 1: sorted words u64 (cell << idxbits | index);  SRC = 2: the same in u32 words.
-// Eight positions per thread, read with 16-byte loads (VEC; the scalar instantiation serves a
-// misaligned cell_id); the cell-size check re-reads position i - max_cell the same way (L2 hits).
+// A streaming kernel: a resident grid strides over chunks of 4096 positions; every thread has four
+// independent, warp-coalesced 16-byte loads in flight per iteration (VEC; the scalar instantiation serves
+// a misaligned cell_id) and in the common case -- no cell boundary among its positions -- writes nothing.
 // ---------------------------------------------------------------------------------------------
 template <int SRC>
 __device__ __forceinline__ int cell_at(const void* src, u32 i, int idxbits) {
@@ -42,101 +52,143 @@ __device__ __forceinline__ int cell_at(const void* src, u32 i, int idxbits) {
 }
 
 template <int SRC, bool VEC>
-__device__ __forceinline__ void cells_at8(const void* src, u32 i0, u32 n_sd, int idxbits, int (&c)[CB_ITEMS]) {
-    if (VEC && i0 + CB_ITEMS <= n_sd) {  // i0 is a multiple of 8 and the base is 16-byte aligned
+__device__ __forceinline__ void cells_at4(const void* src, u32 i0, u32 n_sd, int idxbits, int (&c)[4]) {
+    if (VEC && i0 + 4 <= n_sd) {  // i0 is a multiple of 4 and the base is 16-byte aligned
         if (SRC == 1) {
             const ulonglong2* p = reinterpret_cast<const ulonglong2*>(reinterpret_cast<const u64*>(src) + i0);
-#pragma unroll
-            for (int q = 0; q < CB_ITEMS / 2; ++q) {
-                const ulonglong2 w = __ldg(p + q);
-                c[2 * q] = (int)(w.x >> idxbits);
-                c[2 * q + 1] = (int)(w.y >> idxbits);
-            }
+            const ulonglong2 w0 = __ldg(p), w1 = __ldg(p + 1);
+            c[0] = (int)(w0.x >> idxbits); c[1] = (int)(w0.y >> idxbits);
+            c[2] = (int)(w1.x >> idxbits); c[3] = (int)(w1.y >> idxbits);
         } else {
-            const uint4* p = reinterpret_cast<const uint4*>(reinterpret_cast<const u32*>(src) + i0);
-#pragma unroll
-            for (int q = 0; q < CB_ITEMS / 4; ++q) {
-                const uint4 w = __ldg(p + q);
-                c[4 * q] = (int)(w.x >> idxbits);      // SRC = 0: idxbits = 0, the word is the cell_id itself
-                c[4 * q + 1] = (int)(w.y >> idxbits);
-                c[4 * q + 2] = (int)(w.z >> idxbits);
-                c[4 * q + 3] = (int)(w.w >> idxbits);
-            }
+            const uint4 w = __ldg(reinterpret_cast<const uint4*>(reinterpret_cast<const u32*>(src) + i0));
+            c[0] = (int)(w.x >> idxbits);  // SRC = 0: idxbits = 0, the word is the cell_id itself
+            c[1] = (int)(w.y >> idxbits);
+            c[2] = (int)(w.z >> idxbits);
+            c[3] = (int)(w.w >> idxbits);
         }
     } else {
 #pragma unroll
-        for (int k = 0; k < CB_ITEMS; ++k) c[k] = (i0 + k < n_sd) ? cell_at<SRC>(src, i0 + k, idxbits) : 0x7fffffff;
+        for (int k = 0; k < 4; ++k) c[k] = (i0 + k < n_sd) ? cell_at<SRC>(src, i0 + k, idxbits) : 0x7fffffff;
     }
 }
 
 // Position i opens cell cc and closes cell prev (opening every empty cell in between).  The closed cell
-// [s, i) is larger than max_cell exactly when position i - 1 - max_cell still belongs to it (sorted input),
-// so the cell-size limit costs one extra load per cell, not per super-droplet.  Returns "too large".
+// [s, i) holds more than m entries exactly when position i - 1 - m still belongs to it (sorted input), so its
+// size class costs up to three extra loads per cell, not per super-droplet.  Returns the size class of the
+// closed cell: 0 (<= 64), 1 (<= 128), 2 (<= 256), 3 (larger).
 template <int SRC>
-__device__ __forceinline__ bool open_cells(const void* src, int idxbits, int prev, int cc, u32 i, u32 max_cell,
-                                           u32* __restrict__ cell_start, int32_t* __restrict__ dbg_cell_start) {
+__device__ __forceinline__ u32 open_cells(const void* src, int idxbits, int prev, int cc, u32 i,
+                                          u32* __restrict__ cell_start, int32_t* __restrict__ dbg_cell_start) {
     for (int q = prev + 1; q <= cc; ++q) {
         cell_start[q] = i;
         if (dbg_cell_start) dbg_cell_start[q] = (int32_t)i;
     }
-    return prev >= 0 && i > max_cell && cell_at<SRC>(src, i - 1u - max_cell, idxbits) == prev;
+    if (prev < 0) return 0;
+    u32 cls = 0;
+    if (i > 64u && cell_at<SRC>(src, i - 65u, idxbits) == prev) {
+        cls = 1;
+        if (i > 128u && cell_at<SRC>(src, i - 129u, idxbits) == prev) {
+            cls = 2;
+            if (i > 256u && cell_at<SRC>(src, i - 257u, idxbits) == prev) cls = 3;
+        }
+    }
+    return cls;
 }
 
 template <int SRC, bool VEC>
 __global__ void __launch_bounds__(CB_BLOCK)
-k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32 max_cell, u32 epoch,
-              u32* __restrict__ cell_start, u32* __restrict__ ctl, u32* __restrict__ sticky,
-              int32_t* __restrict__ dbg_cell_start) {
+k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32 max_class, u32 strict, u32 epoch,
+              u32* __restrict__ cell_start, u32* __restrict__ ctl, u32* __restrict__ sticky, u32* __restrict__ run,
+              volatile u32* __restrict__ mapped, int32_t* __restrict__ dbg_cell_start) {
+    __shared__ u32 s_cls;
     // the fused kernel that follows accumulates the zero count; no separate memset of the control block
     if (blockIdx.x == 0 && threadIdx.x == 0) ctl[CTL_ZERO_COUNT] = 0u;
-    const u32 i0 = (blockIdx.x * CB_BLOCK + threadIdx.x) * CB_ITEMS;  // lanes past the end stay for the shuffle
-    int c[CB_ITEMS];
-    cells_at8<SRC, VEC>(src, i0, n_sd, idxbits, c);
-    int prev = __shfl_up_sync(0xffffffffu, c[CB_ITEMS - 1], 1);
-    if ((threadIdx.x & 31) == 0) prev = (i0 == 0 || i0 > n_sd) ? -1 : cell_at<SRC>(src, i0 - 1, idxbits);
+    if (threadIdx.x == 0) s_cls = 0u;
+    const int lane = threadIdx.x & 31;
     bool bad = false;
-    if (i0 + CB_ITEMS < n_sd) {
-        // interior thread, straight-line: every value in range (then the differences cannot overflow);
-        // the OR of the differences to the predecessor is negative when the order is broken, zero when the
-        // thread holds no cell boundary (the common case), positive otherwise
-        bad = (u32)prev + 1u > (u32)n_cell;  // prev is -1 (array start) or a cell_id that must be in range too
-        int ored = 0;
-        int p = prev;
+    u32 cls = 0;
+    const u32 n_chunks = (n_sd + CB_CHUNK - 1) / CB_CHUNK;
+    for (u32 ch = blockIdx.x; ch < n_chunks; ch += gridDim.x) {
+        const u32 base = ch * (u32)CB_CHUNK;
+        int c[CB_K][4];
+        int before[CB_K];  // lane 0: the cell of the position before the warp's 128 positions of round k
 #pragma unroll
-        for (int k = 0; k < CB_ITEMS; ++k) {
-            bad |= (u32)c[k] >= (u32)n_cell;
-            ored |= c[k] - p;
-            p = c[k];
+        for (int k = 0; k < CB_K; ++k) {
+            const u32 i0 = base + ((u32)k * CB_BLOCK + threadIdx.x) * 4u;
+            cells_at4<SRC, VEC>(src, i0, n_sd, idxbits, c[k]);
+            before[k] = (lane == 0 && i0 > 0 && i0 <= n_sd) ? cell_at<SRC>(src, i0 - 1, idxbits) : -1;
         }
-        bad |= ored < 0;
-        if (!bad && ored != 0) {
-            p = prev;
 #pragma unroll
-            for (int k = 0; k < CB_ITEMS; ++k) {
-                if (c[k] != p) bad |= open_cells<SRC>(src, idxbits, p, c[k], i0 + k, max_cell, cell_start, dbg_cell_start);
-                p = c[k];
-            }
-        }
-    } else {
+        for (int k = 0; k < CB_K; ++k) {
+            const u32 i0 = base + ((u32)k * CB_BLOCK + threadIdx.x) * 4u;  // lanes past the end stay for the shuffle
+            int prev = __shfl_up_sync(0xffffffffu, c[k][3], 1);
+            if (lane == 0) prev = before[k];
+            if (i0 + 4 < n_sd) {
+                // interior quad, straight-line: every value in range (then the differences cannot overflow); the
+                // OR of the differences to the predecessor is negative when the order is broken, zero when the
+                // quad holds no cell boundary (the common case), positive otherwise
+                bool b = (u32)prev + 1u > (u32)n_cell;  // prev is -1 (array start) or a cell_id that must be in range too
+                int ored = 0;
+                int p = prev;
 #pragma unroll
-        for (int k = 0; k < CB_ITEMS; ++k) {
-            const u32 i = i0 + k;
-            if (i < n_sd) {
-                const int cc = c[k];
-                if (cc < 0 || cc >= n_cell || cc < prev) {
-                    bad = true;
-                } else {
-                    if (cc != prev) bad |= open_cells<SRC>(src, idxbits, prev, cc, i, max_cell, cell_start, dbg_cell_start);
-                    if (i == n_sd - 1)  // the array end closes cell cc and opens the (empty) rest
-                        bad |= open_cells<SRC>(src, idxbits, cc, n_cell, n_sd, max_cell, cell_start, dbg_cell_start);
+                for (int j = 0; j < 4; ++j) {
+                    b |= (u32)c[k][j] >= (u32)n_cell;
+                    ored |= c[k][j] - p;
+                    p = c[k][j];
                 }
-                prev = cc;
+                b |= ored < 0;
+                if (!b && ored != 0) {
+                    p = prev;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        if (c[k][j] != p)
+                            cls = max(cls, open_cells<SRC>(src, idxbits, p, c[k][j], i0 + j, cell_start, dbg_cell_start));
+                        p = c[k][j];
+                    }
+                }
+                bad |= b;
+            } else {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const u32 i = i0 + j;
+                    if (i < n_sd) {
+                        const int cc = c[k][j];
+                        if (cc < 0 || cc >= n_cell || cc < prev) {
+                            bad = true;
+                        } else {
+                            if (cc != prev)
+                                cls = max(cls, open_cells<SRC>(src, idxbits, prev, cc, i, cell_start, dbg_cell_start));
+                            if (i == n_sd - 1)  // the array end closes cell cc and opens the (empty) rest
+                                cls = max(cls, open_cells<SRC>(src, idxbits, cc, n_cell, n_sd, cell_start, dbg_cell_start));
+                        }
+                        prev = cc;
+                    }
+                }
             }
         }
     }
-    if (bad) {  // out of range, out of order or too large: the step is skipped and reported
-        sticky[STICKY_BAD_DATA] = 1u;
-        ctl[CTL_UNSORTED] = epoch;  // tagged with this step's epoch: stale refusals never match
+    if (bad) cls = 3;  // out of range or out of order: refused like a cell that is too large
+    cls = __reduce_max_sync(0xffffffffu, cls);
+    __syncthreads();
+    if (lane == 0 && cls) atomicMax(&s_cls, cls);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (s_cls) atomicMax(&run[RUN_BOUNDS_CLASS], s_cls);
+        __threadfence();
+        const u32 t = atomicAdd(&run[RUN_BOUNDS_TICKET], 1u);
+        if (t == gridDim.x - 1) {  // the last block: every other block's class is visible (fence + ticket)
+            __threadfence();
+            const u32 worst = atomicExch(&run[RUN_BOUNDS_CLASS], 0u);
+            run[RUN_BOUNDS_TICKET] = 0u;
+            const bool refuse = worst > max_class;
+            if (refuse) {  // the step is skipped as a whole and reported
+                ctl[CTL_UNSORTED] = epoch;  // tagged with this step's epoch: stale refusals never match
+                if (strict) sticky[STICKY_BAD_DATA] = 1u;
+            }
+            mapped[MAPPED_VERDICT_CLASS] = worst;
+            __threadfence_system();
+            mapped[MAPPED_VERDICT_EPOCH] = epoch;
+        }
     }
 }
 
@@ -211,6 +263,15 @@ struct FusedArgs {
     u32* sticky;
     u32* ctl;
     u32 epoch;  // ctl[CTL_UNSORTED] == epoch: k_cell_bounds refused this step's input
+    // zero bookkeeping (row a5 fused into a4) and the halt protocol of sdm_coalescence_steps (see sdm_api.cu):
+    u32* zc_accum;        // += zero multiplicities the array holds after this step
+    const u32* zc_check;  // non-null: the previous step's count, after which a compaction was due -- if it is not 0
+                          // the run halts here (nothing is updated) until the host has compacted
+    u32* zc_clear;        // non-null: the slot the NEXT step accumulates into (zeroed by block 0)
+    u32 halt_tag;         // != 0: a step of a multi-step run; written to run[RUN_HALT] and to the mapped status
+                          // block when this step halts
+    u32* run;             // RUN_* words
+    volatile u32* mapped; // pinned host status words (MAPPED_*), written with a system-scope fence
 };
 
 // Original array index of position e of the run that starts at `start`.
@@ -224,11 +285,11 @@ __device__ __forceinline__ u32 run_index(const FusedArgs& a, u32 start, u32 e) {
 // Per-warp staging of one cell in shared memory, indexed by the position e in the run: the attributes
 // are loaded ONCE, coalesced, before the (ALU-bound) key generation and sort, so the HBM latency hides
 // under them; the pair phase then reads its two members by sorted position from shared memory.
+// Two 16-byte stores per super-droplet: the exact attributes, and the fp32 side values of the cheap early-out.
 template <int WORD, int RMAX>
 struct CellStage {
     longlong2 xv[32 * RMAX];  // (multiplicity, volume bits)
-    uint2 uw[32 * RMAX];      // Philox words 2, 3 of the SD (its uniform, used if it lands on an even slot)
-    u32 key[32 * RMAX];       // full Philox permutation key (wide redo only)
+    float4 aux[32 * RMAX];    // {xi rounded UP to fp32, v rounded UP to fp32, Philox word 3 (bits), Philox key (bits)}
     u32 idx[WORD == 0 ? 1 : 32 * RMAX];  // HYBRID: original index
 };
 
@@ -241,11 +302,14 @@ __device__ __forceinline__ u32 select_reg(const u32 (&x)[R], int i) {
     return v;
 }
 
-// One warp, one cell of 2 <= n_c <= 32 R super-droplets (n_c = 1 only counts its zero).  Returns this
-// lane's share of the number of zero multiplicities the cell holds AFTER the step.
-template <int WORD, int RMAX, int R>
-__device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMAX>& st, u32 start, u32 n_c, int lane) {
+// One warp, one cell of 2 <= n_c <= 32 R super-droplets.  Returns this lane's share of the number of zero
+// multiplicities the cell holds AFTER the step.  The hot flow is straight-line code: loads, Philox blocks (computed
+// for padding slots too, so the R chains interleave), sort and the first-level pair test are predicated, not branched.
+// FULL: n_c == 32 R (every slot holds a super-droplet: no padding, no guards); the caller branches warp-uniformly.
+template <int WORD, int RMAX, int R, int KIND, bool FULL>
+__device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMAX>& st, u32 start, u32 n_c_in, int lane) {
     static_assert(R <= RMAX, "register tile within the staging tile");
+    const u32 n_c = FULL ? 32u * R : n_c_in;
     const PairArgs& pa = a.pair;
     u32 zeros = 0;
     // ---- a1 + load: striped positions e = 32 r + lane (coalesced), everything parked in shared memory ----
@@ -263,48 +327,51 @@ __device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMA
         }
     }
     // keys first: Philox needs only the index, so the attribute loads above stay in flight under it
-    u32 x[R];
+    u32 x[R], w3[R], key[R];
     const int drop = 32 - a.key_bits;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const u32 e = 32u * r + lane;
-        x[r] = 0xFFFFFFFFu;  // padding sorts to the end
-        if (e < n_c && n_c >= 2) {
-            const PhiloxOut w = philox4x32_10(pa.pk, (u64)idx[r]);
-            st.uw[e] = make_uint2(w.w2, w.w3);
-            st.key[e] = w.w0;
-            if (WORD != 0) st.idx[e] = idx[r];
-            x[r] = ((w.w0 >> drop) << 8) | e;
-        }
+        const PhiloxOut w = philox4x32_10(pa.pk, (u64)idx[r]);
+        w3[r] = w.w3; key[r] = w.w0;
+        // padding sorts to the end (a real word with the same upper bits has a smaller position) and keeps a
+        // position inside the staging tile, so that the unguarded reads of the pair test stay in bounds
+        x[r] = (e < n_c) ? (((w.w0 >> drop) << 8) | e) : (0xFFFFFF00u | e);
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const u32 e = 32u * r + lane;
+        const float xf = __ll2float_ru(xi[r]);  // 0 -> 0.0f, xi >= 1 -> >= 1.0f (padding slots hold xi = 1)
+        zeros += (xf == 0.0f);
         if (e < n_c) {
-            zeros += (xi[r] == 0);
             st.xv[e] = make_longlong2(xi[r], __double_as_longlong(vol[r]));
+            st.aux[e] = make_float4(xf, __double2float_ru(vol[r]), __uint_as_float(w3[r]), __uint_as_float(key[r]));
+            if (WORD != 0) st.idx[e] = idx[r];
         }
-    }
-    if (n_c < 2) {
-        if (a.dbg_perm && lane == 0) a.dbg_perm[start] = (int32_t)idx[0];
-        return zeros;
     }
     // ---- a3: sort (truncated key, position) words; slot s = lane R + r afterwards ----
     warp_bitonic_sort<u32, R>(x, lane);
     // neighbours with equal truncated keys: their order is decided by the dropped bits -> wide redo
-    bool tie = false;
-#pragma unroll
-    for (int r = 0; r + 1 < R; ++r) tie |= (((x[r] ^ x[r + 1]) >> 8) == 0) && ((u32)(lane * R + r + 1) < n_c);
+    u32 ties = 0xFFFFFFFFu;  // smallest XOR of two neighbouring words that are both real
     const u32 nxt = __shfl_down_sync(0xffffffffu, x[0], 1);
-    tie |= (lane < 31) && (((x[R - 1] ^ nxt) >> 8) == 0) && ((u32)(lane * R + R) < n_c);
+    if (FULL) {  // a full tile has no padding
+#pragma unroll
+        for (int r = 0; r + 1 < R; ++r) ties = min(ties, x[r] ^ x[r + 1]);
+        if (lane < 31) ties = min(ties, x[R - 1] ^ nxt);
+    } else {
+#pragma unroll
+        for (int r = 0; r + 1 < R; ++r)
+            if ((u32)(lane * R + r + 1) < n_c) ties = min(ties, x[r] ^ x[r + 1]);
+        if (lane < 31 && (u32)(lane * R + R) < n_c) ties = min(ties, x[R - 1] ^ nxt);
+    }
     __syncwarp();  // the staging writes of all lanes are visible from here on
     u32 pos[R];
-    if (__any_sync(0xffffffffu, tie)) {
+    if (__any_sync(0xffffffffu, ties < 0x100u)) {
         u64 wide[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {  // the real words occupy the first n_c slots of the narrow result
             const u32 e = x[r] & 0xFFu;
-            wide[r] = ((u32)(lane * R + r) < n_c) ? (((u64)st.key[e] << 32) | (u64)e) : ~0ull;
+            wide[r] = ((u32)(lane * R + r) < n_c) ? (((u64)__float_as_uint(st.aux[e].w) << 32) | (u64)e) : ~0ull;
         }
         warp_bitonic_sort<u64, R>(wide, lane);
 #pragma unroll
@@ -320,10 +387,12 @@ __device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMA
             if (s < n_c) a.dbg_perm[start + s] = (int32_t)(WORD == 0 ? start + pos[r] : st.idx[pos[r]]);
         }
     }
-    // ---- a4, phase A: every pair of neighbouring slots -- can its gamma be non-zero? ----
+    // ---- a4, level 1: every pair of neighbouring slots -- a dozen fp32 operations decide "gamma = 0 for sure" ----
     constexpr int NP = (R >= 2) ? R / 2 : 1;
     u32 first[NP], second[NP];  // run positions of the pair's members, in shuffled order
-    u32 need = 0;               // bit q: pair q of this lane must run the full rule
+    u32 need = 0;               // bit q: pair q of this lane goes on to the exact levels
+    const float cscale = pa.cheap_c * (float)pair_scale_int(n_c);
+    const bool dbg = pa.dbg_gamma != nullptr;
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
         bool valid;
@@ -336,41 +405,61 @@ __device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMA
             second[q] = __shfl_down_sync(0xffffffffu, pos[0], 1);
             valid = ((lane & 1) == 0) && ((u32)lane + 1u < n_c);
         }
-        if (valid) {
-            if (pa.dbg_gamma) {
-                need |= 1u << q;
-            } else {
-                const longlong2 A = st.xv[first[q]], B = st.xv[second[q]];
-                if (A.x != 0 && B.x != 0) {  // a dead partner: gamma~ = 0 whatever gamma is (R7)
-                    const bool swap = A.x < B.x;
-                    const uint2 w = st.uw[first[q]];
-                    const double vA = __longlong_as_double(A.y), vB = __longlong_as_double(B.y);
-                    if (pair_may_collide(pa, swap ? B.x : A.x, swap ? vB : vA, swap ? vA : vB, w.x, w.y, n_c))
-                        need |= 1u << q;
-                }
-            }
-        }
+        // (slots past n_c hold padding positions: the staged values read there are unspecified, `valid` drops them)
+        const float4 A = st.aux[first[q]], B = st.aux[second[q]];
+        // a dead partner (xi = 0 rounds up to 0.0f, xi >= 1 to >= 1.0f): gamma~ = 0 whatever gamma is (R7)
+        const bool alive = fminf(A.x, B.x) != 0.0f;
+        const bool may = pair_cheap_may_collide<KIND>(cscale, fmaxf(A.x, B.x), A.y, B.y, __float_as_uint(A.z));
+        if (valid && (dbg || (alive && may))) need |= 1u << q;
     }
-    // ---- phase B: the full fp64 rule, only where needed; lanes take their pending pairs one at a time ----
+    // ---- levels 2 and 3: the fp32 interval bound and the full fp64 rule, only where needed; lanes take
+    //      their pending pairs one at a time ----
     while (__any_sync(0xffffffffu, need != 0)) {
         if (need) {
             const int q = __ffs(need) - 1;
             need &= need - 1u;
             const u32 ea = select_reg<NP>(first, q), eb = select_reg<NP>(second, q);
             const longlong2 A = st.xv[ea], B = st.xv[eb];
-            const uint2 w = st.uw[ea];
-            const u32 ja = (WORD == 0) ? start + ea : st.idx[ea];
-            const u32 jb = (WORD == 0) ? start + eb : st.idx[eb];
-            zeros += pair_apply(pa, ja, jb, A.x, __longlong_as_double(A.y), B.x, __longlong_as_double(B.y), w.x, w.y, n_c);
+            const double vA = __longlong_as_double(A.y), vB = __longlong_as_double(B.y);
+            const bool swap = A.x < B.x;
+            const u32 w3a = __float_as_uint(st.aux[ea].z);
+            // w2 = 0 makes u a lower bound of the true uniform: the test stays conservative
+            if (dbg || pair_may_collide(pa, swap ? B.x : A.x, swap ? vB : vA, swap ? vA : vB, 0u, w3a, n_c)) {
+                const u32 ja = (WORD == 0) ? start + ea : st.idx[ea];
+                const u32 jb = (WORD == 0) ? start + eb : st.idx[eb];
+                const PhiloxOut w = philox4x32_10(pa.pk, (u64)ja);  // the exact uniform of the first member (R2)
+                zeros += pair_apply(pa, ja, jb, A.x, vA, B.x, vB, w.w2, w.w3, n_c);
+            }
         }
     }
     return zeros;
 }
 
-template <int WORD, int RMAX>
+template <int WORD, int RMAX, int R, int KIND>
+__device__ __forceinline__ u32 warp_cell_any(const FusedArgs& a, CellStage<WORD, RMAX>& st, u32 start, u32 n_c, int lane) {
+    // regular grids fill their tiles exactly (configs[2], [3]: 32 and 128 per cell): that case runs without guards
+    if (n_c == 32u * R) return warp_cell<WORD, RMAX, R, KIND, true>(a, st, start, n_c, lane);
+    return warp_cell<WORD, RMAX, R, KIND, false>(a, st, start, n_c, lane);
+}
+
+template <int WORD, int RMAX, int KIND>
 __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const FusedArgs a) {
     __shared__ CellStage<WORD, RMAX> s_stage[CF_WARPS];
     if (a.ctl[CTL_UNSORTED] == a.epoch) return;  // k_cell_bounds refused the input: the step is skipped as a whole
+    if (a.halt_tag) {  // a step of sdm_coalescence_steps: a halted run stays halted until the host has compacted
+        const u32 halted = a.run[RUN_HALT];
+        const u32 due_zeros = a.zc_check ? *a.zc_check : 0u;
+        if (halted | due_zeros) {
+            if (!halted && blockIdx.x == 0 && threadIdx.x == 0) {
+                a.run[RUN_HALT] = a.halt_tag;
+                a.mapped[MAPPED_ZEROS] = due_zeros;
+                __threadfence_system();
+                a.mapped[MAPPED_HALT] = a.halt_tag;
+            }
+            return;
+        }
+    }
+    if (a.zc_clear && blockIdx.x == 0 && threadIdx.x == 0) *a.zc_clear = 0u;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     CellStage<WORD, RMAX>& st = s_stage[warp];
     // one warp per cell, one launch wave after another: the block scheduler balances the (data-dependent)
@@ -380,37 +469,44 @@ __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const Fu
     if (c < a.n_cell) {
         const u32 start = __ldg(a.pair.cell_start + c);
         const u32 n_c = __ldg(a.pair.cell_start + c + 1) - start;
-        if (n_c == 0) {
+        if (n_c < 2) {  // nothing to pair; a lone super-droplet still counts as a zero when its multiplicity is 0
+            if (n_c == 1 && lane == 0) {
+                const u32 i = run_index<WORD>(a, start, 0);
+                zeros = (a.pair.xi[i] == 0);
+                if (a.dbg_perm) a.dbg_perm[start] = (int32_t)i;
+            }
         } else if (n_c <= 32) {
-            zeros = warp_cell<WORD, RMAX, 1>(a, st, start, n_c, lane);
+            zeros = warp_cell_any<WORD, RMAX, 1, KIND>(a, st, start, n_c, lane);
         } else if (RMAX >= 2 && n_c <= 64) {
-            if constexpr (RMAX >= 2) zeros = warp_cell<WORD, RMAX, 2>(a, st, start, n_c, lane);
+            if constexpr (RMAX >= 2) zeros = warp_cell_any<WORD, RMAX, 2, KIND>(a, st, start, n_c, lane);
         } else if (RMAX >= 4 && n_c <= 128) {
-            if constexpr (RMAX >= 4) zeros = warp_cell<WORD, RMAX, 4>(a, st, start, n_c, lane);
+            if constexpr (RMAX >= 4) zeros = warp_cell_any<WORD, RMAX, 4, KIND>(a, st, start, n_c, lane);
         } else if (RMAX >= 8 && n_c <= 256) {
-            if constexpr (RMAX >= 8) zeros = warp_cell<WORD, RMAX, 8>(a, st, start, n_c, lane);
+            if constexpr (RMAX >= 8) zeros = warp_cell_any<WORD, RMAX, 8, KIND>(a, st, start, n_c, lane);
         } else if (lane == 0) {
             a.sticky[STICKY_BAD_DATA] = 1u;  // unreachable: k_cell_bounds refuses such cells
         }
     }
     // a5, fused: the number of zero multiplicities after the step (sdm_remove_zero_multiplicity reads it)
     zeros = __reduce_add_sync(0xffffffffu, zeros);
-    if (lane == 0 && zeros) atomicAdd(a.ctl + CTL_ZERO_COUNT, zeros);
+    if (lane == 0 && zeros) atomicAdd(a.zc_accum, zeros);
 }
 
 // src_kind: 0 = cell_id array itself (CELL_SORTED), 1 = u64 sorted words, 2 = u32 sorted words (HYBRID).
-// max_cell = 32 * rmax: the largest cell the fused kernel launched next can hold.
+// rmax: register tile of the fused kernel launched next; it holds cells of up to 32 * rmax super-droplets.
 cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
-                               int idxbits, int rmax) {
-    const u32 grid = (u32)((n_sd + CB_BLOCK * CB_ITEMS - 1) / (CB_BLOCK * CB_ITEMS));
-    const u32 max_cell = 32u * (u32)rmax;
+                               int idxbits, int rmax, bool strict) {
+    const long long n_chunks = (n_sd + CB_CHUNK - 1) / CB_CHUNK;
+    const long long resident = (long long)ctx->sm_count * 6;
+    const u32 grid = (u32)(n_chunks < resident ? n_chunks : resident);
+    const u32 max_class = rmax <= 2 ? 0u : (rmax <= 4 ? 1u : 2u);
     LaunchScope scope(ctx, PROF_CELL_BOUNDS);
     Workspace& ws = ctx->ws;
     const bool vec = (reinterpret_cast<uintptr_t>(src) & 15u) == 0;
-#define SDM_BOUNDS(SRC, VEC, IDXBITS)                                                                       \
-    k_cell_bounds<SRC, VEC><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, IDXBITS, max_cell, \
-                                                                ctx->epoch, ws.cell_start, ws.ctl, ws.sticky,      \
-                                                                ctx->dbg_cell_start)
+#define SDM_BOUNDS(SRC, VEC, IDXBITS)                                                                               \
+    k_cell_bounds<SRC, VEC><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, IDXBITS, max_class,          \
+                                                                strict ? 1u : 0u, ctx->epoch, ws.cell_start, ws.ctl, \
+                                                                ws.sticky, ws.run, ctx->mapped, ctx->dbg_cell_start)
     if (src_kind == 0) {
         if (vec) SDM_BOUNDS(0, true, 0);
         else SDM_BOUNDS(0, false, 0);
@@ -425,29 +521,44 @@ cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int6
     return cudaGetLastError();
 }
 
+// The staging tiles want the shared-memory end of the L1 split.  The attribute is per device and per function:
+// it is set once per context (contexts live on one device) for every instantiation, and the result is checked.
 template <int WORD, int RMAX>
-static void prefer_shared_carveout() {  // the staging tiles want the shared-memory end of the L1 split
-    static bool done = false;
-    if (!done) {
-        cudaFuncSetAttribute(k_cell_fused<WORD, RMAX>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                             cudaSharedmemCarveoutMaxShared);
-        done = true;
-    }
+static cudaError_t prefer_shared_carveout() {
+    cudaError_t e = cudaFuncSetAttribute(k_cell_fused<WORD, RMAX, 0>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                         cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_cell_fused<WORD, RMAX, 1>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                cudaSharedmemCarveoutMaxShared);
+}
+
+cudaError_t init_cell_fused(sdm_ctx*) {
+    cudaError_t e;
+#define SDM_CARVE(W)                                                         \
+    if ((e = prefer_shared_carveout<W, 2>()) != cudaSuccess) return e;       \
+    if ((e = prefer_shared_carveout<W, 4>()) != cudaSuccess) return e;       \
+    if ((e = prefer_shared_carveout<W, 8>()) != cudaSuccess) return e;
+    SDM_CARVE(0) SDM_CARVE(1) SDM_CARVE(2)
+#undef SDM_CARVE
+    return cudaSuccess;
+}
+
+template <int WORD, int KIND>
+static void launch_fused_kind(const FusedArgs& a, int rmax, u32 grid, cudaStream_t st) {
+    if (rmax <= 2) k_cell_fused<WORD, 2, KIND><<<grid, CF_BLOCK, 0, st>>>(a);
+    else if (rmax <= 4) k_cell_fused<WORD, 4, KIND><<<grid, CF_BLOCK, 0, st>>>(a);
+    else k_cell_fused<WORD, 8, KIND><<<grid, CF_BLOCK, 0, st>>>(a);
 }
 
 template <int WORD>
 static void launch_fused_word(const FusedArgs& a, int rmax, u32 grid, cudaStream_t st) {
-    prefer_shared_carveout<WORD, 2>();
-    prefer_shared_carveout<WORD, 4>();
-    prefer_shared_carveout<WORD, 8>();
-    if (rmax <= 2) k_cell_fused<WORD, 2><<<grid, CF_BLOCK, 0, st>>>(a);
-    else if (rmax <= 4) k_cell_fused<WORD, 4><<<grid, CF_BLOCK, 0, st>>>(a);
-    else k_cell_fused<WORD, 8><<<grid, CF_BLOCK, 0, st>>>(a);
+    if (a.pair.kp.kind == 0) launch_fused_kind<WORD, 0>(a, rmax, grid, st);
+    else launch_fused_kind<WORD, 1>(a, rmax, grid, st);
 }
 
 cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int rmax, int64_t* xi,
                               double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
-                              const PhiloxKeys& pk) {
+                              const PhiloxKeys& pk, const StepLinks& links) {
     FusedArgs a;
     a.pair.sorted = nullptr;
     a.pair.xi = reinterpret_cast<long long*>(xi);
@@ -471,6 +582,12 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.sticky = ctx->ws.sticky;
     a.ctl = ctx->ws.ctl;
     a.epoch = ctx->epoch;
+    a.zc_accum = links.zc_accum ? links.zc_accum : ctx->ws.ctl + CTL_ZERO_COUNT;
+    a.zc_check = links.zc_check;
+    a.zc_clear = links.zc_clear;
+    a.halt_tag = links.halt_tag;
+    a.run = ctx->ws.run;
+    a.mapped = ctx->mapped;
     const u32 grid = (u32)((n_cell + CF_WARPS - 1) / CF_WARPS);
     LaunchScope scope(ctx, PROF_CELL_FUSED);
     if (src_kind == 0) launch_fused_word<0>(a, rmax, grid, ctx->stream);

@@ -20,6 +20,7 @@ struct PhiloxKeys {
     u32 k0[10];
     u32 k1[10];
     u32 step_lo, step_hi;
+    u32 p1_lo, p1_hi;  // 0xCD9E8D57 * step_lo: the first round's second product is the same for every super-droplet
     u64 index_base;  // counter of array entry i is index_base + i (SDM_OPT_INDEX_BASE; R34)
 };
 
@@ -34,6 +35,9 @@ __host__ __device__ inline PhiloxKeys make_philox_keys(u64 seed, u64 step, u64 i
     }
     pk.step_lo = (u32)step;
     pk.step_hi = (u32)(step >> 32);
+    const u64 p1 = (u64)0xCD9E8D57u * (u64)pk.step_lo;
+    pk.p1_lo = (u32)p1;
+    pk.p1_hi = (u32)(p1 >> 32);
     pk.index_base = index_base;
     return pk;
 }
@@ -44,9 +48,17 @@ struct PhiloxOut {
 
 __device__ __forceinline__ PhiloxOut philox4x32_10(const PhiloxKeys& pk, u64 i) {
     i += pk.index_base;
-    u32 c0 = (u32)i, c1 = (u32)(i >> 32), c2 = pk.step_lo, c3 = pk.step_hi;
+    u32 c0 = (u32)i, c1 = (u32)(i >> 32), c2, c3 = pk.step_hi;
+    {  // round 0: the counter words 2, 3 are the step, so 0xCD9E8D57 * c2 comes precomputed from the host
+        const u64 p0 = (u64)0xD2511F53u * (u64)c0;
+        const u32 n0 = pk.p1_hi ^ c1 ^ pk.k0[0];
+        c2 = (u32)(p0 >> 32) ^ c3 ^ pk.k1[0];
+        c1 = pk.p1_lo;
+        c3 = (u32)p0;
+        c0 = n0;
+    }
 #pragma unroll
-    for (int r = 0; r < 10; ++r) {
+    for (int r = 1; r < 10; ++r) {
         const u64 p0 = (u64)0xD2511F53u * (u64)c0;  // IMAD.WIDE.U32
         const u64 p1 = (u64)0xCD9E8D57u * (u64)c2;
         const u32 n0 = (u32)(p1 >> 32) ^ c1 ^ pk.k0[r];

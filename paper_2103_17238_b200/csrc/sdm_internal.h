@@ -41,6 +41,23 @@ enum CtlWord {
     CTL_ZERO_COUNT = 25,  // compaction: number of zero-multiplicity entries (low word)
     CTL_WORDS = 64
 };
+// Words of the run block (NOT zeroed per step; zeroed at init and managed by sdm_coalescence_steps).
+enum RunWord {
+    RUN_HALT = 0,  // != 0: the multi-step run is halted (a due compaction found zeros); fused steps exit at once
+    RUN_ZC0 = 1,   // RUN_ZC0 + (s mod 3): zero multiplicities the array holds after step s of the run
+    RUN_BOUNDS_TICKET = 4,  // k_cell_bounds: blocks finished (the last one publishes the verdict and resets it)
+    RUN_BOUNDS_CLASS = 5,   // k_cell_bounds: worst cell-size class seen so far (reset by the last block)
+    RUN_WORDS = 64
+};
+// Words of the pinned, device-mapped host status block: what the host must learn WITHOUT draining the stream.
+enum MappedWord {
+    MAPPED_HALT = 0,     // RUN_HALT's tag
+    MAPPED_ZEROS = 1,    // the zero count that caused the halt
+    MAPPED_VERDICT_EPOCH = 2,  // k_cell_bounds: epoch of the last published verdict
+    MAPPED_VERDICT_CLASS = 3,  //   its worst cell-size class: 0 (<= 64), 1 (<= 128), 2 (<= 256), 3 (larger, or the
+                               //   array is not non-decreasing / holds an out-of-range cell_id)
+    MAPPED_WORDS = 16
+};
 // Sticky words (zeroed at init and by sdm_poll_error only).
 enum StickyWord { STICKY_BAD_DATA = 0, STICKY_WORDS = 64 };
 
@@ -53,6 +70,7 @@ struct Workspace {
     size_t zero_bytes_fixed;  // ctl + digit_hist (contiguous from ctl)
     // [not zeroed] -----------------------------------------------------
     u32* sticky;      // STICKY_WORDS
+    u32* run;         // RUN_WORDS
     u32* cell_start;  // max_n_cell + 1
     u64* buf_a;       // max_n_sd
     u64* buf_b;       // max_n_sd
@@ -113,7 +131,9 @@ struct sdm_ctx {
     // AUTO path selection: verdict of the last general-path step about (cell_id pointer, n_sd, n_cell)
     sdm::Verdict* verdict_host;  // pinned
     sdm::u32* status_host;       // pinned: sticky words then control block, one D2H copy
+    volatile sdm::u32* mapped;   // pinned + mapped: MAPPED_* words written by kernels (same address on the device: UVA)
     cudaEvent_t verdict_event;
+    cudaEvent_t chunk_event[2];  // sdm_coalescence_steps: completion of the two chunks of steps in flight
     // zero-multiplicity count left in ctl[CTL_ZERO_COUNT] by the last fused step (SDM_OPT_TRACK_ZEROS)
     sdm::u32 epoch;  // tag of the current fused-path step (>= 2; see k_cell_bounds)
     sdm::u64 index_base;  // SDM_OPT_INDEX_BASE
@@ -168,11 +188,20 @@ cudaError_t launch_cell_sort_pass(sdm_ctx* ctx, int pass, bool narrow, const int
                                   void* out, int64_t n_sd, int32_t n_cell, const Plan& plan);
 cudaError_t launch_cell_digit_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
                                    const Plan& plan);
+// strict: a refusal (class above the one `rmax` holds) also raises the sticky SDM_ERR_BAD_DATA (explicit paths);
+// AUTO's analysis passes strict = false and falls back instead.
 cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
-                               int idxbits, int rmax);
+                               int idxbits, int rmax, bool strict);
+// Zero bookkeeping / halt protocol of one fused step (all nullable / 0: see FusedArgs in sdm_cellsort.cu).
+struct StepLinks {
+    u32* zc_accum;
+    const u32* zc_check;
+    u32* zc_clear;
+    u32 halt_tag;
+};
 cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int rmax, int64_t* xi,
                               double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
-                              const PhiloxKeys& pk);
+                              const PhiloxKeys& pk, const StepLinks& links);
 cudaError_t launch_tie_repair(sdm_ctx* ctx, u64* sorted, int64_t n_sd, const Plan& plan, const PhiloxKeys& pk);
 cudaError_t launch_debug_perm(sdm_ctx* ctx, const u64* sorted, int64_t n_sd, const Plan& plan);
 cudaError_t launch_count_zero(sdm_ctx* ctx, const int64_t* xi, int64_t n_sd);
@@ -180,6 +209,8 @@ cudaError_t launch_compact(sdm_ctx* ctx, int64_t* xi, double* v, int32_t* cell_i
 cudaError_t launch_cell_stats(sdm_ctx* ctx, const int64_t* xi, const double* v, const int32_t* cell_id,
                               int64_t n_sd, int32_t n_cell, int32_t* count, int64_t* sum_xi,
                               double* sum_xi_v, double* sum_xi_v2);
+cudaError_t init_cell_fused(sdm_ctx* ctx);       // per-device function attributes, once per context
+cudaError_t init_volume_spectrum(sdm_ctx* ctx);
 cudaError_t launch_volume_spectrum(sdm_ctx* ctx, const int64_t* xi, const double* v, int64_t n_sd,
                                    const double* edges_dev, int32_t n_edges, int64_t* count, int64_t* sum_xi,
                                    double* sum_xi_v);

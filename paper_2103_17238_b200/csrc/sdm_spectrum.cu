@@ -102,6 +102,11 @@ k_volume_spectrum(const long long* __restrict__ xi, const double* __restrict__ v
     }
 }
 
+// The opt-in to more than 48 KB of dynamic shared memory is per device: done once per context (sdm_init).
+cudaError_t init_volume_spectrum(sdm_ctx*) {
+    return cudaFuncSetAttribute(k_volume_spectrum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SPEC_SMEM_BUDGET);
+}
+
 static size_t spectrum_smem_bytes(int n_edges, int cols) {
     return (size_t)n_edges * 8 + (size_t)(n_edges - 1) * (size_t)cols * (8 + 4 + 4 + 4) + 16;
 }
@@ -109,11 +114,6 @@ static size_t spectrum_smem_bytes(int n_edges, int cols) {
 cudaError_t launch_volume_spectrum(sdm_ctx* ctx, const int64_t* xi, const double* v, int64_t n_sd,
                                    const double* edges_dev, int32_t n_edges, int64_t* count, int64_t* sum_xi,
                                    double* sum_xi_v) {
-    static bool opted_in = false;
-    if (!opted_in) {
-        cudaFuncSetAttribute(k_volume_spectrum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SPEC_SMEM_BUDGET);
-        opted_in = true;
-    }
     int cols = 32;  // column copies of the per-bin sums: as many as the shared-memory budget allows
     while (cols > 1 && spectrum_smem_bytes(n_edges, cols) > SPEC_SMEM_BUDGET) cols >>= 1;
     const size_t smem = spectrum_smem_bytes(n_edges, cols);

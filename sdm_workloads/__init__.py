@@ -199,3 +199,16 @@ def shard(w: Workload, rank: int, world: int) -> Shard:
     work = dataclasses.replace(w, xi=w.xi[lo:hi].copy(), v=w.v[lo:hi].copy(),
                                cell_id=(w.cell_id[lo:hi] - cell_lo).astype(np.int32), n_cell=cell_hi - cell_lo)
     return Shard(work, rank, world, cell_lo, cell_hi, lo)
+
+
+def rebase(n_sd_per_rank) -> list:
+    """index_base of every rank after a compaction: rank r's first entry is preceded by the survivors of the ranks
+    before it (exclusive scan of the per-rank counts -- what an 8-byte all_gather gives every rank).  Pure index
+    bookkeeping, R34."""
+    bases, acc = [], 0
+    for n in n_sd_per_rank:
+        if n < 0:
+            raise ValueError("negative count")
+        bases.append(acc)
+        acc += int(n)
+    return bases

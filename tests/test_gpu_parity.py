@@ -288,37 +288,34 @@ def test_cell_sorted_path_cell_sizes(dev, per_cell):
     _run_parity(w, dev, path=sdm.PATH_CELL_SORTED, bit_exact=True)
 
 
-def test_auto_path_switches_to_cell_sorted(dev):
+def test_auto_path_picks_the_path_that_fits(dev):
     sdm = _sdm()
     w = W.small("cfg3")
     with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
         xi, v, cell = _to_dev(w, dev)
         kp = _gkp(w)
         ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 0)
-        assert ctx.last_path() == sdm.PATH_GENERAL          # first sight of this cell_id array
-        torch.cuda.synchronize()
+        assert ctx.last_path() == sdm.PATH_CELL_SORTED      # analysed on the device: sorted, cells <= 256
         ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 1)
-        assert ctx.last_path() == sdm.PATH_CELL_SORTED      # verdict: sorted, cells <= 256
-        # an interleaved array with small cells: general once, then the hybrid path
+        assert ctx.last_path() == sdm.PATH_CELL_SORTED
+        # an interleaved array with small cells: general once (which sees the cell sizes), then the hybrid path
         wi = W.small("cfg3", interleave=True)
         xi2, v2, cell2 = _to_dev(wi, dev)
         for s in range(3):
             ctx.coalescence_step(xi2, v2, cell2, wi.n_cell, wi.dt, wi.dV, kp, 42, s)
-            torch.cuda.synchronize()
             assert ctx.last_path() == (sdm.PATH_GENERAL if s == 0 else sdm.PATH_HYBRID)
         # cells larger than the fast path's limit: general path
         big = W.cfg3(n_cell=8, per_cell=300, n_steps=3)
         xb, vb, cb = _to_dev(big, dev)
         for s in range(3):
             ctx.coalescence_step(xb, vb, cb, big.n_cell, big.dt, big.dV, kp, 42, s)
-            torch.cuda.synchronize()
             assert ctx.last_path() == sdm.PATH_GENERAL
         assert ctx.poll_error() == 0
 
 
-def test_cell_sorted_path_refuses_unsorted_input(dev):
-    """explicit CELL_SORTED on an unsorted array, and AUTO with a verdict that went stale because
-    cell_id was modified in place: the step is not applied and SDM_ERR_BAD_DATA is reported."""
+def test_explicit_cell_sorted_path_refuses_unsorted_input(dev):
+    """explicit CELL_SORTED on an unsorted array is the caller's error: the step is not applied and
+    SDM_ERR_BAD_DATA is reported."""
     sdm = _sdm()
     w = W.small("cfg3")
     kp = _gkp(w)
@@ -330,25 +327,60 @@ def test_cell_sorted_path_refuses_unsorted_input(dev):
         ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 0)
         assert ctx.poll_error() == -4
         assert torch.equal(xi, before[0]) and torch.equal(v, before[1])
-        # AUTO: learn "sorted", then break the array in place
-        ctx.set_path(sdm.PATH_AUTO)
-        xi, v, cell = _to_dev(w, dev)
-        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 0)
-        torch.cuda.synchronize()
-        cell[100], cell[5000] = cell[5000].item(), cell[100].item()
-        before = xi.clone(), v.clone()
-        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 1)
-        assert ctx.last_path() == sdm.PATH_CELL_SORTED
-        assert ctx.poll_error() == -4                                     # caught on the device
+        with pytest.raises(sdm.SDMError) as e:                            # the multi-step entry reports it at once
+            ctx.coalescence_steps(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 0, 3)
+        assert e.value.status == -4
         assert torch.equal(xi, before[0]) and torch.equal(v, before[1])
-        # the verdict was reset: the next step takes the general path and matches the oracle
+        assert ctx.poll_error() == 0
+
+
+def test_auto_falls_back_when_cell_id_is_rewritten_in_place(dev):
+    """AUTO never refuses valid input: cell_id rewritten in place between steps (what a displacement step does) makes
+    the next step take the path that fits -- oracle-identical output, status 0 (What's weak 8)."""
+    sdm = _sdm()
+    w = W.small("cfg3")
+    ow = w.copy()
+    okp, kp = _okp(w), _gkp(w)
+    rng = np.random.default_rng(5)
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        expect = [sdm.PATH_CELL_SORTED, sdm.PATH_GENERAL, sdm.PATH_HYBRID, sdm.PATH_HYBRID, sdm.PATH_HYBRID]
+        for s in range(5):
+            if s == 1:      # a few super-droplets move to neighbouring cells: no longer sorted
+                moved = rng.choice(w.n_sd, 200, replace=False)
+                ow.cell_id[moved] = np.clip(ow.cell_id[moved] + rng.integers(-1, 2, 200), 0, w.n_cell - 1).astype(np.int32)
+                cell.copy_(torch.from_numpy(ow.cell_id))
+            if s == 4:      # and the caller sorts everything again, in place
+                order = np.argsort(ow.cell_id, kind="stable")
+                ow.xi, ow.v, ow.cell_id = ow.xi[order].copy(), ow.v[order].copy(), ow.cell_id[order].copy()
+                xi.copy_(torch.from_numpy(ow.xi)); v.copy_(torch.from_numpy(ow.v)); cell.copy_(torch.from_numpy(ow.cell_id))
+            oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, okp, 42, s)
+            ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, s)
+            assert ctx.last_path() == expect[s], f"step {s}"
+            assert ctx.poll_error() == 0
+            assert np.array_equal(xi.cpu().numpy(), ow.xi), f"step {s}"
+            assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v.view(np.int64)), f"step {s}"
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_back_to_back_auto_steps_without_host_sync(dev, name):
+    """Several AUTO steps enqueued with nothing but the library's own calls in between (no poll, no synchronize,
+    no compaction): every call returns 0 and the result is the oracle's (a not-ready event query must not
+    poison the context)."""
+    sdm = _sdm()
+    for interleave in (False, True):
+        w = W.small(name, interleave=interleave)
         ow = w.copy()
-        oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), 42, 0)
-        ow.cell_id[100], ow.cell_id[5000] = ow.cell_id[5000], ow.cell_id[100]
-        oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), 42, 1)
-        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, 1)
-        assert ctx.last_path() == sdm.PATH_GENERAL and ctx.poll_error() == 0
-        assert np.array_equal(xi.cpu().numpy(), ow.xi)
+        okp, kp = _okp(w), _gkp(w)
+        with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+            xi, v, cell = _to_dev(w, dev)
+            for s in range(5):
+                ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, s)   # raises on rc != 0
+            assert ctx.poll_error() == 0
+            for s in range(5):
+                oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, okp, 42, s)
+            assert np.array_equal(xi.cpu().numpy(), ow.xi)
+            assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v.view(np.int64))
 
 
 def test_worked_step_on_device(dev):
@@ -513,6 +545,107 @@ def test_errors_and_bad_data(dev):
         assert ctx.launch_count() > 0
 
 
+# ------------------------------------------------------------------------------------------- the time loop
+def _run_multi(w, dev, path, n_steps, compact_every, chunks=(None,)):
+    """sdm_coalescence_steps against oracle.run, in one call or split into several calls (resume)."""
+    sdm = _sdm()
+    ow = w.copy()
+    n_o = oracle.run(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), w.seed, 0, n_steps, compact_every)
+    with sdm.SDMContext(max(w.n_sd, 1), w.n_cell, device=dev) as ctx:
+        if path is not None:
+            ctx.set_path(path)
+        xi, v, cell = _to_dev(w, dev)
+        n, s = w.n_sd, 0
+        parts = [n_steps] if chunks == (None,) else list(chunks)
+        assert sum(parts) == n_steps
+        for k in parts:
+            # a call's compaction schedule counts from ITS first step: split only at multiples of compact_every
+            assert compact_every == 0 or s % compact_every == 0
+            n = ctx.coalescence_steps(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), w.seed, s, k, compact_every, n_sd=n)
+            s += k
+        assert ctx.poll_error() == 0
+        last = ctx.last_path()
+    assert n == n_o
+    assert np.array_equal(xi[:n].cpu().numpy(), ow.xi[:n])
+    assert np.array_equal(cell[:n].cpu().numpy(), ow.cell_id[:n])
+    assert np.array_equal(v[:n].cpu().numpy().view(np.int64), ow.v[:n].view(np.int64))
+    return n, last
+
+
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg3z", "cfg4", "cfg4s"])
+@pytest.mark.parametrize("path", ["auto", "general", "cell_sorted", "hybrid"])
+def test_multi_step_entry_matches_oracle_run(dev, name, path):
+    """sdm_coalescence_steps == oracle_run: n steps with the config's compaction schedule in ONE call,
+    on every path; cfg3z starts with 2 % zeros (halt at the first due step), cfg4s produces zeros all the time."""
+    sdm = _sdm()
+    if name in ("cfg0", "cfg1") and path in ("cell_sorted", "hybrid"):
+        pytest.skip("single cell: general path only")
+    w = W.small(name, interleave=(path == "hybrid"))
+    p = {"auto": None, "general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED, "hybrid": sdm.PATH_HYBRID}[path]
+    n_steps = {"cfg0": 40, "cfg4s": 30}.get(name, 7)
+    n, last = _run_multi(w, dev, p, n_steps, w.compact_every)
+    if name in ("cfg3z", "cfg4s"):
+        assert n < w.n_sd
+    if path == "auto" and name not in ("cfg0", "cfg1"):
+        assert last == sdm.PATH_CELL_SORTED
+
+
+@pytest.mark.parametrize("name,compact_every", [("cfg4s", 1), ("cfg4s", 3), ("cfg3z", 2), ("cfg4s", 0)])
+def test_multi_step_entry_compaction_schedules(dev, name, compact_every):
+    """every step / every third step / never; more steps than one chunk of the run loop (64) so that a halt is
+    noticed while later chunks are already enqueued"""
+    w = W.small(name)
+    _run_multi(w, dev, None, 150 if name == "cfg4s" else 9, compact_every)
+
+
+def test_multi_step_entry_interleaved_auto_and_resume(dev):
+    """AUTO on an interleaved array: one GENERAL step, then HYBRID for the rest of the call; and a run split into
+    three calls equals the run in one call (counter-based RNG: step0 carries the position)."""
+    sdm = _sdm()
+    _, last = _run_multi(W.small("cfg4s", interleave=True), dev, None, 30, 10)
+    assert last == sdm.PATH_HYBRID
+    _run_multi(W.small("cfg4s"), dev, None, 30, 10, chunks=(10, 0, 20))
+    _run_multi(W.small("cfg0"), dev, None, 40, 0, chunks=(1, 39))
+
+
+def test_multi_step_entry_edge_cases(dev):
+    sdm = _sdm()
+    w = W.small("cfg3")
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        before = xi.clone()
+        assert ctx.coalescence_steps(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), 42, 0, 0, 1) == w.n_sd
+        assert torch.equal(xi, before)
+        assert ctx.coalescence_steps(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), 42, 0, 5, 1, n_sd=0) == 0
+        for bad in (dict(n_steps=-1), dict(compact_every=-1)):
+            args = dict(n_steps=1, compact_every=0)
+            args.update(bad)
+            with pytest.raises(sdm.SDMError) as e:
+                ctx.coalescence_steps(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), 42, 0, args["n_steps"], args["compact_every"])
+            assert e.value.status == -1
+        # everything zero: the first due compaction empties the array and the run ends
+        xi.zero_()
+        assert ctx.coalescence_steps(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), 42, 0, 4, 1) == 0
+        assert ctx.poll_error() == 0
+
+
+def test_host_entry_with_a_different_cell_layout_per_call(dev):
+    """sdm_coalescence_step_host re-uploads cell_id into the same staging address every call; what AUTO
+    learned about the previous contents must not leak into the next call."""
+    sdm = _sdm()
+    wa, wb = W.small("cfg3"), W.small("cfg3", interleave=True)
+    wc = W.cfg3(n_cell=16, per_cell=300, n_steps=1)           # cells too large for the fused kernel
+    with sdm.SDMContext(max(wa.n_sd, wc.n_sd), max(wa.n_cell, wc.n_cell), device=dev, host_staging=True) as ctx:
+        for s, w in enumerate([wa, wb, wa, wc, wb, wa]):
+            ow = w.copy()
+            oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), 42, s)
+            xi, v, cell = (torch.from_numpy(a.copy()).pin_memory() for a in (w.xi, w.v, w.cell_id))
+            ctx.coalescence_step_host(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), 42, s)
+            assert np.array_equal(xi.numpy(), ow.xi), f"call {s}"
+            assert np.array_equal(v.numpy().view(np.int64), ow.v.view(np.int64)), f"call {s}"
+        assert ctx.poll_error() == 0
+
+
 # ------------------------------------------------------------------------------------------- full size
 FULL = {
     "cfg0": lambda: W.cfg0(),
@@ -546,6 +679,93 @@ def test_full_size_configs_two_steps(dev, name):
             gv = v[:n].cpu().numpy()
             _assert_vol_close(gv, ow.v[:n], f"{name} step {s}")
             assert np.array_equal(gv.view(np.int64), ow.v[:n].view(np.int64))
+
+
+def _compare_state(xi, v, cell, ow, n, what):
+    assert np.array_equal(xi[:n].cpu().numpy(), ow.xi[:n]), f"{what}: multiplicity"
+    assert np.array_equal(cell[:n].cpu().numpy(), ow.cell_id[:n]), f"{what}: cell_id"
+    assert np.array_equal(v[:n].cpu().numpy().view(np.int64), ow.v[:n].view(np.int64)), f"{what}: volume bits"
+
+
+@pytest.mark.parametrize("path", ["general", "cell_sorted", "hybrid"])
+def test_full_size_cfg3z_compaction_moves_data(dev, path):
+    """configs[3] at full size with 2 % of the input multiplicities 0 (R32 "3z"): the in-place k_compact runs over
+    4096 ticketed tiles in several waves and really moves data; two steps, a compaction after each, every element
+    against the oracle, on each path."""
+    sdm = _sdm()
+    w = W.cfg3(zero_fraction=0.02)
+    ow = w.copy()
+    okp, gkp = _okp(w), _gkp(w)
+    p = {"general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED, "hybrid": sdm.PATH_HYBRID}[path]
+    n = w.n_sd
+    with sdm.SDMContext(n, w.n_cell, device=dev) as ctx:
+        ctx.set_path(p)
+        ctx.set_option(sdm.OPT_TRACK_ZEROS, 1)
+        xi, v, cell = _to_dev(w, dev)
+        for s in range(2):
+            oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, okp, w.seed, s, n_sd=n)
+            ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, gkp, w.seed, s, n_sd=n)
+            n_o = oracle.remove_zero_multiplicity(ow.xi, ow.v, ow.cell_id, n_sd=n)
+            n_g = ctx.remove_zero_multiplicity(xi, v, cell, n_sd=n)
+            assert n_g == n_o and (s > 0 or n_o < n - 100_000)
+            n = n_o
+            assert ctx.poll_error() == 0
+            _compare_state(xi, v, cell, ow, n, f"{path} step {s}")
+
+
+def test_full_size_cfg4_stress_crosses_a_compaction(dev):
+    """configs[4] at full size with dV = 1 m^3 (R32 "4s"): large gamma, the clamp, splits to zero (the first zeros
+    appear at step 12); 22 steps in ONE sdm_coalescence_steps call with compactions due after steps 10 (nothing to
+    remove) and 20 (the run halts on the device, the host compacts ~4.5e5 entries out of 6.5e6 over 3200 tiles and
+    resumes), every element against oracle_run."""
+    sdm = _sdm()
+    w = W.cfg4(stress=True)
+    ow = w.copy()
+    n_o = oracle.run(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), w.seed, 0, 22, 10)
+    assert n_o < w.n_sd - 100_000
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        n = ctx.coalescence_steps(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), w.seed, 0, 22, 10)
+        assert ctx.poll_error() == 0 and ctx.last_path() == sdm.PATH_CELL_SORTED
+    assert n == n_o
+    _compare_state(xi, v, cell, ow, n, "cfg4s 22 steps")
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+@pytest.mark.parametrize("path", ["general", "hybrid"])
+def test_full_size_interleaved_order(dev, name, path):
+    """R30: the full-size configs in a random memory order -- the input the GENERAL and HYBRID paths exist for --
+    one step (+ configs[3]'s compaction call) against the oracle, every element."""
+    sdm = _sdm()
+    w = W.cfg3(interleave=True) if name == "cfg3" else W.cfg4(interleave=True)
+    ow = w.copy()
+    p = {"general": sdm.PATH_GENERAL, "hybrid": sdm.PATH_HYBRID}[path]
+    n = w.n_sd
+    with sdm.SDMContext(n, w.n_cell, device=dev) as ctx:
+        ctx.set_path(p)
+        xi, v, cell = _to_dev(w, dev)
+        oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), w.seed, 0)
+        ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), w.seed, 0)
+        if w.compact_every:
+            assert ctx.remove_zero_multiplicity(xi, v, cell) == oracle.remove_zero_multiplicity(ow.xi, ow.v, ow.cell_id)
+        assert ctx.poll_error() == 0 and ctx.last_path() == p
+    _compare_state(xi, v, cell, ow, n, f"{name} interleaved {path}")
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_full_size_multi_step_entry(dev, name):
+    """The launch configuration bench.py times: sdm_coalescence_steps on the full-size config (AUTO, debug outputs
+    off), three steps with the config's compaction schedule, every element against oracle_run."""
+    sdm = _sdm()
+    w = FULL[name]()
+    ow = w.copy()
+    n_o = oracle.run(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), w.seed, 0, 3, w.compact_every)
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        n = ctx.coalescence_steps(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), w.seed, 0, 3, w.compact_every)
+        assert ctx.poll_error() == 0 and ctx.last_path() == sdm.PATH_CELL_SORTED
+    assert n == n_o
+    _compare_state(xi, v, cell, ow, n, f"{name} multi-step")
 
 
 def test_cfg0_long_run_matches_oracle(dev):
@@ -592,6 +812,48 @@ def test_shards_with_index_base_reproduce_the_unsharded_step(dev, name, path):
             lo, n = sh.index_base, sw.n_sd
             assert np.array_equal(xi.cpu().numpy(), ow.xi[lo:lo + n])
             assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v[lo:lo + n].view(np.int64))
+
+
+@pytest.mark.parametrize("name", ["cfg3z", "cfg4s"])
+def test_shards_cross_a_compaction_with_rebased_index_base(dev, name):
+    """after a compaction the Philox counter of a shard's first entry is the number of survivors on the
+    ranks before it.  Two shards (one after the other on one GPU), each advanced with sdm_coalescence_steps from
+    compaction to compaction, index_base re-based by sdm_workloads.rebase() from the surviving counts -- the 8-byte
+    all_gather of a multi-GPU run -- against the UNSHARDED oracle run, bit for bit."""
+    sdm = _sdm()
+    w = W.small(name)
+    every = w.compact_every
+    n_rounds = 3
+    ow = w.copy()
+    n_o = oracle.run(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), w.seed, 0, n_rounds * every, every)
+    assert n_o < w.n_sd
+    shards = [W.shard(w, r, 2) for r in range(2)]
+    ctxs = [sdm.SDMContext(sh.work.n_sd, sh.work.n_cell, device=dev) for sh in shards]
+    try:
+        state = [_to_dev(sh.work, dev) for sh in shards]
+        counts = [sh.work.n_sd for sh in shards]
+        for rnd in range(n_rounds):
+            bases = W.rebase(counts)
+            if rnd == 0:
+                assert bases == [sh.index_base for sh in shards]
+            for r, sh in enumerate(shards):
+                sw = sh.work
+                ctxs[r].set_option(sdm.OPT_INDEX_BASE, bases[r])
+                counts[r] = ctxs[r].coalescence_steps(*state[r], sw.n_cell, sw.dt, sw.dV, _gkp(sw), sw.seed, rnd * every,
+                                                      every, every, n_sd=counts[r])
+                assert ctxs[r].poll_error() == 0
+        assert sum(counts) == n_o
+        lo = 0
+        for r, sh in enumerate(shards):
+            xi, v, cell = state[r]
+            n = counts[r]
+            assert np.array_equal(xi[:n].cpu().numpy(), ow.xi[lo:lo + n])
+            assert np.array_equal(v[:n].cpu().numpy().view(np.int64), ow.v[lo:lo + n].view(np.int64))
+            assert np.array_equal(cell[:n].cpu().numpy() + sh.cell_lo, ow.cell_id[lo:lo + n])
+            lo += n
+    finally:
+        for c in ctxs:
+            c.close()
 
 
 # ------------------------------------------------------------------------------------------- NEXT-2: spectrum
