@@ -47,18 +47,35 @@ typedef enum {
     SDM_ERR_BAD_DATA = -4
 } sdm_status;
 
-typedef enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GEOMETRIC = 1 } sdm_kernel_kind;
+typedef enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GEOMETRIC = 1, SDM_KERNEL_GEOMETRIC_TABLE = 2 } sdm_kernel_kind;
 
 /* Coalescence kernel K(v_j, v_k) [m^3 s^-1] (north_star (c)):
  *   Golovin:  K = b (v_j + v_k), b in s^-1, volumes in m^3.
  *   geometric:     K = E pi (r_j + r_k)^2 |v_t(r_j) - v_t(r_k)|, r = cbrt(3 v / 4 pi),
- *                                v_t a three-regime power law (R16). */
+ *                                v_t a three-regime power law (R16).
+ *   geometric + table ("more sophisticated collision kernels ... the influence of electric field";
+ *                                SURVEY 8(f) NEXT-3): the same with E = E(r_big, r_small / r_big) interpolated
+ *                                in the table installed by sdm_set_collision_efficiency(); the field E is ignored. */
 typedef struct {
     int32_t kind; /* sdm_kernel_kind */
     int32_t _pad;
     double b; /* Golovin coefficient, >= 0 */
     double E; /* geometric collision efficiency, >= 0 (configs use 1.0) */
 } sdm_kernel_params;
+
+/* Collision-efficiency table of SDM_KERNEL_GEOMETRIC_TABLE (reading R39; the paper names the kernels of the Berry
+ * 1966 example -- hydrodynamic and electric-field efficiencies -- but prints no numbers, and none are in this
+ * repository: the caller supplies them, one table per variant).
+ *   radius  HOST fp64[n_r], strictly ascending, metres: the grid of the LARGER radius of the pair
+ *   table   HOST fp64[n_r][n_p], row-major, finite and >= 0: E at (radius[i], p_j = j / (n_p - 1)), p = r_small / r_big
+ * Bilinear interpolation in a fixed, FMA-free order:  i = last interval with radius[i] <= r_big (clamped),
+ * t_r = (r_big - radius[i]) / (radius[i+1] - radius[i]) clamped to [0, 1] (outside the grid: the value on its
+ * edge);  f = p (n_p - 1), j = min(floor(f), n_p - 2), t_p = f - j;  e0 = T[i][j] + t_p (T[i][j+1] - T[i][j]),
+ * e1 likewise in row i + 1;  E = e0 + t_r (e1 - e0).  A constant table reproduces SDM_KERNEL_GEOMETRIC bit for bit.
+ * The table is copied into the context's workspace (2 <= n_r, n_p <= 128); all-NULL / 0 arguments remove it.
+ * Errors: INVALID_ARG (bad sizes, radius not ascending, entries negative or not finite), CAPACITY (too large). */
+int sdm_set_collision_efficiency(sdm_ctx* ctx, const double* radius /* host */, int32_t n_r, int32_t n_p,
+                                 const double* table /* host */);
 
 /* Path selection for sdm_coalescence_step / sdm_coalescence_steps (sdm_set_path).  Every path produces the same bits.
  *   GENERAL      global stable LSD radix sort of (cell_id, Philox key): north_star (b).  Any input.
@@ -107,7 +124,8 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
  * droplets are never reordered.  Asynchronous.  (seed, step, array index) fully determine the random
  * numbers, so a run can be resumed bit-exactly.  n_sd == 0 is a no-op.
  * Errors: INVALID_ARG (null pointers, n_sd < 0, n_cell < 1, dt <= 0, dV <= 0, non-finite dt/dV,
- * unknown kernel kind, b < 0 or E < 0), CAPACITY (n_sd > max_n_sd, n_cell > max_n_cell), CUDA. */
+ * unknown kernel kind, b < 0 or E < 0, SDM_KERNEL_GEOMETRIC_TABLE without a table), CAPACITY (n_sd > max_n_sd,
+ * n_cell > max_n_cell), CUDA. */
 int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, const int32_t* cell_id,
                          int64_t n_sd, int32_t n_cell, double dt, double dV,
                          const sdm_kernel_params* kp, uint64_t seed, uint64_t step);
@@ -157,6 +175,24 @@ int sdm_cell_stats(sdm_ctx* ctx, const int64_t* multiplicity, const double* volu
 int sdm_volume_spectrum(sdm_ctx* ctx, const int64_t* multiplicity, const double* volume, int64_t n_sd,
                         const double* volume_edges /* host */, int32_t n_edges, int64_t* count, int64_t* sum_xi,
                         double* sum_xi_v);
+
+/* Particle displacement on the 2-D kinematic grid and the recomputation of cell_id (the step
+ * BEFORE the coalescence path; PAPER.md:80 lists "particle displacement" among the dynamics
+ * describe the kinematic_2d slab with its prescribed flow; the paper states no scheme -- readings R36-R38):
+ *   positions x, z: DEVICE fp64[n_sd] in GRID UNITS, x in [0, nx), z in [0, nz); both directions periodic;
+ *   cell_id = floor(z) * nx + floor(x)  (row-major, x fastest; a position ON a cell edge belongs to the upper cell);
+ *   sdm_displace: one explicit-Euler step with the velocity of the cell the super-droplet is in BEFORE the move,
+ *       c = cell_id(x, z);  x <- wrap(x + (u_cell[c] * dt), nx);  z <- wrap(z + (w_cell[c] * dt), nz)
+ *     u_cell, w_cell: DEVICE fp64[nx * nz], grid units per second, caller-supplied (|u dt| < nx, |w dt| < nz: at most
+ *     one period per step); wrap(q, n): q >= n -> q - n; q < 0 -> q + n; a result still outside [0, n) (a tiny negative
+ *     q whose q + n rounds to n) -> 0.  One multiplication and one addition per coordinate, no FMA.
+ * Both calls (re)write cell_id[n_sd] (DEVICE int32) and are asynchronous; sdm_displace updates x, z in place.  The
+ * coalescence step that follows sees a cell_id that is in general no longer sorted: AUTO takes the path that fits.
+ * Errors: INVALID_ARG (null pointers, n_sd < 0, nx or nz < 1, nx * nz >= 2^31, dt <= 0 or not finite), CUDA. */
+int sdm_cell_id_from_positions(sdm_ctx* ctx, const double* x, const double* z, int64_t n_sd, int32_t nx, int32_t nz,
+                               int32_t* cell_id);
+int sdm_displace(sdm_ctx* ctx, double* x, double* z, int32_t* cell_id, int64_t n_sd, int32_t nx, int32_t nz,
+                 const double* u_cell, const double* w_cell, double dt);
 
 /* Parity instrumentation (off by default; never on in timed runs).  Registers device arrays that
  * every later sdm_coalescence_step fills; pass NULL to switch an output off again.
@@ -225,7 +261,7 @@ int64_t sdm_launch_count(sdm_ctx* ctx);
  * host) since the last read, and resets the accumulation. */
 enum { SDM_PROF_KEYS_HIST = 0, SDM_PROF_CELL_SCAN, SDM_PROF_RADIX_PASS, SDM_PROF_PAIR, SDM_PROF_COUNT_ZERO,
        SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CELL_BOUNDS, SDM_PROF_CELL_FUSED,
-       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_TIE_REPAIR, SDM_PROF_SPECTRUM, SDM_PROF_CLASSES };
+       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_TIE_REPAIR, SDM_PROF_SPECTRUM, SDM_PROF_DISPLACE, SDM_PROF_CLASSES };
 int sdm_profile_enable(sdm_ctx* ctx, int on);
 int sdm_profile_read(sdm_ctx* ctx, double* ms_out /* host */, int64_t* launches_out /* host */);
 

@@ -25,11 +25,13 @@ def _load():
 
 
 class KernelParams(C.Structure):
-    _fields_ = [("kind", C.c_int32), ("_pad", C.c_int32), ("b", C.c_double), ("E", C.c_double)]
+    _fields_ = [("kind", C.c_int32), ("_pad", C.c_int32), ("b", C.c_double), ("E", C.c_double),
+                ("n_r", C.c_int32), ("n_p", C.c_int32), ("radius", C.c_void_p), ("table", C.c_void_p)]
 
 
 GOLOVIN = 0
 GEOMETRIC = 1
+GEOMETRIC_TABLE = 2
 
 _lib = _load()
 
@@ -52,6 +54,8 @@ _lib.oracle_terminal_velocity.argtypes = [C.c_double]
 _lib.oracle_terminal_velocity.restype = C.c_double
 _lib.oracle_radius.argtypes = [C.c_double]
 _lib.oracle_radius.restype = C.c_double
+_lib.oracle_efficiency.argtypes = [C.POINTER(KernelParams), C.c_double, C.c_double]
+_lib.oracle_efficiency.restype = C.c_double
 _lib.oracle_kernel.argtypes = [C.POINTER(KernelParams), C.c_double, C.c_double]
 _lib.oracle_kernel.restype = C.c_double
 _lib.oracle_gamma_from_p.argtypes = [C.c_double, C.c_double]
@@ -80,8 +84,37 @@ _lib.oracle_run.argtypes = [_i64p, _f64p, _i32p, C.c_int64, C.c_int32, C.c_doubl
 _lib.oracle_run.restype = C.c_int64
 
 
+_lib.oracle_wrap_periodic.argtypes = [C.c_double, C.c_int32]
+_lib.oracle_wrap_periodic.restype = C.c_double
+_lib.oracle_cell_of.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_int32]
+_lib.oracle_cell_of.restype = C.c_int32
+_lib.oracle_cell_id_from_positions.argtypes = [_f64p, _f64p, C.c_int64, C.c_int32, C.c_int32, _i32p]
+_lib.oracle_cell_id_from_positions.restype = C.c_int
+_lib.oracle_displace.argtypes = [_f64p, _f64p, _i32p, C.c_int64, C.c_int32, C.c_int32, _f64p, _f64p, C.c_double]
+_lib.oracle_displace.restype = C.c_int
+
+
 def kernel_params(kind: int, b: float = 0.0, E: float = 1.0) -> KernelParams:
-    return KernelParams(kind=kind, _pad=0, b=b, E=E)
+    return KernelParams(kind=kind, _pad=0, b=b, E=E, n_r=0, n_p=0, radius=None, table=None)
+
+
+def geometric_table(radius, table) -> KernelParams:
+    """Geometric kernel with a tabulated collision efficiency E(r_big, r_small / r_big) (R39): `radius` strictly
+    ascending [n_r], `table` [n_r][n_p] over the ratios j / (n_p - 1).  The arrays are kept alive by the result."""
+    r = np.ascontiguousarray(radius, np.float64)
+    t = np.ascontiguousarray(table, np.float64)
+    if r.ndim != 1 or t.ndim != 2 or t.shape[0] != r.shape[0] or r.shape[0] < 2 or t.shape[1] < 2:
+        raise ValueError("table shape")
+    if not np.all(np.diff(r) > 0) or not np.all(np.isfinite(t)) or np.any(t < 0):
+        raise ValueError("table values")
+    kp = KernelParams(kind=GEOMETRIC_TABLE, _pad=0, b=0.0, E=0.0, n_r=r.shape[0], n_p=t.shape[1],
+                      radius=r.ctypes.data, table=t.ctypes.data)
+    kp._keep = (r, t)
+    return kp
+
+
+def efficiency(kp: KernelParams, r_big: float, p: float) -> float:
+    return float(_lib.oracle_efficiency(C.byref(kp), r_big, p))
 
 
 def golovin(b: float) -> KernelParams:
@@ -207,3 +240,28 @@ def run(xi, v, cell_id, n_cell, dt, dV, kp, seed, step0, n_steps, compact_every=
     if r < 0:
         raise ValueError(f"oracle_run failed: {r}")
     return r
+
+
+def wrap_periodic(q: float, n: int) -> float:
+    return float(_lib.oracle_wrap_periodic(q, n))
+
+
+def cell_of(x: float, z: float, nx: int, nz: int) -> int:
+    return int(_lib.oracle_cell_of(x, z, nx, nz))
+
+
+def cell_id_from_positions(x, z, nx, nz) -> np.ndarray:
+    """O8: cell_id = floor(z) * nx + floor(x) for positions in grid units."""
+    out = np.zeros(len(x), np.int32)
+    rc = _lib.oracle_cell_id_from_positions(x, z, len(x), nx, nz, out)
+    if rc != 0:
+        raise ValueError(f"oracle_cell_id_from_positions failed: {rc}")
+    return out
+
+
+def displace(x, z, cell_id, nx, nz, u_cell, w_cell, dt):
+    """O8: one explicit-Euler displacement step on the periodic nx x nz grid, in place; rewrites cell_id."""
+    rc = _lib.oracle_displace(x, z, cell_id, len(x), nx, nz, np.ascontiguousarray(u_cell, np.float64),
+                              np.ascontiguousarray(w_cell, np.float64), dt)
+    if rc != 0:
+        raise ValueError(f"oracle_displace failed: {rc}")

@@ -23,6 +23,11 @@
 //                         closed-form bin masses of the exponential spectrum
 //   geometric kernel .... hand values; det_cbrt vs libm cbrt.  Whole-run statistics
 //                         with the geometric kernel: PARITY UNPINNED beyond invariants.
+//   efficiency table .... a constant table reproduces the geometric kernel bit for bit; a 2 x 2 table by hand;
+//                         scipy's RegularGridInterpolator on random tables; clamping outside the grid
+//   displacement (O8) ... hand cases on cell edges and at the periodic seam, numpy floor/mod, and a
+//                         divergence-free shear field with whole-cell Courant numbers (closed form:
+//                         every row shifts by its own number of cells, occupancy permutes)
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
@@ -85,10 +90,14 @@ void oracle_sd_random_batch(uint64_t seed, uint64_t step, uint64_t i0, int64_t n
 // PAPER.md:96 "geometric sweep-out"; readings R15, R16, R17).
 // ---------------------------------------------------------------------------
 struct oracle_kernel_params {
-    int32_t kind;  // 0 = Golovin, 1 = geometric
+    int32_t kind;  // 0 = Golovin, 1 = geometric, 2 = geometric with a tabulated collision efficiency
     int32_t _pad;
     double b;      // Golovin: K = b (v_j + v_k), b in 1/s, volumes in m^3
     double E;      // geometric: collision efficiency
+    // kind 2 ("more sophisticated collision kernels"; reading R39): E(r_big, p)
+    int32_t n_r, n_p;        // grid: n_r radii (strictly ascending, m), n_p ratios p_j = j / (n_p - 1)
+    const double* radius;    // [n_r]
+    const double* table;     // [n_r][n_p], row-major, >= 0
 };
 
 // R17: libm-free cube root: integer seed for x^(-1/3), four Newton steps on z,
@@ -119,6 +128,32 @@ double oracle_terminal_velocity(double r) {
 
 double oracle_radius(double v) { return oracle_det_cbrt(v * 0.238732414637843); }
 
+// R39: tabulated collision efficiency E(r_big, p), p = r_small / r_big in [0, 1], bilinear in a fixed order:
+//   i   = the interval of the radius grid that holds r_big (largest i with R[i] <= r_big, clamped to [0, n_r - 2]),
+//   t_r = (r_big - R[i]) / (R[i+1] - R[i]) clamped to [0, 1]            (outside the grid: the value on its edge)
+//   f   = p * (n_p - 1);  j = min(floor(f), n_p - 2);  t_p = f - j
+//   e0  = T[i][j]   + t_p * (T[i][j+1]   - T[i][j])
+//   e1  = T[i+1][j] + t_p * (T[i+1][j+1] - T[i+1][j])
+//   E   = e0 + t_r * (e1 - e0)                                            (every product rounded before its sum: no FMA)
+double oracle_efficiency(const oracle_kernel_params* kp, double r_big, double p) {
+    const int32_t n_r = kp->n_r, n_p = kp->n_p;
+    int32_t i = 0;
+    while (i + 2 < n_r && kp->radius[i + 1] <= r_big) ++i;  // linear scan: the last interval whose lower edge is <= r_big
+    double t_r = (r_big - kp->radius[i]) / (kp->radius[i + 1] - kp->radius[i]);
+    if (!(t_r > 0.0)) t_r = 0.0;
+    if (t_r > 1.0) t_r = 1.0;
+    const double f = p * (double)(n_p - 1);
+    int32_t j = (int32_t)std::floor(f);
+    if (j < 0) j = 0;
+    if (j > n_p - 2) j = n_p - 2;
+    const double t_p = f - (double)j;
+    const double* T0 = kp->table + (size_t)i * n_p;
+    const double* T1 = T0 + n_p;
+    const double e0 = T0[j] + t_p * (T0[j + 1] - T0[j]);
+    const double e1 = T1[j] + t_p * (T1[j + 1] - T1[j]);
+    return e0 + t_r * (e1 - e0);
+}
+
 double oracle_kernel(const oracle_kernel_params* kp, double vj, double vk) {
     if (kp->kind == 0) {
         return kp->b * (vj + vk);
@@ -126,7 +161,12 @@ double oracle_kernel(const oracle_kernel_params* kp, double vj, double vk) {
     const double rj = oracle_radius(vj);
     const double rk = oracle_radius(vk);
     const double s = rj + rk;
-    return ((kp->E * 3.141592653589793) * (s * s)) *
+    double E = kp->E;
+    if (kp->kind == 2) {
+        const double r_big = rj > rk ? rj : rk, r_small = rj > rk ? rk : rj;
+        E = oracle_efficiency(kp, r_big, r_big > 0.0 ? r_small / r_big : 0.0);
+    }
+    return ((E * 3.141592653589793) * (s * s)) *
            std::fabs(oracle_terminal_velocity(rj) - oracle_terminal_velocity(rk));
 }
 
@@ -307,6 +347,56 @@ int oracle_volume_spectrum(const int64_t* xi, const double* v, int64_t n_sd, con
         if (count) count[b] += 1;
         if (sum_xi) sum_xi[b] += xi[i];
         if (sum_xi_v) sum_xi_v[b] += (double)xi[i] * x;
+    }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O8  Displacement + cell_id recomputation (the step BEFORE the coalescence path; the paper's
+// "particle displacement" dynamic, on the kinematic_2d grid of PAPER.md:112-118).  The paper gives no
+// scheme; readings R36-R38: positions in GRID UNITS, x in [0, nx), z in [0, nz), both directions
+// periodic; cell_id = floor(z) * nx + floor(x) (row-major, x fastest); one explicit-Euler step with the velocity
+// (grid units per second, caller-supplied per cell) of the cell the super-droplet is in BEFORE the move:
+//     c  = cell_of(x, z)
+//     x1 = x + (u[c] * dt)          (one multiplication, one addition, no FMA)
+//     x1 = wrap(x1, nx)             (at most one period: |u dt| < nx is the caller's contract)
+// and the same for z with w[c], nz.  wrap(q, n): q >= n -> q - n;  q < 0 -> q + n;  and if the result is still
+// outside [0, n) -- only possible when a tiny negative q rounds q + n up to n -- it is 0.
+// ---------------------------------------------------------------------------
+double oracle_wrap_periodic(double q, int32_t n) {
+    const double dn = (double)n;
+    if (q >= dn) q = q - dn;
+    else if (q < 0.0) q = q + dn;
+    if (!(q >= 0.0 && q < dn)) q = 0.0;
+    return q;
+}
+
+int32_t oracle_cell_of(double x, double z, int32_t nx, int32_t nz) {
+    int64_t ix = (int64_t)std::floor(x), iz = (int64_t)std::floor(z);
+    if (ix < 0) ix = 0;  // positions are inside the domain by contract; clamp keeps bad data memory-safe
+    if (ix >= nx) ix = nx - 1;
+    if (iz < 0) iz = 0;
+    if (iz >= nz) iz = nz - 1;
+    return (int32_t)(iz * (int64_t)nx + ix);
+}
+
+int oracle_cell_id_from_positions(const double* x, const double* z, int64_t n_sd, int32_t nx, int32_t nz,
+                                  int32_t* cell_id) {
+    if (n_sd < 0 || nx < 1 || nz < 1 || (int64_t)nx * nz > 2147483647LL) return -1;
+    for (int64_t i = 0; i < n_sd; ++i) cell_id[i] = oracle_cell_of(x[i], z[i], nx, nz);
+    return 0;
+}
+
+int oracle_displace(double* x, double* z, int32_t* cell_id, int64_t n_sd, int32_t nx, int32_t nz,
+                    const double* u_cell, const double* w_cell, double dt) {
+    if (n_sd < 0 || nx < 1 || nz < 1 || (int64_t)nx * nz > 2147483647LL || !(dt > 0.0)) return -1;
+    for (int64_t i = 0; i < n_sd; ++i) {
+        const int32_t c = oracle_cell_of(x[i], z[i], nx, nz);
+        const double x1 = oracle_wrap_periodic(x[i] + (u_cell[c] * dt), nx);
+        const double z1 = oracle_wrap_periodic(z[i] + (w_cell[c] * dt), nz);
+        x[i] = x1;
+        z[i] = z1;
+        cell_id[i] = oracle_cell_of(x1, z1, nx, nz);
     }
     return 0;
 }

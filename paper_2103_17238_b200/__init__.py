@@ -7,6 +7,7 @@ the built CUDA library, or without a CUDA device, the calls raise.
 """
 from .binding import (  # noqa: F401
     GEOMETRIC,
+    GEOMETRIC_TABLE,
     GOLOVIN,
     PATH_AUTO,
     PATH_CELL_SORTED,
@@ -20,6 +21,7 @@ from .binding import (  # noqa: F401
     SDMContext,
     SDMError,
     geometric,
+    geometric_table,
     golovin,
     host_staging_bytes,
     library_path,
@@ -28,7 +30,7 @@ from .binding import (  # noqa: F401
 )
 
 __all__ = [
-    "SDMContext", "SDMError", "KernelParams", "golovin", "geometric", "GOLOVIN", "GEOMETRIC",
+    "SDMContext", "SDMError", "KernelParams", "golovin", "geometric", "geometric_table", "GOLOVIN", "GEOMETRIC", "GEOMETRIC_TABLE",
     "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "OPT_NARROW_KEY_BITS", "OPT_TRACK_ZEROS", "OPT_INDEX_BASE", "OPT_SKIP_KEY_DIGITS", "workspace_bytes", "host_staging_bytes",
     "load_library", "library_path",
 ]

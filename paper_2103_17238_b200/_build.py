@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libsdm_b200.so")
-SOURCES = ["sdm_api.cu", "sdm_hist.cu", "sdm_sort.cu", "sdm_pair.cu", "sdm_cellsort.cu", "sdm_compact.cu", "sdm_spectrum.cu"]
+SOURCES = ["sdm_api.cu", "sdm_hist.cu", "sdm_sort.cu", "sdm_pair.cu", "sdm_cellsort.cu", "sdm_compact.cu", "sdm_spectrum.cu", "sdm_displace.cu"]
 HEADERS = ["sdm_device.cuh", "sdm_internal.h", "sdm_pair.cuh", os.path.join("..", "..", "include", "sdm.h")]
 
 NVCC_FLAGS = [

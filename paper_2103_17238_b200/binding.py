@@ -14,6 +14,7 @@ _LIB_PATH = os.environ.get("SDM_B200_LIBRARY") or os.path.join(_HERE, "libsdm_b2
 
 GOLOVIN = 0
 GEOMETRIC = 1
+GEOMETRIC_TABLE = 2
 PATH_AUTO = 0
 PATH_GENERAL = 1
 PATH_CELL_SORTED = 2
@@ -30,11 +31,12 @@ EXPORTS = [
     "sdm_cell_stats", "sdm_debug_outputs", "sdm_set_path", "sdm_last_path", "sdm_host_staging_bytes",
     "sdm_bind_host_staging", "sdm_coalescence_step_host", "sdm_poll_error", "sdm_launch_count",
     "sdm_philox_fill", "sdm_kernel_eval", "sdm_strerror", "sdm_destroy", "sdm_profile_enable",
-    "sdm_profile_read", "sdm_set_option", "sdm_volume_spectrum",
+    "sdm_profile_read", "sdm_set_option", "sdm_volume_spectrum", "sdm_displace", "sdm_cell_id_from_positions",
+    "sdm_set_collision_efficiency",
 ]
 
 PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
-                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum"]
+                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum", "displace"]
 
 
 class SDMError(RuntimeError):
@@ -53,6 +55,11 @@ def golovin(b: float) -> KernelParams:
 
 def geometric(E: float = 1.0) -> KernelParams:
     return KernelParams(kind=GEOMETRIC, _pad=0, b=0.0, E=float(E))
+
+
+def geometric_table() -> KernelParams:
+    """Geometric kernel with the collision-efficiency table installed by SDMContext.set_collision_efficiency."""
+    return KernelParams(kind=GEOMETRIC_TABLE, _pad=0, b=0.0, E=0.0)
 
 
 _lib = None
@@ -106,6 +113,12 @@ def load_library():
     lib.sdm_coalescence_step_host.restype = C.c_int
     lib.sdm_volume_spectrum.argtypes = [vp, vp, vp, i64, C.POINTER(C.c_double), i32, vp, vp, vp]
     lib.sdm_volume_spectrum.restype = C.c_int
+    lib.sdm_displace.argtypes = [vp, vp, vp, vp, i64, i32, i32, vp, vp, dbl]
+    lib.sdm_displace.restype = C.c_int
+    lib.sdm_cell_id_from_positions.argtypes = [vp, vp, vp, i64, i32, i32, vp]
+    lib.sdm_cell_id_from_positions.restype = C.c_int
+    lib.sdm_set_collision_efficiency.argtypes = [vp, C.POINTER(C.c_double), i32, i32, C.POINTER(C.c_double)]
+    lib.sdm_set_collision_efficiency.restype = C.c_int
     lib.sdm_poll_error.argtypes = [vp]
     lib.sdm_poll_error.restype = C.c_int
     lib.sdm_launch_count.argtypes = [vp]
@@ -280,6 +293,38 @@ class SDMContext:
                                            len(edges), count.data_ptr(), sum_xi.data_ptr(), sum_xi_v.data_ptr())
         _check(rc, "sdm_volume_spectrum")
         return count, sum_xi, sum_xi_v
+
+    def displace(self, x, z, cell_id, nx, nz, u_cell, w_cell, dt, n_sd=None):
+        """sdm_displace: one explicit-Euler step on the periodic nx x nz grid; x, z, cell_id updated in place."""
+        t = self._torch
+        n = int(x.shape[0] if n_sd is None else n_sd)
+        rc = self._lib.sdm_displace(self._h, _ptr(x, t.float64), _ptr(z, t.float64), _ptr(cell_id, t.int32), n, int(nx),
+                                    int(nz), _ptr(u_cell, t.float64), _ptr(w_cell, t.float64), float(dt))
+        _check(rc, "sdm_displace")
+
+    def cell_id_from_positions(self, x, z, nx, nz, cell_id=None, n_sd=None):
+        t = self._torch
+        n = int(x.shape[0] if n_sd is None else n_sd)
+        if cell_id is None:
+            cell_id = t.empty(max(n, 1), dtype=t.int32, device=self.device)
+        rc = self._lib.sdm_cell_id_from_positions(self._h, _ptr(x, t.float64), _ptr(z, t.float64), n, int(nx), int(nz),
+                                                  _ptr(cell_id, t.int32))
+        _check(rc, "sdm_cell_id_from_positions")
+        return cell_id
+
+    def set_collision_efficiency(self, radius, table):
+        """sdm_set_collision_efficiency: `radius` [n_r] ascending (m), `table` [n_r][n_p] (nested sequences or a
+        2-D array); None, None removes the table."""
+        if radius is None and table is None:
+            _check(self._lib.sdm_set_collision_efficiency(self._h, None, 0, 0, None), "sdm_set_collision_efficiency")
+            return
+        rows = [[float(e) for e in row] for row in table]
+        n_r, n_p = len(rows), (len(rows[0]) if rows else 0)
+        if any(len(row) != n_p for row in rows) or len(radius) != n_r:
+            raise ValueError("table shape")
+        r = (C.c_double * n_r)(*[float(x) for x in radius])
+        t = (C.c_double * (n_r * n_p))(*[e for row in rows for e in row])
+        _check(self._lib.sdm_set_collision_efficiency(self._h, r, n_r, n_p, t), "sdm_set_collision_efficiency")
 
     def set_option(self, option: int, value: int):
         _check(self._lib.sdm_set_option(self._h, int(option), int(value)), "sdm_set_option")

@@ -70,6 +70,8 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     w.buf_b = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.cmp_state = reinterpret_cast<u32*>(take(cmp_tiles * 4));
     w.spec_edges = reinterpret_cast<double*>(take((size_t)SPECTRUM_MAX_EDGES * 8));
+    w.eff_radius = reinterpret_cast<double*>(take((size_t)EFF_MAX_R * 8));
+    w.eff_table = reinterpret_cast<double*>(take((size_t)EFF_MAX_R * EFF_MAX_P * 8));
     w.scan_state_bytes = ((size_t)max_n_cell / 4096 + 2) * 8;
     w.scan_state = reinterpret_cast<u64*>(take(w.scan_state_bytes));
     w.run = reinterpret_cast<u32*>(take(RUN_WORDS * 4));
@@ -294,9 +296,11 @@ static int validate_step(sdm_ctx* ctx, const void* xi, const void* v, const void
     if (!(dt > 0.0) || !(dV > 0.0) || !std::isfinite(dt) || !std::isfinite(dV)) return SDM_ERR_INVALID_ARG;
     const double dtdV = dt / dV;
     if (!std::isfinite(dtdV) || !(dtdV > 0.0)) return SDM_ERR_INVALID_ARG;
-    if (kp->kind != SDM_KERNEL_GOLOVIN && kp->kind != SDM_KERNEL_GEOMETRIC) return SDM_ERR_INVALID_ARG;
+    if (kp->kind != SDM_KERNEL_GOLOVIN && kp->kind != SDM_KERNEL_GEOMETRIC && kp->kind != SDM_KERNEL_GEOMETRIC_TABLE)
+        return SDM_ERR_INVALID_ARG;
     if (kp->kind == SDM_KERNEL_GOLOVIN && !(kp->b >= 0.0 && std::isfinite(kp->b))) return SDM_ERR_INVALID_ARG;
     if (kp->kind == SDM_KERNEL_GEOMETRIC && !(kp->E >= 0.0 && std::isfinite(kp->E))) return SDM_ERR_INVALID_ARG;
+    if (kp->kind == SDM_KERNEL_GEOMETRIC_TABLE && ctx->eff_n_r == 0) return SDM_ERR_INVALID_ARG;  // no table installed
     if (n_sd > ctx->max_n_sd || n_cell > ctx->max_n_cell) return SDM_ERR_CAPACITY;
     return SDM_OK;
 }
@@ -315,14 +319,29 @@ struct StepArgs {
     uint64_t seed;
 };
 
-StepArgs make_step_args(int64_t* xi, double* v, const int32_t* cell_id, int64_t n_sd, int32_t n_cell, double dt,
-                        double dV, const sdm_kernel_params* kp, uint64_t seed) {
+KernelParams device_kernel_params(const sdm_ctx* ctx, const sdm_kernel_params* kp) {
+    KernelParams d;
+    d.kind = kp->kind;
+    d.b = kp->b;
+    d.Epi = kp->E * 3.141592653589793;
+    d.n_r = d.n_p = 0;
+    d.eff_radius = d.eff_table = nullptr;
+    if (kp->kind == SDM_KERNEL_GEOMETRIC_TABLE) {  // the bounds of the early-out use the table's maximum
+        d.Epi = ctx->eff_max * 3.141592653589793;
+        d.n_r = ctx->eff_n_r;
+        d.n_p = ctx->eff_n_p;
+        d.eff_radius = ctx->ws.eff_radius;
+        d.eff_table = ctx->ws.eff_table;
+    }
+    return d;
+}
+
+StepArgs make_step_args(const sdm_ctx* ctx, int64_t* xi, double* v, const int32_t* cell_id, int64_t n_sd,
+                        int32_t n_cell, double dt, double dV, const sdm_kernel_params* kp, uint64_t seed) {
     StepArgs A;
     A.xi = xi; A.v = v; A.cell_id = cell_id; A.n_sd = n_sd; A.n_cell = n_cell;
     A.dtdV = dt / dV;
-    A.dkp.kind = kp->kind;
-    A.dkp.b = kp->b;
-    A.dkp.Epi = kp->E * 3.141592653589793;
+    A.dkp = device_kernel_params(ctx, kp);
     A.seed = seed;
     return A;
 }
@@ -524,7 +543,7 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
                 return rc;
         return SDM_OK;
     }
-    const StepArgs A = make_step_args(multiplicity, volume, cell_id, n_sd, n_cell, dt, dV, kp, seed);
+    const StepArgs A = make_step_args(ctx, multiplicity, volume, cell_id, n_sd, n_cell, dt, dV, kp, seed);
     const StepLinks no_links = {nullptr, nullptr, nullptr, 0u};
     ctx->zero_hint_valid = 0;
     // ---- path selection (include/sdm.h, sdm_path) ----
@@ -697,7 +716,7 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
     int64_t s = 0;
     bool general_only = (n_cell <= 1) || ctx->path == SDM_PATH_GENERAL;
     while (s < n_steps && n > 0) {
-        const StepArgs A = make_step_args(multiplicity, volume, cell_id, n, n_cell, dt, dV, kp, seed);
+        const StepArgs A = make_step_args(ctx, multiplicity, volume, cell_id, n, n_cell, dt, dV, kp, seed);
         const Plan plan = make_plan(n, n_cell, ctx->skip_key_digits);
         if (!plan_fits(plan)) return SDM_ERR_CAPACITY;
         FusedSource src;
@@ -779,6 +798,61 @@ int sdm_cell_stats(sdm_ctx* ctx, const int64_t* multiplicity, const double* volu
     if (n_sd == 0) return SDM_OK;
     return note_cuda(ctx, launch_cell_stats(ctx, multiplicity, volume, cell_id, n_sd, n_cell, count, sum_xi,
                                             sum_xi_v, sum_xi_v2));
+}
+
+int sdm_cell_id_from_positions(sdm_ctx* ctx, const double* x, const double* z, int64_t n_sd, int32_t nx, int32_t nz,
+                               int32_t* cell_id) {
+    if (!ctx || n_sd < 0 || nx < 1 || nz < 1 || (int64_t)nx * nz > 2147483647LL) return SDM_ERR_INVALID_ARG;
+    if (n_sd > 0 && (!x || !z || !cell_id)) return SDM_ERR_INVALID_ARG;
+    if (ctx->cuda_error) return SDM_ERR_CUDA;
+    if (n_sd == 0) return SDM_OK;
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
+    return note_cuda(ctx, launch_displace(ctx, false, const_cast<double*>(x), const_cast<double*>(z), cell_id, n_sd, nx,
+                                          nz, nullptr, nullptr, 0.0));
+}
+
+int sdm_displace(sdm_ctx* ctx, double* x, double* z, int32_t* cell_id, int64_t n_sd, int32_t nx, int32_t nz,
+                 const double* u_cell, const double* w_cell, double dt) {
+    if (!ctx || n_sd < 0 || nx < 1 || nz < 1 || (int64_t)nx * nz > 2147483647LL) return SDM_ERR_INVALID_ARG;
+    if (!(dt > 0.0) || !std::isfinite(dt) || !u_cell || !w_cell) return SDM_ERR_INVALID_ARG;
+    if (n_sd > 0 && (!x || !z || !cell_id)) return SDM_ERR_INVALID_ARG;
+    if (ctx->cuda_error) return SDM_ERR_CUDA;
+    if (n_sd == 0) return SDM_OK;
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
+    return note_cuda(ctx, launch_displace(ctx, true, x, z, cell_id, n_sd, nx, nz, u_cell, w_cell, dt));
+}
+
+int sdm_set_collision_efficiency(sdm_ctx* ctx, const double* radius, int32_t n_r, int32_t n_p, const double* table) {
+    if (!ctx) return SDM_ERR_INVALID_ARG;
+    if (!radius && !table && n_r == 0 && n_p == 0) {  // remove the table
+        ctx->eff_n_r = ctx->eff_n_p = 0;
+        return SDM_OK;
+    }
+    if (!radius || !table || n_r < 2 || n_p < 2) return SDM_ERR_INVALID_ARG;
+    if (n_r > EFF_MAX_R || n_p > EFF_MAX_P) return SDM_ERR_CAPACITY;
+    double e_max = 0.0;
+    for (int32_t i = 0; i < n_r; ++i) {
+        if (!std::isfinite(radius[i]) || (i > 0 && !(radius[i] > radius[i - 1]))) return SDM_ERR_INVALID_ARG;
+        for (int32_t j = 0; j < n_p; ++j) {
+            const double e = table[(size_t)i * n_p + j];
+            if (!std::isfinite(e) || e < 0.0) return SDM_ERR_INVALID_ARG;
+            if (e > e_max) e_max = e;
+        }
+    }
+    if (ctx->cuda_error) return SDM_ERR_CUDA;
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
+    int rc;
+    // pageable host memory: both copies are staged before the call returns
+    if ((rc = note_cuda(ctx, cudaMemcpyAsync(ctx->ws.eff_radius, radius, (size_t)n_r * 8, cudaMemcpyHostToDevice,
+                                             ctx->stream))))
+        return rc;
+    if ((rc = note_cuda(ctx, cudaMemcpyAsync(ctx->ws.eff_table, table, (size_t)n_r * n_p * 8, cudaMemcpyHostToDevice,
+                                             ctx->stream))))
+        return rc;
+    ctx->eff_n_r = n_r;
+    ctx->eff_n_p = n_p;
+    ctx->eff_max = e_max;
+    return SDM_OK;
 }
 
 int sdm_poll_error(sdm_ctx* ctx) {
@@ -864,11 +938,8 @@ int sdm_kernel_eval(sdm_ctx* ctx, const sdm_kernel_params* kp, const double* vj,
     if (!ctx || !kp || n < 0 || (n > 0 && (!vj || !vk || !K_out))) return SDM_ERR_INVALID_ARG;
     if (n == 0) return SDM_OK;
     if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
-    KernelParams dkp;
-    dkp.kind = kp->kind;
-    dkp.b = kp->b;
-    dkp.Epi = kp->E * 3.141592653589793;
-    return note_cuda(ctx, launch_kernel_eval(ctx, dkp, vj, vk, n, K_out));
+    if (kp->kind == SDM_KERNEL_GEOMETRIC_TABLE && ctx->eff_n_r == 0) return SDM_ERR_INVALID_ARG;
+    return note_cuda(ctx, launch_kernel_eval(ctx, device_kernel_params(ctx, kp), vj, vk, n, K_out));
 }
 
 }  // extern "C"

@@ -119,10 +119,40 @@ __device__ __forceinline__ u64 ld_stream_u64(const u64* p) {
 // Coalescence kernels (north_star (c); R15-R17).  No FMA anywhere.
 // ------------------------------------------------------------------------------------------
 struct KernelParams {
-    int kind;  // 0 Golovin, 1 geometric
+    int kind;  // 0 Golovin, 1 geometric, 2 geometric with a tabulated collision efficiency (R39)
     double b;
-    double Epi;  // E * pi, one host-side product (E * 3.141592653589793)
+    double Epi;  // E * pi, one host-side product (E * 3.141592653589793); kind 2: E = the table's maximum (bounds only)
+    // kind 2: E(r_big, r_small / r_big) on n_r radii (ascending) x n_p ratios j / (n_p - 1); device pointers
+    int n_r, n_p;
+    const double* eff_radius;
+    const double* eff_table;
 };
+
+// R39: bilinear interpolation in a fixed order (every product rounded before its sum); outside the radius grid the
+// value on its edge.  The interval is the last one whose lower edge is <= r_big (binary search: same interval as the
+// linear scan of the definition).
+__device__ __forceinline__ double collision_efficiency(const KernelParams& kp, double r_big, double p) {
+    int lo = 0, hi = kp.n_r - 1;  // invariant: R[lo] <= r_big (or lo = 0), R[hi] > r_big (or hi = n_r - 1)
+    while (hi - lo > 1) {
+        const int m = (lo + hi) >> 1;
+        if (__ldg(kp.eff_radius + m) <= r_big) lo = m;
+        else hi = m;
+    }
+    const double r0 = __ldg(kp.eff_radius + lo), r1 = __ldg(kp.eff_radius + lo + 1);
+    double t_r = __ddiv_rn(__dsub_rn(r_big, r0), __dsub_rn(r1, r0));
+    if (!(t_r > 0.0)) t_r = 0.0;
+    if (t_r > 1.0) t_r = 1.0;
+    const double f = __dmul_rn(p, (double)(kp.n_p - 1));
+    int j = (int)floor(f);
+    j = j < 0 ? 0 : (j > kp.n_p - 2 ? kp.n_p - 2 : j);
+    const double t_p = __dsub_rn(f, (double)j);
+    const double* T0 = kp.eff_table + (size_t)lo * kp.n_p + j;
+    const double* T1 = T0 + kp.n_p;
+    const double a0 = __ldg(T0), a1 = __ldg(T0 + 1), b0 = __ldg(T1), b1 = __ldg(T1 + 1);
+    const double e0 = __dadd_rn(a0, __dmul_rn(t_p, __dsub_rn(a1, a0)));
+    const double e1 = __dadd_rn(b0, __dmul_rn(t_p, __dsub_rn(b1, b0)));
+    return __dadd_rn(e0, __dmul_rn(t_r, __dsub_rn(e1, e0)));
+}
 
 // R17: libm-free cube root: integer seed for x^(-1/3), four Newton steps, r = x z^2, one polish.
 __device__ __forceinline__ double det_cbrt(double x) {
@@ -156,7 +186,13 @@ __device__ __forceinline__ double coalescence_kernel(const KernelParams& kp, dou
     const double rk = det_cbrt(__dmul_rn(vk, 0.238732414637843));
     const double s = __dadd_rn(rj, rk);
     const double dv = fabs(__dsub_rn(terminal_velocity(rj), terminal_velocity(rk)));
-    return __dmul_rn(__dmul_rn(kp.Epi, __dmul_rn(s, s)), dv);
+    double Epi = kp.Epi;
+    if (kp.kind == 2) {
+        const double r_big = rj > rk ? rj : rk, r_small = rj > rk ? rk : rj;
+        const double E = collision_efficiency(kp, r_big, r_big > 0.0 ? __ddiv_rn(r_small, r_big) : 0.0);
+        Epi = __dmul_rn(E, 3.141592653589793);
+    }
+    return __dmul_rn(__dmul_rn(Epi, __dmul_rn(s, s)), dv);
 }
 
 }  // namespace sdm

@@ -23,6 +23,10 @@ constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
 // Largest cell the register-resident per-cell sort of the fast path handles (one warp, 8 keys per lane).
 constexpr int CELL_FAST_MAX = 256;
 
+// Largest collision-efficiency table sdm_set_collision_efficiency accepts (radii x ratios).
+constexpr int EFF_MAX_R = 128;
+constexpr int EFF_MAX_P = 128;
+
 // Largest number of bin edges sdm_volume_spectrum accepts (edges + per-bin sums live in shared memory).
 constexpr int SPECTRUM_MAX_EDGES = 1025;
 
@@ -76,6 +80,8 @@ struct Workspace {
     u64* buf_b;       // max_n_sd
     u32* cmp_state;   // max compaction tiles
     double* spec_edges;  // SPECTRUM_MAX_EDGES volume edges of sdm_volume_spectrum
+    double* eff_radius;  // EFF_MAX_R radii of the collision-efficiency table
+    double* eff_table;   // EFF_MAX_R x EFF_MAX_P entries
     u64* scan_state;  // k_cell_scan slab states (epoch-tagged; zeroed at init)
     size_t scan_state_bytes;
     size_t total_bytes;
@@ -95,7 +101,7 @@ struct Plan {  // per-step derived quantities
 namespace sdm {
 // Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
 enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
-                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_CLASSES };
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_DISPLACE, PROF_CLASSES };
 // What the last general-path step learned about the cell_id array (pinned host memory, written by an
 // asynchronous copy; valid once `verdict_event` has completed).
 struct Verdict { u32 unsorted; u32 max_count; };
@@ -137,6 +143,8 @@ struct sdm_ctx {
     // zero-multiplicity count left in ctl[CTL_ZERO_COUNT] by the last fused step (SDM_OPT_TRACK_ZEROS)
     sdm::u32 epoch;  // tag of the current fused-path step (>= 2; see k_cell_bounds)
     sdm::u64 index_base;  // SDM_OPT_INDEX_BASE
+    int eff_n_r, eff_n_p;  // collision-efficiency table installed by sdm_set_collision_efficiency (0 = none)
+    double eff_max;        // its largest entry: the E of the conservative early-out bounds
     int track_zeros;
     int zero_hint_valid;
     const void* zero_hint_xi;
@@ -214,6 +222,8 @@ cudaError_t init_volume_spectrum(sdm_ctx* ctx);
 cudaError_t launch_volume_spectrum(sdm_ctx* ctx, const int64_t* xi, const double* v, int64_t n_sd,
                                    const double* edges_dev, int32_t n_edges, int64_t* count, int64_t* sum_xi,
                                    double* sum_xi_v);
+cudaError_t launch_displace(sdm_ctx* ctx, bool move, double* x, double* z, int32_t* cell_id, int64_t n_sd, int32_t nx,
+                            int32_t nz, const double* u_cell, const double* w_cell, double dt);
 cudaError_t launch_philox_fill(sdm_ctx* ctx, const PhiloxKeys& pk, u64 i0, int64_t n, u32* key_out,
                                double* u_out);
 cudaError_t launch_kernel_eval(sdm_ctx* ctx, const KernelParams& kp, const double* vj, const double* vk,

@@ -212,3 +212,38 @@ def rebase(n_sd_per_rank) -> list:
         bases.append(acc)
         acc += int(n)
     return bases
+
+
+# ------------------------------------------------------------------------------------------------
+# Inputs of the displacement step ("a prescribed single-eddy non-divergent
+# flow ... updraft in the left-hand part of the domain, downdraft in the right-hand part").  Input generation only:
+# the method's arithmetic (the Euler step, the wrap, the cell index) lives in oracle/ and in csrc/, not here.
+def grid_shape(n_cell: int):
+    """(nx, nz) of a square 2-D grid with n_cell cells (configs[2]: 128 x 128, configs[3]: 256 x 256)."""
+    nx = int(round(math.sqrt(n_cell)))
+    if nx * nx != n_cell:
+        raise ValueError("not a square grid")
+    return nx, nx
+
+
+def positions_in_cells(cell_id: np.ndarray, nx: int, nz: int, seed: int = 7):
+    """Uniformly random positions (grid units) inside the cell every super-droplet is listed in."""
+    rng = np.random.default_rng(seed)
+    n = cell_id.shape[0]
+    x = (cell_id % nx).astype(np.float64) + rng.random(n)
+    z = (cell_id // nx).astype(np.float64) + rng.random(n)
+    return np.minimum(x, np.nextafter(float(nx), 0.0)), np.minimum(z, np.nextafter(float(nz), 0.0))
+
+
+def single_eddy(nx: int, nz: int, courant_max: float = 0.5, dt: float = 1.0):
+    """Per-cell velocities (grid units per second) of the single-eddy non-divergent flow of the paper's Fig. 2
+    set-up: stream function psi = -A sin(pi z / nz) cos(2 pi x / nx), u = -dpsi/dz, w = dpsi/dx at the cell centres,
+    scaled so that the largest Courant number |u| dt, |w| dt is `courant_max`.  Updraft on the left, downdraft on
+    the right.  Returns (u_cell, w_cell), each float64[nx * nz], row-major like cell_id."""
+    xc = (np.arange(nx) + 0.5) / nx
+    zc = (np.arange(nz) + 0.5) / nz
+    X, Z = np.meshgrid(xc, zc)                      # shape (nz, nx): row = z index
+    u = (math.pi / nz) * np.cos(math.pi * Z) * np.cos(2 * math.pi * X) * nz
+    w = (2 * math.pi / nx) * np.sin(math.pi * Z) * np.sin(2 * math.pi * X) * nx
+    scale = courant_max / (dt * max(np.abs(u).max(), np.abs(w).max()))
+    return (u * scale).ravel().copy(), (w * scale).ravel().copy()

@@ -906,6 +906,156 @@ def test_volume_spectrum_edges_and_degenerate_inputs(dev):
                 ctx.volume_spectrum(xi1, v1, bad)
 
 
+# ------------------------------------------------------------------------------------------- NEXT-3: efficiency table
+def _eff_table():
+    rng = np.random.default_rng(12)
+    radius = np.exp(np.linspace(np.log(2e-9), np.log(2e-3), 11))
+    table = rng.random((11, 6))
+    table[:, 0] *= 0.1
+    return radius, table
+
+
+@pytest.mark.parametrize("which", ["random", "constant"])
+def test_efficiency_table_kernel_bit_exact(dev, which):
+    """SDM_KERNEL_GEOMETRIC_TABLE (R39): K on the device == the oracle's, bit for bit, on volumes that cover the whole
+    radius grid, its outside, equal radii (p = 1) and a zero volume; a constant table == the geometric kernel."""
+    sdm = _sdm()
+    radius, table = _eff_table()
+    if which == "constant":
+        table = np.full_like(table, 0.625)
+    rng = np.random.default_rng(3)
+    n = 20_000
+    vj = np.exp(rng.uniform(np.log(1e-27), np.log(1e-6), n))
+    vk = np.exp(rng.uniform(np.log(1e-27), np.log(1e-6), n))
+    vk[:100] = vj[:100]
+    vj[100], vk[100] = 0.0, 1e-15
+    vj[101:111] = 4.0 / 3.0 * np.pi * radius[:10] ** 3           # on the grid nodes
+    okp = oracle.geometric_table(radius, table)
+    want = np.array([oracle.kernel(okp, float(a), float(b)) for a, b in zip(vj, vk)])
+    with sdm.SDMContext(1024, 1, device=dev) as ctx:
+        with pytest.raises(sdm.SDMError):                           # no table installed yet
+            ctx.kernel_eval(sdm.geometric_table(), torch.from_numpy(vj).to(dev), torch.from_numpy(vk).to(dev))
+        ctx.set_collision_efficiency(radius, table)
+        got = ctx.kernel_eval(sdm.geometric_table(), torch.from_numpy(vj).to(dev), torch.from_numpy(vk).to(dev)).cpu().numpy()
+        assert np.array_equal(got.view(np.int64), want.view(np.int64))
+        if which == "constant":
+            geo = ctx.kernel_eval(sdm.geometric(0.625), torch.from_numpy(vj).to(dev), torch.from_numpy(vk).to(dev)).cpu().numpy()
+            assert np.array_equal(got.view(np.int64), geo.view(np.int64))
+        for bad_r, bad_t in (([1.0, 1.0], [[0, 1], [0, 1]]), ([1.0, 2.0], [[0, -1], [0, 1]]), ([1.0], [[0.0, 1.0]])):
+            with pytest.raises(sdm.SDMError):
+                ctx.set_collision_efficiency(bad_r, bad_t)
+        ctx.set_collision_efficiency(None, None)
+        with pytest.raises(sdm.SDMError):
+            ctx.coalescence_step(torch.ones(4, dtype=torch.int64, device=dev), torch.ones(4, dtype=torch.float64, device=dev),
+                                 torch.zeros(4, dtype=torch.int32, device=dev), 1, 1.0, 1.0, sdm.geometric_table(), 42, 0)
+
+
+@pytest.mark.parametrize("path", ["general", "cell_sorted", "hybrid"])
+@pytest.mark.parametrize("dV", [400.0, 0.04])
+def test_efficiency_table_whole_steps(dev, path, dV):
+    """whole steps with a tabulated efficiency (entries from 0 to 1: the early-out bounds use the table's maximum),
+    p from << 1 to >> 1, debug outputs off, state bit for bit against the oracle"""
+    sdm = _sdm()
+    radius, table = _eff_table()
+    w = W.small("cfg3", interleave=(path == "hybrid"))
+    ow = w.copy()
+    okp = oracle.geometric_table(radius, table)
+    p = {"general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED, "hybrid": sdm.PATH_HYBRID}[path]
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        ctx.set_path(p)
+        ctx.set_collision_efficiency(radius, table)
+        xi, v, cell = _to_dev(w, dev)
+        for s in range(4):
+            oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, dV, okp, 42, s)
+            ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, dV, sdm.geometric_table(), 42, s)
+            assert ctx.poll_error() == 0
+            assert np.array_equal(xi.cpu().numpy(), ow.xi), f"step {s}"
+            assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v.view(np.int64)), f"step {s}"
+    assert not np.array_equal(ow.xi, w.xi)
+
+
+# ------------------------------------------------------------------------------------------- NEXT-4: displacement
+@pytest.mark.parametrize("n_off", [0, 1])
+def test_displacement_against_oracle(dev, n_off):
+    """sdm_displace / sdm_cell_id_from_positions vs the oracle (O8): positions and cell_id bit for bit over ten steps
+    of the paper's single-eddy flow, including positions on cell edges, at the periodic seam, and (n_off = 1) arrays
+    that are neither 16-byte aligned nor even in length."""
+    sdm = _sdm()
+    w = W.small("cfg3")
+    nx, nz = 19, 17
+    u, wv = W.single_eddy(nx, nz, courant_max=0.9)
+    x, z = W.positions_in_cells(w.cell_id, nx, nz)
+    x[:40] = np.arange(40) % nx                       # exactly on the edges
+    z[40:80] = np.arange(40) % nz
+    x[80:90] = np.nextafter(float(nx), 0.0)           # the last representable position before the seam
+    x[90:100] = 0.0
+    n = w.n_sd - 3 * n_off
+    ox, oz = x[:n].copy(), z[:n].copy()
+    ocell = oracle.cell_id_from_positions(ox, oz, nx, nz)
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        gx_all, gz_all = torch.from_numpy(x).to(dev), torch.from_numpy(z).to(dev)
+        gc_all = torch.zeros(w.n_sd + 1, dtype=torch.int32, device=dev)
+        gx, gz, gc = gx_all[n_off:n_off + n], gz_all[n_off:n_off + n], gc_all[n_off:n_off + n]
+        ox, oz = x[n_off:n_off + n].copy(), z[n_off:n_off + n].copy()
+        ocell = oracle.cell_id_from_positions(ox, oz, nx, nz)
+        gu, gw = torch.from_numpy(u).to(dev), torch.from_numpy(wv).to(dev)
+        ctx.cell_id_from_positions(gx, gz, nx, nz, cell_id=gc)
+        assert np.array_equal(gc.cpu().numpy(), ocell)
+        for step in range(10):
+            dt = 1.0 if step % 2 == 0 else 0.37
+            oracle.displace(ox, oz, ocell, nx, nz, u, wv, dt)
+            ctx.displace(gx, gz, gc, nx, nz, gu, gw, dt)
+            assert np.array_equal(gx.cpu().numpy().view(np.int64), ox.view(np.int64)), f"x step {step}"
+            assert np.array_equal(gz.cpu().numpy().view(np.int64), oz.view(np.int64)), f"z step {step}"
+            assert np.array_equal(gc.cpu().numpy(), ocell), f"cell_id step {step}"
+        assert ctx.poll_error() == 0
+        # the seam: a tiny negative coordinate folds to 0, a step of a whole period lands where it started
+        sx = torch.tensor([1e-300, 0.25, nx - 0.25, 0.0], dtype=torch.float64, device=dev)
+        sz = torch.tensor([0.5, 0.5, 0.5, 0.5], dtype=torch.float64, device=dev)
+        sc = torch.zeros(4, dtype=torch.int32, device=dev)
+        su = torch.full((nx * nz,), -2e-300, dtype=torch.float64, device=dev)
+        ctx.displace(sx, sz, sc, nx, nz, su, torch.zeros_like(su), 1.0)
+        hx, hz, hc = np.array([1e-300, 0.25, nx - 0.25, 0.0]), np.full(4, 0.5), np.zeros(4, np.int32)
+        oracle.displace(hx, hz, hc, nx, nz, np.full(nx * nz, -2e-300), np.zeros(nx * nz), 1.0)
+        assert sx.cpu().numpy().tolist() == hx.tolist() and hx[0] == 0.0 and hx[3] == 0.0
+        assert sc.cpu().numpy().tolist() == hc.tolist()
+        with pytest.raises(sdm.SDMError):
+            ctx.displace(sx, sz, sc, 0, nz, su, su, 1.0)
+        with pytest.raises(sdm.SDMError):
+            ctx.displace(sx, sz, sc, nx, nz, su, su, 0.0)
+
+
+def test_displacement_then_coalescence_time_loop(dev):
+    """The 2-D loop the displacement exists for: displace, then one coalescence step on the
+    cell_id it produced -- no longer sorted, so AUTO leaves the cell-sorted path -- for six steps against the oracle
+    doing the same; state, positions and cell_id bit for bit."""
+    sdm = _sdm()
+    w = W.small("cfg3")
+    ow = w.copy()
+    nx, nz = 19, 17
+    u, wv = W.single_eddy(nx, nz, courant_max=0.6)
+    x, z = W.positions_in_cells(w.cell_id, nx, nz)
+    ox, oz = x.copy(), z.copy()
+    okp, kp = _okp(w), _gkp(w)
+    paths = []
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev) as ctx:
+        xi, v, cell = _to_dev(w, dev)
+        gx, gz = torch.from_numpy(x).to(dev), torch.from_numpy(z).to(dev)
+        gu, gw = torch.from_numpy(u).to(dev), torch.from_numpy(wv).to(dev)
+        for s in range(6):
+            oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, okp, 42, s)
+            ctx.coalescence_step(xi, v, cell, w.n_cell, w.dt, w.dV, kp, 42, s)
+            paths.append(ctx.last_path())
+            oracle.displace(ox, oz, ow.cell_id, nx, nz, u, wv, w.dt)
+            ctx.displace(gx, gz, cell, nx, nz, gu, gw, w.dt)
+            assert ctx.poll_error() == 0
+            assert np.array_equal(cell.cpu().numpy(), ow.cell_id), f"cell_id step {s}"
+            assert np.array_equal(xi.cpu().numpy(), ow.xi), f"step {s}"
+            assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v.view(np.int64)), f"step {s}"
+    assert paths[0] == sdm.PATH_CELL_SORTED and sdm.PATH_CELL_SORTED not in paths[1:]
+    assert sdm.PATH_HYBRID in paths
+
+
 # ------------------------------------------------------------------------------------------- races / path equality
 @pytest.mark.parametrize("name", ["cfg3", "cfg4"])
 def test_full_size_paths_agree_and_repeat(dev, name):
