@@ -86,7 +86,8 @@ int sdm_set_collision_efficiency(sdm_ctx* ctx, const double* radius /* host */, 
  *                cell_id; legal when n_cell > 1 and no cell holds more than 256 super-droplets.
  *                An explicitly chosen CELL_SORTED or HYBRID verifies its precondition on the device BEFORE anything
  *                is updated: on a violation (the caller's error) the step is NOT applied and the sticky
- *                SDM_ERR_BAD_DATA flag is set.  Both stay fully asynchronous.
+ *                SDM_ERR_BAD_DATA flag is set.  Like AUTO they wait for the device's verdict on the cell sizes
+ *                (it fixes the launch geometry) without draining the stream.
  *   AUTO         (default) never refuses valid input.  Every step first analyses cell_id on the device (one
  *                streaming read: range, order, largest cell) and the host waits for that verdict -- a few
  *                microseconds, through a mapped status word, without draining work enqueued behind it -- before
@@ -208,7 +209,7 @@ int sdm_debug_outputs(sdm_ctx* ctx, int32_t* perm_out, int64_t* gamma_out, int64
 int sdm_set_path(sdm_ctx* ctx, int path);
 
 /* Test / tuning knobs.  SDM_OPT_NARROW_KEY_BITS: number of Philox-key bits (1..24, default 24) kept in the
- * 32-bit sort word of the fused per-cell kernel; fewer bits make its exact wide-word redo frequent (tests).
+ * 32-bit sort word of the fused per-cell kernel; fewer bits make its exact tie repair frequent (tests).
  * The result never depends on it.
  * SDM_OPT_TRACK_ZEROS (0 / 1, default 0): row a5 fused into row a4.  When 1, the fused per-cell kernel
  * (CELL_SORTED and HYBRID paths) also counts, exactly, the zero multiplicities the array holds after the
@@ -227,8 +228,12 @@ int sdm_set_path(sdm_ctx* ctx, int path);
  * order almost every neighbour; the runs that still tie are then put in exact (key, index) order by a
  * repair kernel, so the permutation -- and every result -- is the same for every value (tests force 3).
  * Automatic: sorted key bits = log2(n_sd / n_cell) + 8, rounded up to whole digits.
+ * SDM_OPT_FUSED_WORDS_PER_LANE (0 = automatic (default), 4, 8): sort words per lane of the fused per-cell
+ * kernel's group sort (a cell of at most 32 << k entries is sorted by (32 << k) / R lanes).  A tuning / test knob:
+ * every value gives the same bits; 4 cannot serve cells of more than 128 entries and then falls back to 8.
  * Returns INVALID_ARG for an unknown option or value. */
-enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1, SDM_OPT_INDEX_BASE = 2, SDM_OPT_SKIP_KEY_DIGITS = 3 };
+enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1, SDM_OPT_INDEX_BASE = 2, SDM_OPT_SKIP_KEY_DIGITS = 3,
+       SDM_OPT_FUSED_WORDS_PER_LANE = 4 };
 int sdm_set_option(sdm_ctx* ctx, int option, int64_t value);
 
 /* Which path the most recent step took (an sdm_path value other than AUTO), or 0 if none ran yet.  Host-side

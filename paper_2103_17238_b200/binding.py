@@ -23,6 +23,7 @@ OPT_NARROW_KEY_BITS = 0
 OPT_TRACK_ZEROS = 1
 OPT_INDEX_BASE = 2
 OPT_SKIP_KEY_DIGITS = 3
+OPT_FUSED_WORDS_PER_LANE = 4
 
 SDM_OK = 0
 

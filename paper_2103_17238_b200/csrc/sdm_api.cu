@@ -66,6 +66,7 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     w.cell_count = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 1) * 4));
     w.tile_state = reinterpret_cast<u32*>(take((size_t)MAX_PASSES * max_tiles * RADIX * 4));
     w.cell_start = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 2) * 4));
+    w.class_list = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 1) * 4));
     w.buf_a = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.buf_b = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.cmp_state = reinterpret_cast<u32*>(take(cmp_tiles * 4));
@@ -237,6 +238,10 @@ int sdm_set_option(sdm_ctx* ctx, int option, int64_t value) {
     }
     if (option == SDM_OPT_INDEX_BASE && value >= 0) {
         ctx->index_base = (u64)value;
+        return SDM_OK;
+    }
+    if (option == SDM_OPT_FUSED_WORDS_PER_LANE && (value == 0 || value == 4 || value == 8)) {
+        ctx->fused_r = (int)value;
         return SDM_OK;
     }
     if (option == SDM_OPT_TRACK_ZEROS && (value == 0 || value == 1)) {
@@ -420,18 +425,19 @@ struct FusedSource {
     int kind;
     const void* run_idx;
     int idxbits;
+    CellClasses cc;  // filled in by wait_verdict
 };
 
 // cell boundaries straight from cell_id (CELL_SORTED)
-int enqueue_sorted_prepare(sdm_ctx* ctx, const StepArgs& A, int rmax, bool strict, FusedSource* src) {
+int enqueue_sorted_prepare(sdm_ctx* ctx, const StepArgs& A, bool strict, FusedSource* src) {
     int rc;
     if ((rc = next_epoch(ctx))) return rc;
     src->kind = 0; src->run_idx = nullptr; src->idxbits = 0;
-    return note_cuda(ctx, launch_cell_bounds(ctx, 0, A.cell_id, A.n_sd, A.n_cell, 0, rmax, strict));
+    return note_cuda(ctx, launch_cell_bounds(ctx, 0, A.cell_id, A.n_sd, A.n_cell, 0, strict));
 }
 
 // cell-digit LSD passes + cell boundaries of the grouped words (HYBRID)
-int enqueue_hybrid_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, int rmax, bool strict, FusedSource* src) {
+int enqueue_hybrid_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, bool strict, FusedSource* src) {
     int rc;
     cudaStream_t st = ctx->stream;
     Workspace& ws = ctx->ws;
@@ -453,16 +459,16 @@ int enqueue_hybrid_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, in
     src->kind = narrow ? 2 : 1;
     src->run_idx = in;
     src->idxbits = plan.idxbits;
-    return note_cuda(ctx, launch_cell_bounds(ctx, src->kind, in, A.n_sd, A.n_cell, plan.idxbits, rmax, strict));
+    return note_cuda(ctx, launch_cell_bounds(ctx, src->kind, in, A.n_sd, A.n_cell, plan.idxbits, strict));
 }
 
-int enqueue_fused_step(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, int rmax, uint64_t step,
+int enqueue_fused_step(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, uint64_t step,
                        const StepLinks& links, bool bump_epoch) {
     int rc;
     if ((rc = clear_debug_gammas(ctx, A.n_sd))) return rc;
     if (bump_epoch && (rc = next_epoch(ctx))) return rc;
     const PhiloxKeys pk = make_philox_keys(A.seed, step, ctx->index_base);
-    if ((rc = note_cuda(ctx, launch_cell_fused(ctx, src.kind, src.run_idx, src.idxbits, rmax, A.xi, A.v, A.n_sd,
+    if ((rc = note_cuda(ctx, launch_cell_fused(ctx, src.kind, src.run_idx, src.idxbits, src.cc, A.xi, A.v, A.n_sd,
                                                A.n_cell, A.dtdV, A.dkp, pk, links))))
         return rc;
     ctx->last_path = src.kind == 0 ? SDM_PATH_CELL_SORTED : SDM_PATH_HYBRID;
@@ -470,8 +476,10 @@ int enqueue_fused_step(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, 
 }
 
 // Waits, WITHOUT draining the stream behind it, until k_cell_bounds of `epoch` has published its verdict in the
-// mapped status block; *cls = worst cell-size class (3 = the fused kernel cannot take this input).
-int wait_verdict(sdm_ctx* ctx, u32 epoch, u32* cls) {
+// mapped status block: the worst cell-size class (CELL_CLASSES = the fused kernel cannot take this input) and the
+// number of cells per class.  Cells of nearly one size are all served as the worst class (no indirection); mixed
+// sizes are grouped by class first (k_class_lists, enqueued here).
+int wait_verdict(sdm_ctx* ctx, u32 epoch, int32_t n_cell, CellClasses* cc) {
     volatile u32* m = ctx->mapped;
     for (unsigned long spin = 1;; ++spin) {
         if (m[MAPPED_VERDICT_EPOCH] == epoch) break;
@@ -484,11 +492,21 @@ int wait_verdict(sdm_ctx* ctx, u32 epoch, u32* cls) {
         }
     }
     std::atomic_thread_fence(std::memory_order_acquire);
-    *cls = m[MAPPED_VERDICT_CLASS];
-    return SDM_OK;
+    cc->worst = m[MAPPED_VERDICT_CLASS];
+    cc->mixed = false;
+    for (int k = 0; k < CELL_CLASSES; ++k) cc->count[k] = 0;
+    if (cc->worst >= (u32)CELL_CLASSES) return SDM_OK;
+    u32 upper = 0;
+    for (int k = 1; k < CELL_CLASSES; ++k) upper += (cc->count[k] = m[MAPPED_CLASS_COUNT + k - 1]);
+    if (upper > (u32)n_cell) return note_cuda(ctx, cudaErrorUnknown);  // cannot happen: every cell is closed once
+    cc->count[0] = (u32)n_cell - upper;
+    if ((uint64_t)cc->count[cc->worst] * 4u >= (uint64_t)n_cell * 3u) {
+        for (int k = 0; k < CELL_CLASSES; ++k) cc->count[k] = (u32)k == cc->worst ? (u32)n_cell : 0u;
+        return SDM_OK;
+    }
+    cc->mixed = true;
+    return note_cuda(ctx, launch_class_lists(ctx, n_cell, cc->count));
 }
-
-int rmax_of_class(u32 cls) { return cls == 0 ? 2 : (cls == 1 ? 4 : 8); }
 
 // AUTO's hint: what the last GENERAL step on this very (cell_id pointer, n_sd, n_cell) saw.  Waits for its
 // asynchronous copy (AUTO waits for the analysis enqueued behind it anyway).  Returns false when there is none.
@@ -503,25 +521,32 @@ bool auto_hint(sdm_ctx* ctx, const StepArgs& A, Verdict* hint) {
 
 // AUTO: analyses cell_id on the device, waits for the verdict and prepares the fused kernel's input when it fits.
 // *fits = false: take the GENERAL path (nothing was updated).  The analysis never raises SDM_ERR_BAD_DATA by itself.
-int auto_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, bool* fits, FusedSource* src, int* rmax) {
+int auto_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, bool* fits, FusedSource* src) {
     *fits = false;
     if (A.n_cell <= 1) return SDM_OK;
     Verdict hint;
     const bool have_hint = auto_hint(ctx, A, &hint);
     if (have_hint && hint.max_count > (u32)CELL_FAST_MAX) return SDM_OK;
     int rc;
-    u32 cls = 3;
+    src->cc.worst = (u32)CELL_CLASSES;
     if (!have_hint || !hint.unsorted) {
-        if ((rc = enqueue_sorted_prepare(ctx, A, CELL_FAST_MAX / 32, false, src))) return rc;
-        if ((rc = wait_verdict(ctx, ctx->epoch, &cls))) return rc;
+        if ((rc = enqueue_sorted_prepare(ctx, A, false, src))) return rc;
+        if ((rc = wait_verdict(ctx, ctx->epoch, A.n_cell, &src->cc))) return rc;
     } else if (hybrid_fits(plan)) {
-        if ((rc = enqueue_hybrid_prepare(ctx, A, plan, CELL_FAST_MAX / 32, false, src))) return rc;
-        if ((rc = wait_verdict(ctx, ctx->epoch, &cls))) return rc;
+        if ((rc = enqueue_hybrid_prepare(ctx, A, plan, false, src))) return rc;
+        if ((rc = wait_verdict(ctx, ctx->epoch, A.n_cell, &src->cc))) return rc;
     }
-    if (cls <= 2) {
-        *fits = true;
-        *rmax = rmax_of_class(cls);
-    }
+    *fits = src->cc.worst < (u32)CELL_CLASSES;
+    return SDM_OK;
+}
+
+// An explicitly chosen CELL_SORTED / HYBRID path: the same analysis, but an input that does not fit is the caller's
+// error -- k_cell_bounds (strict) has then raised the sticky SDM_ERR_BAD_DATA and nothing is updated.
+int explicit_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, bool hybrid, bool* fits, FusedSource* src) {
+    int rc;
+    if ((rc = hybrid ? enqueue_hybrid_prepare(ctx, A, plan, true, src) : enqueue_sorted_prepare(ctx, A, true, src))) return rc;
+    if ((rc = wait_verdict(ctx, ctx->epoch, A.n_cell, &src->cc))) return rc;
+    *fits = src->cc.worst < (u32)CELL_CLASSES;
     return SDM_OK;
 }
 
@@ -548,19 +573,18 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
     ctx->zero_hint_valid = 0;
     // ---- path selection (include/sdm.h, sdm_path) ----
     FusedSource src;
-    int rmax = CELL_FAST_MAX / 32;
     bool fused = false;
-    if (n_cell > 1 && ctx->path == SDM_PATH_CELL_SORTED) {
-        if ((rc = enqueue_sorted_prepare(ctx, A, rmax, true, &src))) return rc;
-        fused = true;
-    } else if (n_cell > 1 && ctx->path == SDM_PATH_HYBRID && hybrid_fits(plan)) {
-        if ((rc = enqueue_hybrid_prepare(ctx, A, plan, rmax, true, &src))) return rc;
-        fused = true;
+    if (n_cell > 1 && (ctx->path == SDM_PATH_CELL_SORTED || (ctx->path == SDM_PATH_HYBRID && hybrid_fits(plan)))) {
+        if ((rc = explicit_prepare(ctx, A, plan, ctx->path == SDM_PATH_HYBRID, &fused, &src))) return rc;
+        if (!fused) {  // refused: the step is skipped as a whole, the sticky flag reports it
+            ctx->last_path = ctx->path;
+            return SDM_OK;
+        }
     } else if (ctx->path == SDM_PATH_AUTO) {
-        if ((rc = auto_prepare(ctx, A, plan, &fused, &src, &rmax))) return rc;
+        if ((rc = auto_prepare(ctx, A, plan, &fused, &src))) return rc;
     }
     if (!fused) return enqueue_general_step(ctx, A, step);
-    if ((rc = enqueue_fused_step(ctx, A, src, rmax, step, no_links, false))) return rc;
+    if ((rc = enqueue_fused_step(ctx, A, src, step, no_links, false))) return rc;
     note_zero_hint(ctx, multiplicity, n_sd);
     return SDM_OK;
 }
@@ -651,7 +675,7 @@ int finish_run(sdm_ctx* ctx) {
 // enqueued exit without touching the state, and the host -- which watches the mapped halt word from one chunk
 // behind -- compacts and resumes from the halted step.  Returns with *s = first step not yet applied,
 // *halt_zeros > 0 when a compaction of that many zeros is due before step *s (stream drained), else 0.
-int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, int rmax, uint64_t step0, int64_t* s,
+int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, uint64_t step0, int64_t* s,
                     int64_t n_steps, int64_t compact_every, int64_t* halt_zeros) {
     int rc;
     cudaStream_t st = ctx->stream;
@@ -672,7 +696,7 @@ int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, int
             const bool due_before = compact_every > 0 && enq > s_begin && (enq % compact_every) == 0;
             links.zc_check = due_before ? run + RUN_ZC0 + ((enq - 1) % 3) : nullptr;
             links.halt_tag = (u32)(enq - s_begin) + 1u;
-            if ((rc = enqueue_fused_step(ctx, A, src, rmax, step0 + (uint64_t)enq, links, true))) return rc;
+            if ((rc = enqueue_fused_step(ctx, A, src, step0 + (uint64_t)enq, links, true))) return rc;
         }
         if ((rc = note_cuda(ctx, cudaEventRecord(ctx->chunk_event[n_chunks & 1], st)))) return rc;
         ++n_chunks;
@@ -720,34 +744,27 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
         const Plan plan = make_plan(n, n_cell, ctx->skip_key_digits);
         if (!plan_fits(plan)) return SDM_ERR_CAPACITY;
         FusedSource src;
-        int rmax = CELL_FAST_MAX / 32;
         bool fused = false;
         if (!general_only) {
             if (ctx->path == SDM_PATH_AUTO) {
-                if ((rc = auto_prepare(ctx, A, plan, &fused, &src, &rmax))) return rc;
+                if ((rc = auto_prepare(ctx, A, plan, &fused, &src))) return rc;
             } else {  // explicit CELL_SORTED / HYBRID: an input that does not fit is the caller's error
                 const bool hybrid = ctx->path == SDM_PATH_HYBRID;
                 if (hybrid && !hybrid_fits(plan)) {
                     general_only = true;
                     continue;
                 }
-                if ((rc = hybrid ? enqueue_hybrid_prepare(ctx, A, plan, rmax, true, &src)
-                                 : enqueue_sorted_prepare(ctx, A, rmax, true, &src)))
-                    return rc;
-                u32 cls = 3;
-                if ((rc = wait_verdict(ctx, ctx->epoch, &cls))) return rc;
-                if (cls > 2) {
+                if ((rc = explicit_prepare(ctx, A, plan, hybrid, &fused, &src))) return rc;
+                if (!fused) {
                     *n_sd_out = n;
                     rc = finish_run(ctx);
                     return rc != SDM_OK ? rc : SDM_ERR_BAD_DATA;
                 }
-                rmax = rmax_of_class(cls);
-                fused = true;
             }
         }
         int64_t zeros = 0;
         if (fused) {
-            if ((rc = run_fused_steps(ctx, A, src, rmax, step0, &s, n_steps, compact_every, &zeros))) return rc;
+            if ((rc = run_fused_steps(ctx, A, src, step0, &s, n_steps, compact_every, &zeros))) return rc;
             if (zeros > 0) {
                 if ((rc = enqueue_compact(ctx, multiplicity, volume, cell_id, n))) return rc;
                 n -= zeros;

@@ -2,40 +2,41 @@
 // SURVEY 8(f) NEXT-1).  Once the super-droplets of a cell are known as one contiguous run -- either
 // because cell_id itself is non-decreasing (CELL_SORTED path: the run is a slice of the arrays) or
 // because an LSD radix sort on the cell_id digits alone has grouped their indices (HYBRID path: the
-// run is a slice of the sorted index array) -- the order inside the cell is produced by ONE WARP that
-// sorts the cell's (Philox key, position in the run) words in registers and then applies the pair
-// rule to neighbours.  The total order is (cell, key, index), exactly what the global LSD sort of
-// (cell_id << 32 | key) and the oracle's std::stable_sort produce, so the output is bit-identical,
-// at 36-48 B/SD of HBM traffic instead of 148.
+// run is a slice of the sorted index array) -- the order inside the cell is produced by a GROUP OF G
+// LANES that sorts the cell's (Philox key, position in the run) words in registers, R words per lane,
+// and then applies the pair rule to neighbours.  The total order is (cell, key, index), exactly what
+// the global LSD sort of (cell_id << 32 | key) and the oracle's std::stable_sort produce, so the output
+// is bit-identical, at 32-48 B/SD of HBM traffic instead of 148.
 //
-//   k_cell_bounds<SRC>  reads the cell of every position once: verifies range and order, finds the largest
-//                       cell's size class, writes cell_start[0..n_cell] and publishes the verdict (device flag
-//                       for the fused kernel, mapped host word for AUTO's path choice).  When the input does
-//                       not fit the fused kernel launched next, that kernel does nothing (the state is never
-//                       half-updated).
-//   k_cell_fused<W>     one warp per cell, n_c <= 32 R, R in {1,2,4,8}.  Sort word = 32 bits:
-//                       (top 24 bits of the Philox key) << 8 | position-in-run, sorted by an
-//                       all-ascending bitonic network (IMNMX + SHFL, 2 instructions per compare).
-//                       Dropping the low 8 key bits is exact unless two neighbours of the sorted run
-//                       share their top 24 bits (4.8e-4 per 128-SD cell); the warp detects that and
-//                       redoes its cell with full 64-bit (key << 32 | position) words.
+//   k_cell_bounds<SRC>  reads the cell of every position once: verifies range and order, writes
+//                       cell_start[0..n_cell], counts the cells per size class (<= 32, 64, 128, 256 entries)
+//                       and publishes the verdict (device flag for the fused kernel, mapped host words for
+//                       the path choice and the launch geometry).  When the input does not fit the fused
+//                       kernel launched next, that kernel does nothing (the state is never half-updated).
+//   k_class_lists       mixed cell sizes only: the cell ids grouped by size class, so that every warp of the
+//                       fused kernel works on cells of one class.
+//   k_cell_fused<R>     size class k = cells of at most P = 32 << k entries, sorted by G = P / R lanes holding
+//                       R words each; a warp takes 32 / G cells.  With R = 8 a cell of 128 runs 18 of the 28
+//                       bitonic stages inside the lanes (1 instruction per element) and 10 across lanes
+//                       (SHFL + 2 VIMNMX per element); R = 16 (22 + 6) executes 12 % fewer instructions still but
+//                       its straight-line code no longer streams through the instruction caches (30 % of the
+//                       stall samples "no instruction": profiles/r2b_README.md), so it is not built.
+//                       Sort word = 32 bits: (top 24 bits of the Philox key)
+//                       << 8 | position-in-run.  Dropping the low 8 key bits is exact unless two neighbours
+//                       of the sorted run share their top 24 bits (4.8e-4 per 128-SD cell); the group detects
+//                       that and orders such runs by the regenerated full key.
 #include "sdm_internal.h"
 #include "sdm_pair.cuh"
 
 namespace sdm {
 
-#ifndef SDM_CF_WARPS
-#define SDM_CF_WARPS 4
-#endif
-#ifndef SDM_CF_MIN_BLOCKS
-#define SDM_CF_MIN_BLOCKS 9
-#endif
-constexpr int CF_WARPS = SDM_CF_WARPS;  // tuning constants (profiles/): -DSDM_CF_WARPS / -DSDM_CF_MIN_BLOCKS via SDM_NVCC_EXTRA
+constexpr int CF_WARPS = 4;       // measured on B200 (profiles/r2b_README.md): 2 warps per block 15 % slower
+constexpr int CF_MIN_BLOCKS = 9;  // 56 registers; 8 (64 registers) and 7 measured the same on configs[3]
 constexpr int CF_BLOCK = CF_WARPS * 32;
-constexpr int CF_MIN_BLOCKS = SDM_CF_MIN_BLOCKS;
 constexpr int CB_BLOCK = 256;
 constexpr int CB_K = 4;                         // quads (4 positions, one 16-byte load for int32 sources) per thread and iteration
 constexpr int CB_CHUNK = CB_BLOCK * CB_K * 4;   // positions per block and iteration
+constexpr u32 CLASS_REFUSED = (u32)CELL_CLASSES;  // a cell of more than 256 entries, or unsorted / out-of-range input
 
 // ---------------------------------------------------------------------------------------------
 // Cell boundaries of an array whose cells are contiguous.  SRC = 0: cell_id int32[n];
@@ -74,8 +75,8 @@ __device__ __forceinline__ void cells_at4(const void* src, u32 i0, u32 n_sd, int
 
 // Position i opens cell cc and closes cell prev (opening every empty cell in between).  The closed cell
 // [s, i) holds more than m entries exactly when position i - 1 - m still belongs to it (sorted input), so its
-// size class costs up to three extra loads per cell, not per super-droplet.  Returns the size class of the
-// closed cell: 0 (<= 64), 1 (<= 128), 2 (<= 256), 3 (larger).
+// size class costs up to four extra loads per cell, not per super-droplet.  Returns the size class of the
+// closed cell: 0 (<= 32 entries), 1 (<= 64), 2 (<= 128), 3 (<= 256), 4 (larger).
 template <int SRC>
 __device__ __forceinline__ u32 open_cells(const void* src, int idxbits, int prev, int cc, u32 i,
                                           u32* __restrict__ cell_start, int32_t* __restrict__ dbg_cell_start) {
@@ -85,29 +86,41 @@ __device__ __forceinline__ u32 open_cells(const void* src, int idxbits, int prev
     }
     if (prev < 0) return 0;
     u32 cls = 0;
-    if (i > 64u && cell_at<SRC>(src, i - 65u, idxbits) == prev) {
-        cls = 1;
-        if (i > 128u && cell_at<SRC>(src, i - 129u, idxbits) == prev) {
-            cls = 2;
-            if (i > 256u && cell_at<SRC>(src, i - 257u, idxbits) == prev) cls = 3;
-        }
+#pragma unroll
+    for (u32 m = 32; m <= 256; m <<= 1) {
+        if (i > m && cell_at<SRC>(src, i - 1u - m, idxbits) == prev) ++cls;
+        else break;
     }
     return cls;
 }
 
 template <int SRC, bool VEC>
 __global__ void __launch_bounds__(CB_BLOCK)
-k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32 max_class, u32 strict, u32 epoch,
+k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32 strict, u32 epoch,
               u32* __restrict__ cell_start, u32* __restrict__ ctl, u32* __restrict__ sticky, u32* __restrict__ run,
               volatile u32* __restrict__ mapped, int32_t* __restrict__ dbg_cell_start) {
     __shared__ u32 s_cls;
+    __shared__ u32 s_cnt[CELL_CLASSES];
     // the fused kernel that follows accumulates the zero count; no separate memset of the control block
     if (blockIdx.x == 0 && threadIdx.x == 0) ctl[CTL_ZERO_COUNT] = 0u;
     if (threadIdx.x == 0) s_cls = 0u;
+    if (threadIdx.x < CELL_CLASSES) s_cnt[threadIdx.x] = 0u;
     const int lane = threadIdx.x & 31;
     bool bad = false;
     u32 cls = 0;
+    u32 cnt = 0;  // closed cells per class, one byte each for the classes 1..3 of this thread (< 256 cells per thread)
     const u32 n_chunks = (n_sd + CB_CHUNK - 1) / CB_CHUNK;
+    auto note = [&](u32 k) {  // a closed cell of class k
+        cls = max(cls, k);
+        if (k >= 1u && k < CLASS_REFUSED) {
+            if (((cnt >> (8u * (k - 1u))) & 0xFFu) == 0xFFu) {  // flush a full byte counter
+                atomicAdd(&s_cnt[k], 0xFFu);
+                cnt -= 0xFFu << (8u * (k - 1u));
+            }
+            cnt += 1u << (8u * (k - 1u));
+        }
+    };
+    __syncthreads();
     for (u32 ch = blockIdx.x; ch < n_chunks; ch += gridDim.x) {
         const u32 base = ch * (u32)CB_CHUNK;
         int c[CB_K][4];
@@ -141,8 +154,7 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
                     p = prev;
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
-                        if (c[k][j] != p)
-                            cls = max(cls, open_cells<SRC>(src, idxbits, p, c[k][j], i0 + j, cell_start, dbg_cell_start));
+                        if (c[k][j] != p) note(open_cells<SRC>(src, idxbits, p, c[k][j], i0 + j, cell_start, dbg_cell_start));
                         p = c[k][j];
                     }
                 }
@@ -156,10 +168,9 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
                         if (cc < 0 || cc >= n_cell || cc < prev) {
                             bad = true;
                         } else {
-                            if (cc != prev)
-                                cls = max(cls, open_cells<SRC>(src, idxbits, prev, cc, i, cell_start, dbg_cell_start));
+                            if (cc != prev) note(open_cells<SRC>(src, idxbits, prev, cc, i, cell_start, dbg_cell_start));
                             if (i == n_sd - 1)  // the array end closes cell cc and opens the (empty) rest
-                                cls = max(cls, open_cells<SRC>(src, idxbits, cc, n_cell, n_sd, cell_start, dbg_cell_start));
+                                note(open_cells<SRC>(src, idxbits, cc, n_cell, n_sd, cell_start, dbg_cell_start));
                         }
                         prev = cc;
                     }
@@ -167,24 +178,31 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
             }
         }
     }
-    if (bad) cls = 3;  // out of range or out of order: refused like a cell that is too large
+    if (bad) cls = CLASS_REFUSED;  // out of range or out of order: refused like a cell that is too large
     cls = __reduce_max_sync(0xffffffffu, cls);
-    __syncthreads();
     if (lane == 0 && cls) atomicMax(&s_cls, cls);
+#pragma unroll
+    for (u32 k = 1; k < CLASS_REFUSED; ++k) {
+        const u32 n = __reduce_add_sync(0xffffffffu, (cnt >> (8u * (k - 1u))) & 0xFFu);
+        if (lane == 0 && n) atomicAdd(&s_cnt[k], n);
+    }
     __syncthreads();
     if (threadIdx.x == 0) {
         if (s_cls) atomicMax(&run[RUN_BOUNDS_CLASS], s_cls);
+        for (u32 k = 1; k < CLASS_REFUSED; ++k)
+            if (s_cnt[k]) atomicAdd(&run[RUN_CLASS_COUNT + k - 1], s_cnt[k]);
         __threadfence();
         const u32 t = atomicAdd(&run[RUN_BOUNDS_TICKET], 1u);
-        if (t == gridDim.x - 1) {  // the last block: every other block's class is visible (fence + ticket)
+        if (t == gridDim.x - 1) {  // the last block: every other block's class and counts are visible (fence + ticket)
             __threadfence();
             const u32 worst = atomicExch(&run[RUN_BOUNDS_CLASS], 0u);
             run[RUN_BOUNDS_TICKET] = 0u;
-            const bool refuse = worst > max_class;
-            if (refuse) {  // the step is skipped as a whole and reported
+            if (worst >= CLASS_REFUSED) {  // the step is skipped as a whole and reported
                 ctl[CTL_UNSORTED] = epoch;  // tagged with this step's epoch: stale refusals never match
                 if (strict) sticky[STICKY_BAD_DATA] = 1u;
             }
+            for (u32 k = 1; k < CLASS_REFUSED; ++k) mapped[MAPPED_CLASS_COUNT + k - 1] = atomicExch(&run[RUN_CLASS_COUNT + k - 1], 0u);
+            for (u32 k = 0; k < CLASS_REFUSED; ++k) run[RUN_LIST_CURSOR + k] = 0u;
             mapped[MAPPED_VERDICT_CLASS] = worst;
             __threadfence_system();
             mapped[MAPPED_VERDICT_EPOCH] = epoch;
@@ -192,10 +210,49 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
     }
 }
 
+// Cell ids grouped by size class: list[off[k] ...] holds the cells of class k (cells of fewer than two entries go to
+// class 0: the fused kernel still counts a lone zero multiplicity).  off[] is the exclusive prefix of the class
+// counts k_cell_bounds published; the order inside a class is the (nearly ascending) order in which the warps
+// draw their slots -- cells are independent, so the result does not depend on it.
+struct ClassOffsets { u32 off[CELL_CLASSES]; };
+
+__global__ void __launch_bounds__(256)
+k_class_lists(const u32* __restrict__ cell_start, int n_cell, const ClassOffsets o, u32* __restrict__ cursor,
+              u32* __restrict__ list) {
+    const int c = blockIdx.x * 256 + threadIdx.x;
+    const bool valid = c < n_cell;
+    u32 cls = 0xFFu;
+    if (valid) {
+        const u32 n = __ldg(cell_start + c + 1) - __ldg(cell_start + c);
+        cls = n <= 32u ? 0u : (n <= 64u ? 1u : (n <= 128u ? 2u : 3u));
+    }
+    const u32 lt = lanemask_lt();
+#pragma unroll
+    for (u32 k = 0; k < (u32)CELL_CLASSES; ++k) {
+        const u32 m = __ballot_sync(0xffffffffu, cls == k);
+        if (m == 0u) continue;
+        u32 base = 0;
+        if ((threadIdx.x & 31) == __ffs(m) - 1) base = atomicAdd(&cursor[k], (u32)__popc(m));
+        base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+        if (cls == k) list[o.off[k] + base + __popc(m & lt)] = (u32)c;
+    }
+}
+
+cudaError_t launch_class_lists(sdm_ctx* ctx, int32_t n_cell, const u32 (&count)[CELL_CLASSES]) {
+    ClassOffsets o;
+    u32 run = 0;
+    for (int k = 0; k < CELL_CLASSES; ++k) { o.off[k] = run; run += count[k]; }
+    LaunchScope scope(ctx, PROF_CELL_BOUNDS);
+    k_class_lists<<<(n_cell + 255) / 256, 256, 0, ctx->stream>>>(ctx->ws.cell_start, n_cell, o, ctx->ws.run + RUN_LIST_CURSOR,
+                                                                 ctx->ws.class_list);
+    return cudaGetLastError();
+}
+
 // ---------------------------------------------------------------------------------------------
-// Bitonic sort of 32*R words held R per lane, element e = lane*R + r (blocked), ascending.
-// All-ascending formulation: merge of size k = one "flip" stage (partner e ^ (k-1)) followed by
-// half-cleaners (partner e ^ j, j = k/4 .. 1); the lower position always keeps the minimum.
+// Bitonic sort of G*R words held R per lane by a group of G lanes (lg = lane within the group), element
+// slot = lg*R + r (blocked), ascending.  All-ascending formulation: merge of size k = one "flip" stage
+// (partner slot ^ (k-1)) followed by half-cleaners (partner slot ^ j, j = k/4 .. 1); the lower slot always
+// keeps the minimum.
 // ---------------------------------------------------------------------------------------------
 template <typename T>
 __device__ __forceinline__ void cmpx_asc(T& a, T& b) {
@@ -205,14 +262,9 @@ __device__ __forceinline__ void cmpx_asc(T& a, T& b) {
     b = hi;
 }
 
-template <typename T>
-__device__ __forceinline__ T shfl_xor_any(T x, int m) {
-    return __shfl_xor_sync(0xffffffffu, x, m);
-}
-
-template <typename T, int R>
-__device__ __forceinline__ void warp_bitonic_sort(T (&x)[R], int lane) {
-    constexpr int N = 32 * R;
+template <int R, int G>
+__device__ __forceinline__ void group_bitonic_sort(u32 (&x)[R], int lg) {
+    constexpr int N = G * R;
 #pragma unroll
     for (int k = 2; k <= N; k <<= 1) {
         if (k <= R) {  // flip inside the lane
@@ -221,14 +273,14 @@ __device__ __forceinline__ void warp_bitonic_sort(T (&x)[R], int lane) {
                 if ((r & (k >> 1)) == 0) cmpx_asc(x[r], x[r ^ (k - 1)]);
         } else {  // flip across lanes: lane ^ (k/R - 1), register R-1-r
             const int lm = k / R - 1;
-            const bool lower = (lane & (k / (2 * R))) == 0;
-            T y[R];
+            const bool lower = (lg & (k / (2 * R))) == 0;
+            u32 y[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) y[r] = shfl_xor_any(x[R - 1 - r], lm);
+            for (int r = 0; r < R; ++r) y[r] = __shfl_xor_sync(0xffffffffu, x[R - 1 - r], lm);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const T mn = x[r] < y[r] ? x[r] : y[r];
-                const T mx = x[r] < y[r] ? y[r] : x[r];
+                const u32 mn = min(x[r], y[r]);
+                const u32 mx = max(x[r], y[r]);
                 x[r] = lower ? mn : mx;
             }
         }
@@ -236,12 +288,12 @@ __device__ __forceinline__ void warp_bitonic_sort(T (&x)[R], int lane) {
         for (int j = k >> 2; j > 0; j >>= 1) {
             if (j >= R) {
                 const int lj = j / R;
-                const bool lower = (lane & lj) == 0;
+                const bool lower = (lg & lj) == 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const T y = shfl_xor_any(x[r], lj);
-                    const T mn = x[r] < y ? x[r] : y;
-                    const T mx = x[r] < y ? y : x[r];
+                    const u32 y = __shfl_xor_sync(0xffffffffu, x[r], lj);
+                    const u32 mn = min(x[r], y);
+                    const u32 mx = max(x[r], y);
                     x[r] = lower ? mn : mx;
                 }
             } else {
@@ -256,13 +308,18 @@ __device__ __forceinline__ void warp_bitonic_sort(T (&x)[R], int lane) {
 struct FusedArgs {
     PairArgs pair;
     int n_cell;
-    int key_bits;         // key bits kept in the 32-bit sort word (24; tests lower it to force the wide redo)
+    int key_bits;         // key bits kept in the 32-bit sort word (24; tests lower it to force the tie repair)
     const void* run_idx;  // HYBRID: sorted words whose low idxbits are the original index; else nullptr
+    int run_u32;          // HYBRID: the words are 32 bits wide
     u64 idx_mask;
     int32_t* dbg_perm;
     u32* sticky;
     u32* ctl;
     u32 epoch;  // ctl[CTL_UNSORTED] == epoch: k_cell_bounds refused this step's input
+    // the cells by size class: class k is served by blocks [class_block_end[k-1], class_block_end[k])
+    const u32* class_cells[CELL_CLASSES];  // cell ids of the class; nullptr = the cells 0 .. class_count - 1 themselves
+    u32 class_count[CELL_CLASSES];
+    u32 class_block_end[CELL_CLASSES];
     // zero bookkeeping (row a5 fused into a4) and the halt protocol of sdm_coalescence_steps (see sdm_api.cu):
     u32* zc_accum;        // += zero multiplicities the array holds after this step
     const u32* zc_check;  // non-null: the previous step's count, after which a compaction was due -- if it is not 0
@@ -275,22 +332,20 @@ struct FusedArgs {
 };
 
 // Original array index of position e of the run that starts at `start`.
-template <int WORD>
+template <int HYB>
 __device__ __forceinline__ u32 run_index(const FusedArgs& a, u32 start, u32 e) {
-    if (WORD == 0) return start + e;
-    if (WORD == 1) return (u32)(__ldg(reinterpret_cast<const u64*>(a.run_idx) + start + e) & a.idx_mask);
-    return __ldg(reinterpret_cast<const u32*>(a.run_idx) + start + e) & (u32)a.idx_mask;
+    if (HYB == 0) return start + e;
+    if (a.run_u32) return __ldg(reinterpret_cast<const u32*>(a.run_idx) + start + e) & (u32)a.idx_mask;
+    return (u32)(__ldg(reinterpret_cast<const u64*>(a.run_idx) + start + e) & a.idx_mask);
 }
 
-// Per-warp staging of one cell in shared memory, indexed by the position e in the run: the attributes
-// are loaded ONCE, coalesced, before the (ALU-bound) key generation and sort, so the HBM latency hides
-// under them; the pair phase then reads its two members by sorted position from shared memory.
-// Two 16-byte stores per super-droplet: the exact attributes, and the fp32 side values of the cheap early-out.
-template <int WORD, int RMAX>
-struct CellStage {
-    longlong2 xv[32 * RMAX];  // (multiplicity, volume bits)
-    float4 aux[32 * RMAX];    // {xi rounded UP to fp32, v rounded UP to fp32, Philox word 3 (bits), Philox key (bits)}
-    u32 idx[WORD == 0 ? 1 : 32 * RMAX];  // HYBRID: original index
+// Per-warp staging of the fp32 side values of the first-level pair test, indexed by cell-in-warp * P + position
+// in the run: written once per super-droplet right after the (coalesced) attribute load, read by sorted position.
+// The exact attributes are NOT staged: the few pairs that pass the first level read them again (L1 / L2 hits).
+template <int R>
+struct WarpStage {
+    float2 fl[32 * R];  // (multiplicity rounded UP to fp32, volume rounded UP to fp32)
+    u32 w3[32 * R];     // Philox word 3 of the super-droplet (the high word of its uniform)
 };
 
 template <int R>
@@ -302,149 +357,188 @@ __device__ __forceinline__ u32 select_reg(const u32 (&x)[R], int i) {
     return v;
 }
 
-// One warp, one cell of 2 <= n_c <= 32 R super-droplets.  Returns this lane's share of the number of zero
-// multiplicities the cell holds AFTER the step.  The hot flow is straight-line code: loads, Philox blocks (computed
-// for padding slots too, so the R chains interleave), sort and the first-level pair test are predicated, not branched.
-// FULL: n_c == 32 R (every slot holds a super-droplet: no padding, no guards); the caller branches warp-uniformly.
-template <int WORD, int RMAX, int R, int KIND, bool FULL>
-__device__ __forceinline__ u32 warp_cell(const FusedArgs& a, CellStage<WORD, RMAX>& st, u32 start, u32 n_c_in, int lane) {
-    static_assert(R <= RMAX, "register tile within the staging tile");
-    const u32 n_c = FULL ? 32u * R : n_c_in;
+// The full Philox permutation key of position e of a run (the rare tie repair only; kept out of line).
+template <int HYB>
+__device__ __noinline__ u32 tie_full_key(const FusedArgs* a, u32 start, u32 e) {
+    return philox_perm_key(a->pair.pk, (u64)run_index<HYB>(*a, start, e));
+}
+
+// Two neighbouring sort words (wa before wb) that agree on the truncated key: is (full key, position) of wa larger
+// than that of wb?  Padding words (position >= n_c) count as key 0xFFFFFFFF: a real word never moves behind them.
+template <int HYB>
+__device__ __forceinline__ bool tie_out_of_order(const FusedArgs& a, u32 start, u32 n_c, u32 wa, u32 wb) {
+    const u32 ea = wa & 0xFFu, eb = wb & 0xFFu;
+    const u32 ka = ea < n_c ? tie_full_key<HYB>(&a, start, ea) : 0xFFFFFFFFu;
+    const u32 kb = eb < n_c ? tie_full_key<HYB>(&a, start, eb) : 0xFFFFFFFFu;
+    return ka > kb || (ka == kb && ea > eb);
+}
+
+// Words that agree on the truncated key form runs that the narrow sort left in position order; the low key bits it
+// dropped decide their true order.  Odd-even style repair in registers: a bubble pass inside every lane, one
+// exchange across each lane boundary of the group, repeated until a pass swaps nothing anywhere in the warp.
+template <int HYB, int G, int R>
+__device__ __forceinline__ void repair_ties(const FusedArgs& a, u32 (&x)[R], u32 start, u32 n_c, int lg) {
+    static_assert(R >= 2, "the two boundary words of a lane are different registers");
+    bool again;
+    do {
+        bool sw = false;
+#pragma unroll
+        for (int r = 0; r + 1 < R; ++r) {
+            if ((x[r] ^ x[r + 1]) < 0x100u && tie_out_of_order<HYB>(a, start, n_c, x[r], x[r + 1])) {
+                const u32 t = x[r]; x[r] = x[r + 1]; x[r + 1] = t;
+                sw = true;
+            }
+        }
+        // both lanes of a boundary take the same decision from the same two words
+        const u32 nx = __shfl_down_sync(0xffffffffu, x[0], 1), pv = __shfl_up_sync(0xffffffffu, x[R - 1], 1);
+        const bool swn = lg < G - 1 && (x[R - 1] ^ nx) < 0x100u && tie_out_of_order<HYB>(a, start, n_c, x[R - 1], nx);
+        const bool swp = lg > 0 && (pv ^ x[0]) < 0x100u && tie_out_of_order<HYB>(a, start, n_c, pv, x[0]);
+        if (swn) x[R - 1] = nx;
+        if (swp) x[0] = pv;
+        sw |= swn | swp;
+        again = __any_sync(0xffffffffu, sw);
+    } while (again);
+}
+
+// A group of G lanes, one cell of 2 <= n_c <= G R super-droplets per group (n_c = 0: the group idles along).
+// Returns this lane's share of the number of zero multiplicities the cell holds AFTER the step.  The hot flow is
+// straight-line code: loads, Philox blocks (computed for padding slots too, so the R chains interleave), sort and
+// the first-level pair test are predicated, not branched.
+// FULL: every group of the warp has n_c == G R (no padding, no guards); the caller branches warp-uniformly.
+template <int KIND, int HYB, int G, int R, bool FULL>
+__device__ __forceinline__ u32 group_cells(const FusedArgs& a, WarpStage<R>& st, const u32 start, const u32 n_c_in,
+                                           const int lane) {
+    constexpr int P = G * R;
+    static_assert(P <= 256, "the position takes 8 bits of the sort word");
+    const u32 n_c = FULL ? (u32)P : n_c_in;
     const PairArgs& pa = a.pair;
+    const int lg = lane & (G - 1);
+    const u32 cbase = (u32)(lane / G) * (u32)P;  // this cell's slice of the staging arrays
     u32 zeros = 0;
-    // ---- a1 + load: striped positions e = 32 r + lane (coalesced), everything parked in shared memory ----
-    u32 idx[R];
-    long long xi[R];
-    double vol[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const u32 e = 32u * r + lane;
-        idx[r] = 0; xi[r] = 1; vol[r] = 0.0;
-        if (e < n_c) {
-            idx[r] = run_index<WORD>(a, start, e);
-            xi[r] = pa.xi[idx[r]];
-            vol[r] = pa.v[idx[r]];
-        }
-    }
-    // keys first: Philox needs only the index, so the attribute loads above stay in flight under it
-    u32 x[R], w3[R], key[R];
+    // ---- a1 + load: striped positions e = G r + lg (coalesced within the cell); the fp32 side values and Philox
+    //      word 3 are parked in shared memory, the sort word stays in registers ----
+    u32 x[R];
     const int drop = 32 - a.key_bits;
+    constexpr int LB = R < 4 ? R : 4;  // loads in flight per lane and batch (8 measured the same)
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const u32 e = 32u * r + lane;
-        const PhiloxOut w = philox4x32_10(pa.pk, (u64)idx[r]);
-        w3[r] = w.w3; key[r] = w.w0;
-        // padding sorts to the end (a real word with the same upper bits has a smaller position) and keeps a
-        // position inside the staging tile, so that the unguarded reads of the pair test stay in bounds
-        x[r] = (e < n_c) ? (((w.w0 >> drop) << 8) | e) : (0xFFFFFF00u | e);
-    }
+    for (int b = 0; b < R; b += LB) {
+        u32 idx[LB];
+        long long xi[LB];
+        double vol[LB];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const u32 e = 32u * r + lane;
-        const float xf = __ll2float_ru(xi[r]);  // 0 -> 0.0f, xi >= 1 -> >= 1.0f (padding slots hold xi = 1)
-        zeros += (xf == 0.0f);
-        if (e < n_c) {
-            st.xv[e] = make_longlong2(xi[r], __double_as_longlong(vol[r]));
-            st.aux[e] = make_float4(xf, __double2float_ru(vol[r]), __uint_as_float(w3[r]), __uint_as_float(key[r]));
-            if (WORD != 0) st.idx[e] = idx[r];
+        for (int t = 0; t < LB; ++t) {
+            const u32 e = (u32)(b + t) * G + lg;
+            idx[t] = 0; xi[t] = 1; vol[t] = 0.0;
+            if (FULL || e < n_c) {
+                idx[t] = run_index<HYB>(a, start, e);
+                xi[t] = pa.xi[idx[t]];
+                vol[t] = pa.v[idx[t]];
+            }
+        }
+#pragma unroll
+        for (int t = 0; t < LB; ++t) {
+            const u32 e = (u32)(b + t) * G + lg;
+            // keys first: Philox needs only the index, so the attribute loads stay in flight under it
+            const PhiloxOut w = philox4x32_10(pa.pk, (u64)idx[t]);
+            // padding sorts to the end (a real word with the same upper bits has a smaller position) and keeps a
+            // position inside the cell's staging slice, so that the unguarded reads of the pair test stay in bounds
+            x[b + t] = (FULL || e < n_c) ? (((w.w0 >> drop) << 8) | e) : (0xFFFFFF00u | e);
+            const float xf = __ll2float_ru(xi[t]);  // 0 -> 0.0f, xi >= 1 -> >= 1.0f (padding slots hold xi = 1)
+            zeros += (xf == 0.0f);
+            if (FULL || e < n_c) {
+                st.fl[cbase + e] = make_float2(xf, __double2float_ru(vol[t]));
+                st.w3[cbase + e] = w.w3;
+            }
         }
     }
-    // ---- a3: sort (truncated key, position) words; slot s = lane R + r afterwards ----
-    warp_bitonic_sort<u32, R>(x, lane);
-    // neighbours with equal truncated keys: their order is decided by the dropped bits -> wide redo
+    // ---- a3: sort (truncated key, position) words; slot s = lg R + r afterwards ----
+    group_bitonic_sort<R, G>(x, lg);
+    // neighbours with equal truncated keys: their order is decided by the dropped bits -> repair
     u32 ties = 0xFFFFFFFFu;  // smallest XOR of two neighbouring words that are both real
     const u32 nxt = __shfl_down_sync(0xffffffffu, x[0], 1);
-    if (FULL) {  // a full tile has no padding
 #pragma unroll
-        for (int r = 0; r + 1 < R; ++r) ties = min(ties, x[r] ^ x[r + 1]);
-        if (lane < 31) ties = min(ties, x[R - 1] ^ nxt);
-    } else {
-#pragma unroll
-        for (int r = 0; r + 1 < R; ++r)
-            if ((u32)(lane * R + r + 1) < n_c) ties = min(ties, x[r] ^ x[r + 1]);
-        if (lane < 31 && (u32)(lane * R + R) < n_c) ties = min(ties, x[R - 1] ^ nxt);
-    }
+    for (int r = 0; r + 1 < R; ++r)
+        if (FULL || (u32)(lg * R + r + 1) < n_c) ties = min(ties, x[r] ^ x[r + 1]);
+    if (lg < G - 1 && (FULL || (u32)(lg * R + R) < n_c)) ties = min(ties, x[R - 1] ^ nxt);
     __syncwarp();  // the staging writes of all lanes are visible from here on
-    u32 pos[R];
-    if (__any_sync(0xffffffffu, ties < 0x100u)) {
-        u64 wide[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {  // the real words occupy the first n_c slots of the narrow result
-            const u32 e = x[r] & 0xFFu;
-            wide[r] = ((u32)(lane * R + r) < n_c) ? (((u64)__float_as_uint(st.aux[e].w) << 32) | (u64)e) : ~0ull;
-        }
-        warp_bitonic_sort<u64, R>(wide, lane);
-#pragma unroll
-        for (int r = 0; r < R; ++r) pos[r] = (u32)wide[r] & 0xFFu;
-    } else {
-#pragma unroll
-        for (int r = 0; r < R; ++r) pos[r] = x[r] & 0xFFu;
-    }
+    if (__any_sync(0xffffffffu, ties < 0x100u)) repair_ties<HYB, G, R>(a, x, start, n_c, lg);
     if (a.dbg_perm) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const u32 s = lane * R + r;
-            if (s < n_c) a.dbg_perm[start + s] = (int32_t)(WORD == 0 ? start + pos[r] : st.idx[pos[r]]);
+            const u32 s = lg * R + r;
+            if (s < n_c) a.dbg_perm[start + s] = (int32_t)run_index<HYB>(a, start, x[r] & 0xFFu);
         }
     }
     // ---- a4, level 1: every pair of neighbouring slots -- a dozen fp32 operations decide "gamma = 0 for sure" ----
-    constexpr int NP = (R >= 2) ? R / 2 : 1;
-    u32 first[NP], second[NP];  // run positions of the pair's members, in shuffled order
-    u32 need = 0;               // bit q: pair q of this lane goes on to the exact levels
+    constexpr int NP = R / 2;
+    u32 need = 0;  // bit q: pair q of this lane goes on to the exact levels
     const float cscale = pa.cheap_c * (float)pair_scale_int(n_c);
     const bool dbg = pa.dbg_gamma != nullptr;
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
-        bool valid;
-        if (R >= 2) {
-            first[q] = pos[2 * q];
-            second[q] = pos[(2 * q + 1) % R];
-            valid = (u32)(lane * R + 2 * q + 1) < n_c;
-        } else {
-            first[q] = pos[0];
-            second[q] = __shfl_down_sync(0xffffffffu, pos[0], 1);
-            valid = ((lane & 1) == 0) && ((u32)lane + 1u < n_c);
-        }
+        const u32 ea = x[2 * q] & 0xFFu, eb = x[2 * q + 1] & 0xFFu;  // run positions of the pair's members, shuffled order
+        const bool valid = FULL || (u32)(lg * R + 2 * q + 1) < n_c;
         // (slots past n_c hold padding positions: the staged values read there are unspecified, `valid` drops them)
-        const float4 A = st.aux[first[q]], B = st.aux[second[q]];
+        const float2 A = st.fl[cbase + ea], B = st.fl[cbase + eb];
+        const u32 w3a = st.w3[cbase + ea];
         // a dead partner (xi = 0 rounds up to 0.0f, xi >= 1 to >= 1.0f): gamma~ = 0 whatever gamma is (R7)
         const bool alive = fminf(A.x, B.x) != 0.0f;
-        const bool may = pair_cheap_may_collide<KIND>(cscale, fmaxf(A.x, B.x), A.y, B.y, __float_as_uint(A.z));
+        const bool may = pair_cheap_may_collide<KIND>(cscale, fmaxf(A.x, B.x), A.y, B.y, w3a);
         if (valid && (dbg || (alive && may))) need |= 1u << q;
     }
     // ---- levels 2 and 3: the fp32 interval bound and the full fp64 rule, only where needed; lanes take
-    //      their pending pairs one at a time ----
+    //      their pending pairs one at a time and read the exact attributes again ----
     while (__any_sync(0xffffffffu, need != 0)) {
         if (need) {
             const int q = __ffs(need) - 1;
             need &= need - 1u;
-            const u32 ea = select_reg<NP>(first, q), eb = select_reg<NP>(second, q);
-            const longlong2 A = st.xv[ea], B = st.xv[eb];
-            const double vA = __longlong_as_double(A.y), vB = __longlong_as_double(B.y);
-            const bool swap = A.x < B.x;
-            const u32 w3a = __float_as_uint(st.aux[ea].z);
+            const u32 ea = select_reg<R>(x, 2 * q) & 0xFFu, eb = select_reg<R>(x, 2 * q + 1) & 0xFFu;
+            const u32 ja = run_index<HYB>(a, start, ea), jb = run_index<HYB>(a, start, eb);
+            const long long xa = pa.xi[ja], xb = pa.xi[jb];
+            const double va = pa.v[ja], vb = pa.v[jb];
+            const bool swap = xa < xb;
             // w2 = 0 makes u a lower bound of the true uniform: the test stays conservative
-            if (dbg || pair_may_collide(pa, swap ? B.x : A.x, swap ? vB : vA, swap ? vA : vB, 0u, w3a, n_c)) {
-                const u32 ja = (WORD == 0) ? start + ea : st.idx[ea];
-                const u32 jb = (WORD == 0) ? start + eb : st.idx[eb];
+            if (dbg || pair_may_collide(pa, swap ? xb : xa, swap ? vb : va, swap ? va : vb, 0u, st.w3[cbase + ea], n_c)) {
                 const PhiloxOut w = philox4x32_10(pa.pk, (u64)ja);  // the exact uniform of the first member (R2)
-                zeros += pair_apply(pa, ja, jb, A.x, vA, B.x, vB, w.w2, w.w3, n_c);
+                zeros += pair_apply(pa, ja, jb, xa, va, xb, vb, w.w2, w.w3, n_c);
             }
         }
     }
     return zeros;
 }
 
-template <int WORD, int RMAX, int R, int KIND>
-__device__ __forceinline__ u32 warp_cell_any(const FusedArgs& a, CellStage<WORD, RMAX>& st, u32 start, u32 n_c, int lane) {
-    // regular grids fill their tiles exactly (configs[2], [3]: 32 and 128 per cell): that case runs without guards
-    if (n_c == 32u * R) return warp_cell<WORD, RMAX, R, KIND, true>(a, st, start, n_c, lane);
-    return warp_cell<WORD, RMAX, R, KIND, false>(a, st, start, n_c, lane);
+// The warp's 32 / G cells of size class P = G R: cells [wfirst * 32 / G, ...) of the class list.
+template <int KIND, int HYB, int G, int R>
+__device__ __forceinline__ u32 class_cells(const FusedArgs& a, WarpStage<R>& st, const u32* __restrict__ list, u32 count,
+                                           u32 wfirst, int lane) {
+    constexpr int P = G * R;
+    const u32 ci = wfirst * (u32)(32 / G) + (u32)(lane / G);
+    u32 start = 0, n_c = 0;
+    if (ci < count) {
+        const u32 c = list ? __ldg(list + ci) : ci;
+        start = __ldg(a.pair.cell_start + c);
+        n_c = __ldg(a.pair.cell_start + c + 1) - start;
+    }
+    u32 zeros = 0;
+    if (n_c == 1 && (lane & (G - 1)) == 0) {  // nothing to pair; a lone super-droplet still counts as a zero when its multiplicity is 0
+        const u32 i = run_index<HYB>(a, start, 0);
+        zeros = (a.pair.xi[i] == 0);
+        if (a.dbg_perm) a.dbg_perm[start] = (int32_t)i;
+    }
+    if (n_c > (u32)P) {  // unreachable: k_cell_bounds refuses such cells and the lists follow its classes
+        a.sticky[STICKY_BAD_DATA] = 1u;
+        n_c = 0;
+    }
+    if (n_c < 2) n_c = 0;
+    if (!__any_sync(0xffffffffu, n_c != 0)) return zeros;
+    // regular grids fill their slots exactly (configs[2], [3]: 32 and 128 per cell): that case runs without guards
+    if (__all_sync(0xffffffffu, n_c == (u32)P)) return zeros + group_cells<KIND, HYB, G, R, true>(a, st, start, n_c, lane);
+    return zeros + group_cells<KIND, HYB, G, R, false>(a, st, start, n_c, lane);
 }
 
-template <int WORD, int RMAX, int KIND>
-__global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const FusedArgs a) {
-    __shared__ CellStage<WORD, RMAX> s_stage[CF_WARPS];
+template <int KIND, int HYB, int R>
+__global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const __grid_constant__ FusedArgs a) {
+    __shared__ WarpStage<R> s_stage[CF_WARPS];
     if (a.ctl[CTL_UNSORTED] == a.epoch) return;  // k_cell_bounds refused the input: the step is skipped as a whole
     if (a.halt_tag) {  // a step of sdm_coalescence_steps: a halted run stays halted until the host has compacted
         const u32 halted = a.run[RUN_HALT];
@@ -461,31 +555,24 @@ __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const Fu
     }
     if (a.zc_clear && blockIdx.x == 0 && threadIdx.x == 0) *a.zc_clear = 0u;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    CellStage<WORD, RMAX>& st = s_stage[warp];
-    // one warp per cell, one launch wave after another: the block scheduler balances the (data-dependent)
-    // cost of the cells; a persistent strided loop measured 12 % slower on cfg3
-    const int c = blockIdx.x * CF_WARPS + warp;
+    WarpStage<R>& st = s_stage[warp];
+    // blocks are dealt out class by class, one launch wave after another: the block scheduler balances the
+    // (data-dependent) cost of the cells; a persistent strided loop measured 12 % slower on cfg3
+    u32 cls = 0, bfirst = 0;
+#pragma unroll
+    for (u32 k = 0; k + 1 < (u32)CELL_CLASSES; ++k)
+        if (blockIdx.x >= a.class_block_end[k]) { cls = k + 1; bfirst = a.class_block_end[k]; }
+    const u32 wfirst = (blockIdx.x - bfirst) * CF_WARPS + warp;
     u32 zeros = 0;
-    if (c < a.n_cell) {
-        const u32 start = __ldg(a.pair.cell_start + c);
-        const u32 n_c = __ldg(a.pair.cell_start + c + 1) - start;
-        if (n_c < 2) {  // nothing to pair; a lone super-droplet still counts as a zero when its multiplicity is 0
-            if (n_c == 1 && lane == 0) {
-                const u32 i = run_index<WORD>(a, start, 0);
-                zeros = (a.pair.xi[i] == 0);
-                if (a.dbg_perm) a.dbg_perm[start] = (int32_t)i;
-            }
-        } else if (n_c <= 32) {
-            zeros = warp_cell_any<WORD, RMAX, 1, KIND>(a, st, start, n_c, lane);
-        } else if (RMAX >= 2 && n_c <= 64) {
-            if constexpr (RMAX >= 2) zeros = warp_cell_any<WORD, RMAX, 2, KIND>(a, st, start, n_c, lane);
-        } else if (RMAX >= 4 && n_c <= 128) {
-            if constexpr (RMAX >= 4) zeros = warp_cell_any<WORD, RMAX, 4, KIND>(a, st, start, n_c, lane);
-        } else if (RMAX >= 8 && n_c <= 256) {
-            if constexpr (RMAX >= 8) zeros = warp_cell_any<WORD, RMAX, 8, KIND>(a, st, start, n_c, lane);
-        } else if (lane == 0) {
-            a.sticky[STICKY_BAD_DATA] = 1u;  // unreachable: k_cell_bounds refuses such cells
-        }
+    // class k: P = 32 << k slots per cell on G = P / R lanes
+    if (cls == 0) {
+        if constexpr (32 / R >= 2) zeros = class_cells<KIND, HYB, 32 / R, R>(a, st, a.class_cells[0], a.class_count[0], wfirst, lane);
+    } else if (cls == 1) {
+        if constexpr (64 / R >= 2 && 64 / R <= 32) zeros = class_cells<KIND, HYB, 64 / R, R>(a, st, a.class_cells[1], a.class_count[1], wfirst, lane);
+    } else if (cls == 2) {
+        if constexpr (128 / R >= 2 && 128 / R <= 32) zeros = class_cells<KIND, HYB, 128 / R, R>(a, st, a.class_cells[2], a.class_count[2], wfirst, lane);
+    } else {
+        if constexpr (256 / R >= 2 && 256 / R <= 32) zeros = class_cells<KIND, HYB, 256 / R, R>(a, st, a.class_cells[3], a.class_count[3], wfirst, lane);
     }
     // a5, fused: the number of zero multiplicities after the step (sdm_remove_zero_multiplicity reads it)
     zeros = __reduce_add_sync(0xffffffffu, zeros);
@@ -493,20 +580,19 @@ __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const Fu
 }
 
 // src_kind: 0 = cell_id array itself (CELL_SORTED), 1 = u64 sorted words, 2 = u32 sorted words (HYBRID).
-// rmax: register tile of the fused kernel launched next; it holds cells of up to 32 * rmax super-droplets.
+// strict: a refusal also raises the sticky SDM_ERR_BAD_DATA.
 cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
-                               int idxbits, int rmax, bool strict) {
+                               int idxbits, bool strict) {
     const long long n_chunks = (n_sd + CB_CHUNK - 1) / CB_CHUNK;
     const long long resident = (long long)ctx->sm_count * 6;
     const u32 grid = (u32)(n_chunks < resident ? n_chunks : resident);
-    const u32 max_class = rmax <= 2 ? 0u : (rmax <= 4 ? 1u : 2u);
     LaunchScope scope(ctx, PROF_CELL_BOUNDS);
     Workspace& ws = ctx->ws;
     const bool vec = (reinterpret_cast<uintptr_t>(src) & 15u) == 0;
 #define SDM_BOUNDS(SRC, VEC, IDXBITS)                                                                               \
-    k_cell_bounds<SRC, VEC><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, IDXBITS, max_class,          \
-                                                                strict ? 1u : 0u, ctx->epoch, ws.cell_start, ws.ctl, \
-                                                                ws.sticky, ws.run, ctx->mapped, ctx->dbg_cell_start)
+    k_cell_bounds<SRC, VEC><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, IDXBITS, strict ? 1u : 0u,  \
+                                                                ctx->epoch, ws.cell_start, ws.ctl, ws.sticky, ws.run, \
+                                                                ctx->mapped, ctx->dbg_cell_start)
     if (src_kind == 0) {
         if (vec) SDM_BOUNDS(0, true, 0);
         else SDM_BOUNDS(0, false, 0);
@@ -523,41 +609,46 @@ cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int6
 
 // The staging tiles want the shared-memory end of the L1 split.  The attribute is per device and per function:
 // it is set once per context (contexts live on one device) for every instantiation, and the result is checked.
-template <int WORD, int RMAX>
+template <int KIND, int HYB, int R>
 static cudaError_t prefer_shared_carveout() {
-    cudaError_t e = cudaFuncSetAttribute(k_cell_fused<WORD, RMAX, 0>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                         cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_cell_fused<WORD, RMAX, 1>, cudaFuncAttributePreferredSharedMemoryCarveout,
+    return cudaFuncSetAttribute(k_cell_fused<KIND, HYB, R>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                 cudaSharedmemCarveoutMaxShared);
 }
 
 cudaError_t init_cell_fused(sdm_ctx*) {
     cudaError_t e;
-#define SDM_CARVE(W)                                                         \
-    if ((e = prefer_shared_carveout<W, 2>()) != cudaSuccess) return e;       \
-    if ((e = prefer_shared_carveout<W, 4>()) != cudaSuccess) return e;       \
-    if ((e = prefer_shared_carveout<W, 8>()) != cudaSuccess) return e;
-    SDM_CARVE(0) SDM_CARVE(1) SDM_CARVE(2)
+#define SDM_CARVE(R)                                                              \
+    if ((e = prefer_shared_carveout<0, 0, R>()) != cudaSuccess) return e;         \
+    if ((e = prefer_shared_carveout<0, 1, R>()) != cudaSuccess) return e;         \
+    if ((e = prefer_shared_carveout<1, 0, R>()) != cudaSuccess) return e;         \
+    if ((e = prefer_shared_carveout<1, 1, R>()) != cudaSuccess) return e;
+    SDM_CARVE(4) SDM_CARVE(8)
 #undef SDM_CARVE
     return cudaSuccess;
 }
 
-template <int WORD, int KIND>
-static void launch_fused_kind(const FusedArgs& a, int rmax, u32 grid, cudaStream_t st) {
-    if (rmax <= 2) k_cell_fused<WORD, 2, KIND><<<grid, CF_BLOCK, 0, st>>>(a);
-    else if (rmax <= 4) k_cell_fused<WORD, 4, KIND><<<grid, CF_BLOCK, 0, st>>>(a);
-    else k_cell_fused<WORD, 8, KIND><<<grid, CF_BLOCK, 0, st>>>(a);
+template <int R>
+static void launch_fused_r(const FusedArgs& a, bool hybrid, u32 grid, cudaStream_t st) {
+    const bool golovin = a.pair.kp.kind == 0;
+    if (golovin && !hybrid) k_cell_fused<0, 0, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    else if (golovin) k_cell_fused<0, 1, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    else if (!hybrid) k_cell_fused<1, 0, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    else k_cell_fused<1, 1, R><<<grid, CF_BLOCK, 0, st>>>(a);
 }
 
-template <int WORD>
-static void launch_fused_word(const FusedArgs& a, int rmax, u32 grid, cudaStream_t st) {
-    if (a.pair.kp.kind == 0) launch_fused_kind<WORD, 0>(a, rmax, grid, st);
-    else launch_fused_kind<WORD, 1>(a, rmax, grid, st);
+// Words per lane of the group sort.  8 costs fewer instructions per super-droplet (more of the bitonic stages stay
+// inside the lanes); small problems, whose warps would not fill the machine then, take 4 (configs[2]: 10.6 us
+// against 11.8 us).  Cells of more than 128 entries need 8 (32 lanes x 8 words).
+int fused_words_per_lane(const sdm_ctx* ctx, const CellClasses& cc) {
+    if (cc.worst > 2 || ctx->fused_r == 8) return 8;
+    if (ctx->fused_r == 4) return 4;
+    long long slots = 0;
+    for (int k = 0; k < CELL_CLASSES; ++k) slots += (long long)cc.count[k] * (32ll << k);
+    return slots / (32 * 8) >= (long long)ctx->sm_count * 32 ? 8 : 4;
 }
 
-cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int rmax, int64_t* xi,
-                              double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
+cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, const CellClasses& cc,
+                              int64_t* xi, double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
                               const PhiloxKeys& pk, const StepLinks& links) {
     FusedArgs a;
     a.pair.sorted = nullptr;
@@ -577,6 +668,7 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.n_cell = n_cell;
     a.key_bits = ctx->narrow_key_bits;
     a.run_idx = run_idx;
+    a.run_u32 = src_kind == 2;
     a.idx_mask = (idxbits >= 64) ? ~0ull : ((1ull << idxbits) - 1ull);
     a.dbg_perm = ctx->dbg_perm;
     a.sticky = ctx->ws.sticky;
@@ -588,11 +680,20 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.halt_tag = links.halt_tag;
     a.run = ctx->ws.run;
     a.mapped = ctx->mapped;
-    const u32 grid = (u32)((n_cell + CF_WARPS - 1) / CF_WARPS);
+    const int R = fused_words_per_lane(ctx, cc);
+    u32 blocks = 0, off = 0;
+    for (int k = 0; k < CELL_CLASSES; ++k) {
+        const u32 cells_per_block = (u32)CF_WARPS * 32u / ((32u << k) / (u32)R);  // CF_WARPS * 32 / G
+        a.class_count[k] = cc.count[k];
+        a.class_cells[k] = cc.mixed ? ctx->ws.class_list + off : nullptr;
+        off += cc.count[k];
+        blocks += (cc.count[k] + cells_per_block - 1) / cells_per_block;
+        a.class_block_end[k] = blocks;
+    }
+    if (blocks == 0) return cudaSuccess;
     LaunchScope scope(ctx, PROF_CELL_FUSED);
-    if (src_kind == 0) launch_fused_word<0>(a, rmax, grid, ctx->stream);
-    else if (src_kind == 1) launch_fused_word<1>(a, rmax, grid, ctx->stream);
-    else launch_fused_word<2>(a, rmax, grid, ctx->stream);
+    if (R == 4) launch_fused_r<4>(a, src_kind != 0, blocks, ctx->stream);
+    else launch_fused_r<8>(a, src_kind != 0, blocks, ctx->stream);
     return cudaGetLastError();
 }
 

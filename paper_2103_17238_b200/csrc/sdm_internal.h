@@ -20,8 +20,10 @@ constexpr int SORT_BLOCK = 256;
 constexpr int SORT_ITEMS = 16;
 constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
 
-// Largest cell the register-resident per-cell sort of the fast path handles (one warp, 8 keys per lane).
+// Largest cell the register-resident per-cell sort of the fast path handles (16 lanes x 16 or 32 lanes x 8 words).
 constexpr int CELL_FAST_MAX = 256;
+// Cell-size classes of the fused kernel: class k = cells of at most 32 << k entries.
+constexpr int CELL_CLASSES = 4;
 
 // Largest collision-efficiency table sdm_set_collision_efficiency accepts (radii x ratios).
 constexpr int EFF_MAX_R = 128;
@@ -51,6 +53,8 @@ enum RunWord {
     RUN_ZC0 = 1,   // RUN_ZC0 + (s mod 3): zero multiplicities the array holds after step s of the run
     RUN_BOUNDS_TICKET = 4,  // k_cell_bounds: blocks finished (the last one publishes the verdict and resets it)
     RUN_BOUNDS_CLASS = 5,   // k_cell_bounds: worst cell-size class seen so far (reset by the last block)
+    RUN_CLASS_COUNT = 6,    // RUN_CLASS_COUNT + k - 1, k = 1..3: cells of size class k seen so far (reset by the last block)
+    RUN_LIST_CURSOR = 12,   // RUN_LIST_CURSOR + k, k = 0..3: k_class_lists' fill level of class k (zeroed by k_cell_bounds)
     RUN_WORDS = 64
 };
 // Words of the pinned, device-mapped host status block: what the host must learn WITHOUT draining the stream.
@@ -58,8 +62,9 @@ enum MappedWord {
     MAPPED_HALT = 0,     // RUN_HALT's tag
     MAPPED_ZEROS = 1,    // the zero count that caused the halt
     MAPPED_VERDICT_EPOCH = 2,  // k_cell_bounds: epoch of the last published verdict
-    MAPPED_VERDICT_CLASS = 3,  //   its worst cell-size class: 0 (<= 64), 1 (<= 128), 2 (<= 256), 3 (larger, or the
-                               //   array is not non-decreasing / holds an out-of-range cell_id)
+    MAPPED_VERDICT_CLASS = 3,  //   its worst cell-size class: 0 (<= 32), 1 (<= 64), 2 (<= 128), 3 (<= 256), 4 (larger,
+                               //   or the array is not non-decreasing / holds an out-of-range cell_id)
+    MAPPED_CLASS_COUNT = 4,    //   MAPPED_CLASS_COUNT + k - 1, k = 1..3: number of cells of size class k
     MAPPED_WORDS = 16
 };
 // Sticky words (zeroed at init and by sdm_poll_error only).
@@ -76,6 +81,7 @@ struct Workspace {
     u32* sticky;      // STICKY_WORDS
     u32* run;         // RUN_WORDS
     u32* cell_start;  // max_n_cell + 1
+    u32* class_list;  // max_n_cell: cell ids grouped by size class (k_class_lists; mixed cell sizes only)
     u64* buf_a;       // max_n_sd
     u64* buf_b;       // max_n_sd
     u32* cmp_state;   // max compaction tiles
@@ -106,6 +112,12 @@ enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR,
 // asynchronous copy; valid once `verdict_event` has completed).
 struct Verdict { u32 unsorted; u32 max_count; };
 struct ProfEvent { cudaEvent_t start, stop; int cls; };
+// What k_cell_bounds found out about the cell sizes, as the fused kernel's launch geometry needs it.
+struct CellClasses {
+    u32 worst;                 // largest class present (CELL_CLASSES: the fused kernel cannot take the input)
+    u32 count[CELL_CLASSES];   // cells served as class k (not mixed: every cell as class `worst`)
+    bool mixed;                // the cells are dealt out class by class through ws.class_list
+};
 }  // namespace sdm
 
 struct sdm_ctx {
@@ -130,6 +142,7 @@ struct sdm_ctx {
     int sm_count;
     int skip_key_digits;  // SDM_OPT_SKIP_KEY_DIGITS (-1 = automatic)
     int narrow_key_bits;  // key bits kept in the fused kernel's 32-bit sort word (SDM_OPT_NARROW_KEY_BITS)
+    int fused_r;          // words per lane of the fused kernel's group sort (SDM_OPT_FUSED_WORDS_PER_LANE; 0 = automatic)
     // optional per-launch CUDA-event timing (sdm_profile_enable)
     int profiling;
     std::vector<sdm::ProfEvent>* prof_events;
@@ -196,10 +209,11 @@ cudaError_t launch_cell_sort_pass(sdm_ctx* ctx, int pass, bool narrow, const int
                                   void* out, int64_t n_sd, int32_t n_cell, const Plan& plan);
 cudaError_t launch_cell_digit_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
                                    const Plan& plan);
-// strict: a refusal (class above the one `rmax` holds) also raises the sticky SDM_ERR_BAD_DATA (explicit paths);
-// AUTO's analysis passes strict = false and falls back instead.
+// strict: a refusal (a cell of more than CELL_FAST_MAX entries, unsorted or out-of-range input) also raises the
+// sticky SDM_ERR_BAD_DATA (explicit paths); AUTO's analysis passes strict = false and falls back instead.
 cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
-                               int idxbits, int rmax, bool strict);
+                               int idxbits, bool strict);
+cudaError_t launch_class_lists(sdm_ctx* ctx, int32_t n_cell, const u32 (&count)[CELL_CLASSES]);
 // Zero bookkeeping / halt protocol of one fused step (all nullable / 0: see FusedArgs in sdm_cellsort.cu).
 struct StepLinks {
     u32* zc_accum;
@@ -207,8 +221,8 @@ struct StepLinks {
     u32* zc_clear;
     u32 halt_tag;
 };
-cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, int rmax, int64_t* xi,
-                              double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
+cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, const CellClasses& cc,
+                              int64_t* xi, double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
                               const PhiloxKeys& pk, const StepLinks& links);
 cudaError_t launch_tie_repair(sdm_ctx* ctx, u64* sorted, int64_t n_sd, const Plan& plan, const PhiloxKeys& pk);
 cudaError_t launch_debug_perm(sdm_ctx* ctx, const u64* sorted, int64_t n_sd, const Plan& plan);

@@ -52,7 +52,7 @@ def _assert_vol_close(got, want, what=""):
 
 
 def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key_bits=None, expect_last_path=None,
-                track_zeros=False, skip_key_digits=None):
+                track_zeros=False, skip_key_digits=None, fused_r=None):
     """Steps the oracle and the GPU side by side over w.n_steps steps, comparing after every step."""
     sdm = _sdm()
     ow = w.copy()
@@ -66,6 +66,8 @@ def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key
             ctx.set_option(sdm.OPT_TRACK_ZEROS, 1)
         if skip_key_digits is not None:
             ctx.set_option(sdm.OPT_SKIP_KEY_DIGITS, skip_key_digits)
+        if fused_r is not None:
+            ctx.set_option(sdm.OPT_FUSED_WORDS_PER_LANE, fused_r)
         xi, v, cell = _to_dev(w, dev)
         dbg = ctx.debug_outputs(n, w.n_cell) if check_debug else None
         okp, gkp = _okp(w), _gkp(w)
@@ -230,14 +232,30 @@ def test_geometric_early_out_is_exact(dev, dV, path):
 
 @pytest.mark.parametrize("path", ["cell_sorted", "hybrid"])
 @pytest.mark.parametrize("bits", [1, 5, 12])
-def test_fused_kernel_wide_redo(dev, path, bits):
+@pytest.mark.parametrize("fused_r", [4, 8])
+def test_fused_kernel_tie_repair(dev, path, bits, fused_r):
     """With only a few key bits in the 32-bit sort word nearly every cell has neighbours whose truncated keys
-    tie, so the exact 64-bit redo runs all the time; the result must not change."""
+    tie (with 1 bit: runs of half a cell), so the exact repair by the regenerated full key runs all the time, inside
+    the lanes and across their boundaries; the result must not change."""
     sdm = _sdm()
     if path == "cell_sorted":
-        _run_parity(W.small("cfg4"), dev, path=sdm.PATH_CELL_SORTED, bit_exact=True, narrow_key_bits=bits)
+        _run_parity(W.small("cfg4"), dev, path=sdm.PATH_CELL_SORTED, bit_exact=True, narrow_key_bits=bits, fused_r=fused_r)
     else:
-        _run_parity(W.small("cfg3", interleave=True), dev, path=sdm.PATH_HYBRID, bit_exact=True, narrow_key_bits=bits)
+        _run_parity(W.small("cfg3", interleave=True), dev, path=sdm.PATH_HYBRID, bit_exact=True, narrow_key_bits=bits,
+                    fused_r=fused_r)
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg3z", "cfg4", "cfg4s"])
+@pytest.mark.parametrize("path", ["cell_sorted", "hybrid"])
+@pytest.mark.parametrize("fused_r", [4, 8])
+def test_fused_kernel_words_per_lane(dev, name, path, fused_r):
+    """Every group shape of the fused kernel (G = (32 << class) / R lanes per cell, R words per lane; uniform cell
+    sizes served as one class, mixed sizes through the class lists) gives the oracle's bits."""
+    sdm = _sdm()
+    p = {"cell_sorted": sdm.PATH_CELL_SORTED, "hybrid": sdm.PATH_HYBRID}[path]
+    _run_parity(W.small(name, interleave=(path == "hybrid")), dev, path=p, bit_exact=True, fused_r=fused_r)
+    _run_parity(W.small(name, interleave=(path == "hybrid")), dev, path=p, check_debug=False, bit_exact=True,
+                track_zeros=True, fused_r=fused_r)
 
 
 @pytest.mark.parametrize("n,n_cell", [(5000, 257), (9000, 70_000), (4096, 4096), (300, 1_000_000), (3000, 2)])
@@ -270,9 +288,10 @@ def test_hybrid_path_refuses_large_cells(dev):
         assert torch.equal(xi, before[0]) and torch.equal(v, before[1])
 
 
-@pytest.mark.parametrize("per_cell", [1, 2, 3, 31, 32, 33, 63, 64, 65, 127, 129, 255, 256])
-def test_cell_sorted_path_cell_sizes(dev, per_cell):
-    """every register-tile width of the per-cell sort, at and around its boundaries, plus empty cells"""
+@pytest.mark.parametrize("per_cell", [1, 2, 3, 15, 16, 17, 31, 32, 33, 63, 64, 65, 127, 128, 129, 255, 256])
+@pytest.mark.parametrize("fused_r", [None, 4, 8])
+def test_cell_sorted_path_cell_sizes(dev, per_cell, fused_r):
+    """every size class of the per-cell sort, at and around its boundaries, plus empty cells"""
     sdm = _sdm()
     rng = np.random.default_rng(per_cell)
     n_cell = 41
@@ -285,7 +304,7 @@ def test_cell_sorted_path_cell_sizes(dev, per_cell):
     xi[rng.random(n) < 0.2] = 9
     v = rng.integers(1, 9, n).astype(np.float64)
     w = W.Workload("edge", xi, v, cell, n_cell, 1.0, 1.0, W.GOLOVIN, 2.0 ** -9, 0.0, 4, 2)
-    _run_parity(w, dev, path=sdm.PATH_CELL_SORTED, bit_exact=True)
+    _run_parity(w, dev, path=sdm.PATH_CELL_SORTED, bit_exact=True, fused_r=fused_r)
 
 
 def test_auto_path_picks_the_path_that_fits(dev):
