@@ -40,7 +40,7 @@ METRIC = "super-droplet-steps/s per coalescence step; achieved HBM GB/s vs B200 
 UNIT = "SD-steps/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 L2_BYTES = 126e6
-PATH_NAMES = {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid"}
+PATH_NAMES = {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid", 4: "box_one_block"}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -99,6 +99,8 @@ def algorithmic_bytes(n_cell: int):
         "cell_digit_hist": 4,                        # read cell_id
         "tie_repair": 8,                             # read the sorted words (rewrites only tied runs)
         "volume_spectrum": 16,
+        "cell_classes": 0,                           # reads cell_start (n_cell words)
+        "box_step": 32,                              # read xi,v 16 + write xi,v 16 (one block, keys regenerated)
     }
 
 

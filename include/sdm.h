@@ -88,15 +88,20 @@ int sdm_set_collision_efficiency(sdm_ctx* ctx, const double* radius /* host */, 
  *                is updated: on a violation (the caller's error) the step is NOT applied and the sticky
  *                SDM_ERR_BAD_DATA flag is set.  Like AUTO they wait for the device's verdict on the cell sizes
  *                (it fixes the launch geometry) without draining the stream.
+ *   BOX          one cell of at most 8192 super-droplets (the paper's box example; SURVEY 8(f)
+ *                NEXT-1 "single-CTA fused step for tiny N"): the whole step -- keys, shuffle by counting placement of
+ *                the uniform keys, pair rule -- in one launch of one block out of shared memory.  Chosen explicitly
+ *                on an input that does not fit, the step takes the GENERAL path.
  *   AUTO         (default) never refuses valid input.  Every step first analyses cell_id on the device (one
  *                streaming read: range, order, largest cell) and the host waits for that verdict -- a few
  *                microseconds, through a mapped status word, without draining work enqueued behind it -- before
  *                it enqueues either the fused kernel (CELL_SORTED when the array is non-decreasing, HYBRID when the
- *                previous GENERAL step on the same array saw small cells in any order) or the GENERAL path.  So
+ *                previous GENERAL step on the same array saw small cells in any order), the BOX step (one small
+ *                cell) or the GENERAL path.  So
  *                cell_id may be rewritten in place between steps (a displacement step does exactly that): the
  *                next step simply takes the path that fits.  sdm_coalescence_steps pays the analysis once per
  *                call instead of once per step.  sdm_set_path() forgets what was learned. */
-typedef enum { SDM_PATH_AUTO = 0, SDM_PATH_GENERAL = 1, SDM_PATH_CELL_SORTED = 2, SDM_PATH_HYBRID = 3 } sdm_path;
+typedef enum { SDM_PATH_AUTO = 0, SDM_PATH_GENERAL = 1, SDM_PATH_CELL_SORTED = 2, SDM_PATH_HYBRID = 3, SDM_PATH_BOX = 4 } sdm_path;
 
 /* Bytes of device workspace sdm_init() needs for problems up to (max_n_sd, max_n_cell).
  * Returns 0 when the arguments are invalid (max_n_sd < 0, max_n_sd >= 2^30, max_n_cell < 1). */
@@ -266,7 +271,8 @@ int64_t sdm_launch_count(sdm_ctx* ctx);
  * host) since the last read, and resets the accumulation. */
 enum { SDM_PROF_KEYS_HIST = 0, SDM_PROF_CELL_SCAN, SDM_PROF_RADIX_PASS, SDM_PROF_PAIR, SDM_PROF_COUNT_ZERO,
        SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CELL_BOUNDS, SDM_PROF_CELL_FUSED,
-       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_TIE_REPAIR, SDM_PROF_SPECTRUM, SDM_PROF_DISPLACE, SDM_PROF_CLASSES };
+       SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_TIE_REPAIR, SDM_PROF_SPECTRUM, SDM_PROF_DISPLACE, SDM_PROF_CELL_CLASSES,
+       SDM_PROF_BOX_STEP, SDM_PROF_CLASSES };
 int sdm_profile_enable(sdm_ctx* ctx, int on);
 int sdm_profile_read(sdm_ctx* ctx, double* ms_out /* host */, int64_t* launches_out /* host */);
 

@@ -19,6 +19,7 @@ PATH_AUTO = 0
 PATH_GENERAL = 1
 PATH_CELL_SORTED = 2
 PATH_HYBRID = 3
+PATH_BOX = 4
 OPT_NARROW_KEY_BITS = 0
 OPT_TRACK_ZEROS = 1
 OPT_INDEX_BASE = 2
@@ -37,7 +38,7 @@ EXPORTS = [
 ]
 
 PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
-                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum", "displace"]
+                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum", "displace", "cell_classes", "box_step"]
 
 
 class SDMError(RuntimeError):

@@ -66,7 +66,7 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     w.cell_count = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 1) * 4));
     w.tile_state = reinterpret_cast<u32*>(take((size_t)MAX_PASSES * max_tiles * RADIX * 4));
     w.cell_start = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 2) * 4));
-    w.class_list = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 1) * 4));
+    w.class_list = reinterpret_cast<u32*>(take((size_t)CELL_CLASSES * (size_t)max_n_cell * 4));
     w.buf_a = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.buf_b = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
     w.cmp_state = reinterpret_cast<u32*>(take(cmp_tiles * 4));
@@ -166,7 +166,8 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
         cudaEventCreateWithFlags(&ctx->verdict_event, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->chunk_event[0], cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->chunk_event[1], cudaEventDisableTiming) != cudaSuccess ||
-        init_cell_fused(ctx) != cudaSuccess || init_volume_spectrum(ctx) != cudaSuccess) {
+        init_cell_fused(ctx) != cudaSuccess || init_box_step(ctx) != cudaSuccess ||
+        init_volume_spectrum(ctx) != cudaSuccess) {
         free_ctx(ctx);
         return SDM_ERR_CUDA;
     }
@@ -220,7 +221,7 @@ const char* sdm_strerror(int status) {
 }
 
 int sdm_set_path(sdm_ctx* ctx, int path) {
-    if (!ctx || path < SDM_PATH_AUTO || path > SDM_PATH_HYBRID) return SDM_ERR_INVALID_ARG;
+    if (!ctx || path < SDM_PATH_AUTO || path > SDM_PATH_BOX) return SDM_ERR_INVALID_ARG;
     ctx->path = path;
     ctx->verdict_valid = 0;  // AUTO re-learns the cell order on its next step
     return SDM_OK;
@@ -419,6 +420,27 @@ int enqueue_general_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
     return SDM_OK;
 }
 
+// BOX path: a single cell of at most BOX_MAX super-droplets, the whole step in one launch of one block.
+bool box_fits(const sdm_ctx* ctx, const StepArgs& A) {
+    return A.n_cell == 1 && A.n_sd <= BOX_MAX && (ctx->path == SDM_PATH_AUTO || ctx->path == SDM_PATH_BOX);
+}
+
+int enqueue_box_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
+    int rc;
+    if ((rc = clear_debug_gammas(ctx, A.n_sd))) return rc;
+    const PhiloxKeys pk = make_philox_keys(A.seed, step, ctx->index_base);
+    ctx->zero_hint_valid = 0;
+    ctx->verdict_valid = 0;
+    if ((rc = note_cuda(ctx, launch_box_step(ctx, A.xi, A.v, A.n_sd, A.dtdV, A.dkp, pk)))) return rc;
+    ctx->last_path = SDM_PATH_BOX;
+    return SDM_OK;
+}
+
+// A step without the fused per-cell kernel: the one-block box step when it fits, else the GENERAL path.
+int enqueue_unfused_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
+    return box_fits(ctx, A) ? enqueue_box_step(ctx, A, step) : enqueue_general_step(ctx, A, step);
+}
+
 // The index runs of the fused kernel: CELL_SORTED reads the arrays directly (kind 0); HYBRID gathers through the
 // words `run_idx` (kind 1: u64, kind 2: u32) that LSD passes over the cell_id digits alone have grouped by cell.
 struct FusedSource {
@@ -478,7 +500,7 @@ int enqueue_fused_step(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, 
 // Waits, WITHOUT draining the stream behind it, until k_cell_bounds of `epoch` has published its verdict in the
 // mapped status block: the worst cell-size class (CELL_CLASSES = the fused kernel cannot take this input) and the
 // number of cells per class.  Cells of nearly one size are all served as the worst class (no indirection); mixed
-// sizes are grouped by class first (k_class_lists, enqueued here).
+// sizes go through the class lists k_cell_classes has written.
 int wait_verdict(sdm_ctx* ctx, u32 epoch, int32_t n_cell, CellClasses* cc) {
     volatile u32* m = ctx->mapped;
     for (unsigned long spin = 1;; ++spin) {
@@ -496,16 +518,15 @@ int wait_verdict(sdm_ctx* ctx, u32 epoch, int32_t n_cell, CellClasses* cc) {
     cc->mixed = false;
     for (int k = 0; k < CELL_CLASSES; ++k) cc->count[k] = 0;
     if (cc->worst >= (u32)CELL_CLASSES) return SDM_OK;
-    u32 upper = 0;
-    for (int k = 1; k < CELL_CLASSES; ++k) upper += (cc->count[k] = m[MAPPED_CLASS_COUNT + k - 1]);
-    if (upper > (u32)n_cell) return note_cuda(ctx, cudaErrorUnknown);  // cannot happen: every cell is closed once
-    cc->count[0] = (u32)n_cell - upper;
+    uint64_t total = 0;
+    for (int k = 0; k < CELL_CLASSES; ++k) total += (cc->count[k] = m[MAPPED_CLASS_COUNT + k]);
+    if (total != (uint64_t)n_cell) return note_cuda(ctx, cudaErrorUnknown);  // cannot happen: every cell is listed once
     if ((uint64_t)cc->count[cc->worst] * 4u >= (uint64_t)n_cell * 3u) {
         for (int k = 0; k < CELL_CLASSES; ++k) cc->count[k] = (u32)k == cc->worst ? (u32)n_cell : 0u;
         return SDM_OK;
     }
     cc->mixed = true;
-    return note_cuda(ctx, launch_class_lists(ctx, n_cell, cc->count));
+    return SDM_OK;
 }
 
 // AUTO's hint: what the last GENERAL step on this very (cell_id pointer, n_sd, n_cell) saw.  Waits for its
@@ -583,7 +604,7 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
     } else if (ctx->path == SDM_PATH_AUTO) {
         if ((rc = auto_prepare(ctx, A, plan, &fused, &src))) return rc;
     }
-    if (!fused) return enqueue_general_step(ctx, A, step);
+    if (!fused) return enqueue_unfused_step(ctx, A, step);
     if ((rc = enqueue_fused_step(ctx, A, src, step, no_links, false))) return rc;
     note_zero_hint(ctx, multiplicity, n_sd);
     return SDM_OK;
@@ -774,7 +795,7 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
             // (cells of at most 256 super-droplets), and the loop comes back to try
             bool retry_fused = false;
             while (s < n_steps && !retry_fused) {
-                if ((rc = enqueue_general_step(ctx, A, step0 + (uint64_t)s))) return rc;
+                if ((rc = enqueue_unfused_step(ctx, A, step0 + (uint64_t)s))) return rc;
                 ++s;
                 if (!general_only) {
                     Verdict hint;

@@ -8,13 +8,13 @@
 // the global LSD sort of (cell_id << 32 | key) and the oracle's std::stable_sort produce, so the output
 // is bit-identical, at 32-48 B/SD of HBM traffic instead of 148.
 //
-//   k_cell_bounds<SRC>  reads the cell of every position once: verifies range and order, writes
-//                       cell_start[0..n_cell], counts the cells per size class (<= 32, 64, 128, 256 entries)
-//                       and publishes the verdict (device flag for the fused kernel, mapped host words for
-//                       the path choice and the launch geometry).  When the input does not fit the fused
-//                       kernel launched next, that kernel does nothing (the state is never half-updated).
-//   k_class_lists       mixed cell sizes only: the cell ids grouped by size class, so that every warp of the
-//                       fused kernel works on cells of one class.
+//   k_cell_bounds<SRC>  reads the cell of every position once (a pure streaming kernel): verifies range and
+//                       order, writes cell_start[0..n_cell].
+//   k_cell_classes      one thread per cell: size class (<= 32, 64, 128, 256 entries), the cell ids grouped by
+//                       class (so that every warp of the fused kernel works on cells of one class) and the
+//                       verdict (device flag for the fused kernel, mapped host words for the path choice and
+//                       the launch geometry).  When the input does not fit the fused kernel launched next,
+//                       that kernel does nothing (the state is never half-updated).
 //   k_cell_fused<R>     size class k = cells of at most P = 32 << k entries, sorted by G = P / R lanes holding
 //                       R words each; a warp takes 32 / G cells.  With R = 8 a cell of 128 runs 18 of the 28
 //                       bitonic stages inside the lanes (1 instruction per element) and 10 across lanes
@@ -73,54 +73,24 @@ __device__ __forceinline__ void cells_at4(const void* src, u32 i0, u32 n_sd, int
     }
 }
 
-// Position i opens cell cc and closes cell prev (opening every empty cell in between).  The closed cell
-// [s, i) holds more than m entries exactly when position i - 1 - m still belongs to it (sorted input), so its
-// size class costs up to four extra loads per cell, not per super-droplet.  Returns the size class of the
-// closed cell: 0 (<= 32 entries), 1 (<= 64), 2 (<= 128), 3 (<= 256), 4 (larger).
-template <int SRC>
-__device__ __forceinline__ u32 open_cells(const void* src, int idxbits, int prev, int cc, u32 i,
-                                          u32* __restrict__ cell_start, int32_t* __restrict__ dbg_cell_start) {
+// Position i opens cell cc (and every empty cell between prev and cc).
+__device__ __forceinline__ void open_cells(int prev, int cc, u32 i, u32* __restrict__ cell_start,
+                                           int32_t* __restrict__ dbg_cell_start) {
     for (int q = prev + 1; q <= cc; ++q) {
         cell_start[q] = i;
         if (dbg_cell_start) dbg_cell_start[q] = (int32_t)i;
     }
-    if (prev < 0) return 0;
-    u32 cls = 0;
-#pragma unroll
-    for (u32 m = 32; m <= 256; m <<= 1) {
-        if (i > m && cell_at<SRC>(src, i - 1u - m, idxbits) == prev) ++cls;
-        else break;
-    }
-    return cls;
 }
 
 template <int SRC, bool VEC>
 __global__ void __launch_bounds__(CB_BLOCK)
-k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32 strict, u32 epoch,
-              u32* __restrict__ cell_start, u32* __restrict__ ctl, u32* __restrict__ sticky, u32* __restrict__ run,
-              volatile u32* __restrict__ mapped, int32_t* __restrict__ dbg_cell_start) {
-    __shared__ u32 s_cls;
-    __shared__ u32 s_cnt[CELL_CLASSES];
+k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u32* __restrict__ cell_start,
+              u32* __restrict__ ctl, u32* __restrict__ run, int32_t* __restrict__ dbg_cell_start) {
     // the fused kernel that follows accumulates the zero count; no separate memset of the control block
     if (blockIdx.x == 0 && threadIdx.x == 0) ctl[CTL_ZERO_COUNT] = 0u;
-    if (threadIdx.x == 0) s_cls = 0u;
-    if (threadIdx.x < CELL_CLASSES) s_cnt[threadIdx.x] = 0u;
     const int lane = threadIdx.x & 31;
     bool bad = false;
-    u32 cls = 0;
-    u32 cnt = 0;  // closed cells per class, one byte each for the classes 1..3 of this thread (< 256 cells per thread)
     const u32 n_chunks = (n_sd + CB_CHUNK - 1) / CB_CHUNK;
-    auto note = [&](u32 k) {  // a closed cell of class k
-        cls = max(cls, k);
-        if (k >= 1u && k < CLASS_REFUSED) {
-            if (((cnt >> (8u * (k - 1u))) & 0xFFu) == 0xFFu) {  // flush a full byte counter
-                atomicAdd(&s_cnt[k], 0xFFu);
-                cnt -= 0xFFu << (8u * (k - 1u));
-            }
-            cnt += 1u << (8u * (k - 1u));
-        }
-    };
-    __syncthreads();
     for (u32 ch = blockIdx.x; ch < n_chunks; ch += gridDim.x) {
         const u32 base = ch * (u32)CB_CHUNK;
         int c[CB_K][4];
@@ -154,7 +124,7 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
                     p = prev;
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
-                        if (c[k][j] != p) note(open_cells<SRC>(src, idxbits, p, c[k][j], i0 + j, cell_start, dbg_cell_start));
+                        if (c[k][j] != p) open_cells(p, c[k][j], i0 + j, cell_start, dbg_cell_start);
                         p = c[k][j];
                     }
                 }
@@ -168,9 +138,9 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
                         if (cc < 0 || cc >= n_cell || cc < prev) {
                             bad = true;
                         } else {
-                            if (cc != prev) note(open_cells<SRC>(src, idxbits, prev, cc, i, cell_start, dbg_cell_start));
-                            if (i == n_sd - 1)  // the array end closes cell cc and opens the (empty) rest
-                                note(open_cells<SRC>(src, idxbits, cc, n_cell, n_sd, cell_start, dbg_cell_start));
+                            if (cc != prev) open_cells(prev, cc, i, cell_start, dbg_cell_start);
+                            if (i == n_sd - 1)  // the array end opens the (empty) rest and closes the array
+                                open_cells(cc, n_cell, n_sd, cell_start, dbg_cell_start);
                         }
                         prev = cc;
                     }
@@ -178,22 +148,49 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
             }
         }
     }
-    if (bad) cls = CLASS_REFUSED;  // out of range or out of order: refused like a cell that is too large
-    cls = __reduce_max_sync(0xffffffffu, cls);
-    if (lane == 0 && cls) atomicMax(&s_cls, cls);
-#pragma unroll
-    for (u32 k = 1; k < CLASS_REFUSED; ++k) {
-        const u32 n = __reduce_add_sync(0xffffffffu, (cnt >> (8u * (k - 1u))) & 0xFFu);
-        if (lane == 0 && n) atomicAdd(&s_cnt[k], n);
+    // out of range or out of order: refused like a cell that is too large (k_cell_classes publishes the verdict)
+    if (__any_sync(0xffffffffu, bad) && lane == 0) atomicMax(&run[RUN_BOUNDS_CLASS], CLASS_REFUSED);
+}
+
+// Second half of the analysis, one thread per cell: the size class of every cell from cell_start (0: <= 32 entries,
+// 1: <= 64, 2: <= 128, 3: <= 256, refused: larger), the cell ids grouped by class (list[k * stride ...]: cells of
+// fewer than two entries go to class 0 -- the fused kernel still counts a lone zero multiplicity; the order inside a
+// class is the (nearly ascending) order in which the warps draw their slots -- cells are independent, so no result
+// depends on it), and the verdict: the last block publishes the worst class and the class counts through the mapped
+// status words, and raises the device-side refusal flag the fused kernel looks at.
+__global__ void __launch_bounds__(256)
+k_cell_classes(const u32* __restrict__ cell_start, int n_cell, u32 strict, u32 epoch, u32* __restrict__ ctl,
+               u32* __restrict__ sticky, u32* __restrict__ run, volatile u32* __restrict__ mapped,
+               u32* __restrict__ list, u32 stride) {
+    __shared__ u32 s_cls;
+    if (threadIdx.x == 0) s_cls = 0u;
+    __syncthreads();
+    const int c = blockIdx.x * 256 + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    u32 cls = 0xFFu;
+    if (c < n_cell) {
+        const u32 n = cell_start[c + 1] - cell_start[c];
+        cls = n <= 32u ? 0u : (n <= 64u ? 1u : (n <= 128u ? 2u : (n <= 256u ? 3u : CLASS_REFUSED)));
     }
+    const u32 lt = lanemask_lt();
+#pragma unroll
+    for (u32 k = 0; k < CLASS_REFUSED; ++k) {
+        const u32 m = __ballot_sync(0xffffffffu, cls == k);
+        if (m == 0u) continue;
+        const int leader = __ffs(m) - 1;
+        u32 base = 0;
+        if (lane == leader) base = atomicAdd(&run[RUN_LIST_CURSOR + k], (u32)__popc(m));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (cls == k) list[(size_t)k * stride + base + __popc(m & lt)] = (u32)c;
+    }
+    const u32 wcls = __reduce_max_sync(0xffffffffu, cls == 0xFFu ? 0u : cls);
+    if (lane == 0 && wcls) atomicMax(&s_cls, wcls);
     __syncthreads();
     if (threadIdx.x == 0) {
         if (s_cls) atomicMax(&run[RUN_BOUNDS_CLASS], s_cls);
-        for (u32 k = 1; k < CLASS_REFUSED; ++k)
-            if (s_cnt[k]) atomicAdd(&run[RUN_CLASS_COUNT + k - 1], s_cnt[k]);
         __threadfence();
         const u32 t = atomicAdd(&run[RUN_BOUNDS_TICKET], 1u);
-        if (t == gridDim.x - 1) {  // the last block: every other block's class and counts are visible (fence + ticket)
+        if (t == gridDim.x - 1) {  // the last block: every other block's class and list entries are visible (fence + ticket)
             __threadfence();
             const u32 worst = atomicExch(&run[RUN_BOUNDS_CLASS], 0u);
             run[RUN_BOUNDS_TICKET] = 0u;
@@ -201,51 +198,12 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
                 ctl[CTL_UNSORTED] = epoch;  // tagged with this step's epoch: stale refusals never match
                 if (strict) sticky[STICKY_BAD_DATA] = 1u;
             }
-            for (u32 k = 1; k < CLASS_REFUSED; ++k) mapped[MAPPED_CLASS_COUNT + k - 1] = atomicExch(&run[RUN_CLASS_COUNT + k - 1], 0u);
-            for (u32 k = 0; k < CLASS_REFUSED; ++k) run[RUN_LIST_CURSOR + k] = 0u;
+            for (u32 k = 0; k < CLASS_REFUSED; ++k) mapped[MAPPED_CLASS_COUNT + k] = atomicExch(&run[RUN_LIST_CURSOR + k], 0u);
             mapped[MAPPED_VERDICT_CLASS] = worst;
             __threadfence_system();
             mapped[MAPPED_VERDICT_EPOCH] = epoch;
         }
     }
-}
-
-// Cell ids grouped by size class: list[off[k] ...] holds the cells of class k (cells of fewer than two entries go to
-// class 0: the fused kernel still counts a lone zero multiplicity).  off[] is the exclusive prefix of the class
-// counts k_cell_bounds published; the order inside a class is the (nearly ascending) order in which the warps
-// draw their slots -- cells are independent, so the result does not depend on it.
-struct ClassOffsets { u32 off[CELL_CLASSES]; };
-
-__global__ void __launch_bounds__(256)
-k_class_lists(const u32* __restrict__ cell_start, int n_cell, const ClassOffsets o, u32* __restrict__ cursor,
-              u32* __restrict__ list) {
-    const int c = blockIdx.x * 256 + threadIdx.x;
-    const bool valid = c < n_cell;
-    u32 cls = 0xFFu;
-    if (valid) {
-        const u32 n = __ldg(cell_start + c + 1) - __ldg(cell_start + c);
-        cls = n <= 32u ? 0u : (n <= 64u ? 1u : (n <= 128u ? 2u : 3u));
-    }
-    const u32 lt = lanemask_lt();
-#pragma unroll
-    for (u32 k = 0; k < (u32)CELL_CLASSES; ++k) {
-        const u32 m = __ballot_sync(0xffffffffu, cls == k);
-        if (m == 0u) continue;
-        u32 base = 0;
-        if ((threadIdx.x & 31) == __ffs(m) - 1) base = atomicAdd(&cursor[k], (u32)__popc(m));
-        base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
-        if (cls == k) list[o.off[k] + base + __popc(m & lt)] = (u32)c;
-    }
-}
-
-cudaError_t launch_class_lists(sdm_ctx* ctx, int32_t n_cell, const u32 (&count)[CELL_CLASSES]) {
-    ClassOffsets o;
-    u32 run = 0;
-    for (int k = 0; k < CELL_CLASSES; ++k) { o.off[k] = run; run += count[k]; }
-    LaunchScope scope(ctx, PROF_CELL_BOUNDS);
-    k_class_lists<<<(n_cell + 255) / 256, 256, 0, ctx->stream>>>(ctx->ws.cell_start, n_cell, o, ctx->ws.run + RUN_LIST_CURSOR,
-                                                                 ctx->ws.class_list);
-    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -580,30 +538,38 @@ __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const __
 }
 
 // src_kind: 0 = cell_id array itself (CELL_SORTED), 1 = u64 sorted words, 2 = u32 sorted words (HYBRID).
-// strict: a refusal also raises the sticky SDM_ERR_BAD_DATA.
+// strict: a refusal also raises the sticky SDM_ERR_BAD_DATA.  Two launches: the streaming boundary kernel over the
+// super-droplets, then the per-cell class kernel that publishes the verdict.
 cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
                                int idxbits, bool strict) {
     const long long n_chunks = (n_sd + CB_CHUNK - 1) / CB_CHUNK;
-    const long long resident = (long long)ctx->sm_count * 6;
+    const long long resident = (long long)ctx->sm_count * 8;
     const u32 grid = (u32)(n_chunks < resident ? n_chunks : resident);
-    LaunchScope scope(ctx, PROF_CELL_BOUNDS);
     Workspace& ws = ctx->ws;
     const bool vec = (reinterpret_cast<uintptr_t>(src) & 15u) == 0;
-#define SDM_BOUNDS(SRC, VEC, IDXBITS)                                                                               \
-    k_cell_bounds<SRC, VEC><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, IDXBITS, strict ? 1u : 0u,  \
-                                                                ctx->epoch, ws.cell_start, ws.ctl, ws.sticky, ws.run, \
-                                                                ctx->mapped, ctx->dbg_cell_start)
-    if (src_kind == 0) {
-        if (vec) SDM_BOUNDS(0, true, 0);
-        else SDM_BOUNDS(0, false, 0);
-    } else if (src_kind == 1) {
-        if (vec) SDM_BOUNDS(1, true, idxbits);
-        else SDM_BOUNDS(1, false, idxbits);
-    } else {
-        if (vec) SDM_BOUNDS(2, true, idxbits);
-        else SDM_BOUNDS(2, false, idxbits);
-    }
+    {
+        LaunchScope scope(ctx, PROF_CELL_BOUNDS);
+#define SDM_BOUNDS(SRC, VEC, IDXBITS)                                                                                   \
+    k_cell_bounds<SRC, VEC><<<grid, CB_BLOCK, 0, ctx->stream>>>(src, (u32)n_sd, n_cell, IDXBITS, ws.cell_start, ws.ctl, \
+                                                                ws.run, ctx->dbg_cell_start)
+        if (src_kind == 0) {
+            if (vec) SDM_BOUNDS(0, true, 0);
+            else SDM_BOUNDS(0, false, 0);
+        } else if (src_kind == 1) {
+            if (vec) SDM_BOUNDS(1, true, idxbits);
+            else SDM_BOUNDS(1, false, idxbits);
+        } else {
+            if (vec) SDM_BOUNDS(2, true, idxbits);
+            else SDM_BOUNDS(2, false, idxbits);
+        }
 #undef SDM_BOUNDS
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    LaunchScope scope(ctx, PROF_CELL_CLASSES);
+    k_cell_classes<<<(n_cell + 255) / 256, 256, 0, ctx->stream>>>(ws.cell_start, n_cell, strict ? 1u : 0u, ctx->epoch, ws.ctl,
+                                                                  ws.sticky, ws.run, ctx->mapped, ws.class_list,
+                                                                  (u32)ctx->max_n_cell);
     return cudaGetLastError();
 }
 
@@ -681,12 +647,11 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.run = ctx->ws.run;
     a.mapped = ctx->mapped;
     const int R = fused_words_per_lane(ctx, cc);
-    u32 blocks = 0, off = 0;
+    u32 blocks = 0;
     for (int k = 0; k < CELL_CLASSES; ++k) {
         const u32 cells_per_block = (u32)CF_WARPS * 32u / ((32u << k) / (u32)R);  // CF_WARPS * 32 / G
         a.class_count[k] = cc.count[k];
-        a.class_cells[k] = cc.mixed ? ctx->ws.class_list + off : nullptr;
-        off += cc.count[k];
+        a.class_cells[k] = cc.mixed ? ctx->ws.class_list + (size_t)k * (size_t)ctx->max_n_cell : nullptr;
         blocks += (cc.count[k] + cells_per_block - 1) / cells_per_block;
         a.class_block_end[k] = blocks;
     }

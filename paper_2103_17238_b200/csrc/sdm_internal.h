@@ -22,6 +22,8 @@ constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
 
 // Largest cell the register-resident per-cell sort of the fast path handles (16 lanes x 16 or 32 lanes x 8 words).
 constexpr int CELL_FAST_MAX = 256;
+// Largest single-cell problem the one-block box step takes (sdm_box.cu).
+constexpr int BOX_MAX = 8192;
 // Cell-size classes of the fused kernel: class k = cells of at most 32 << k entries.
 constexpr int CELL_CLASSES = 4;
 
@@ -53,8 +55,7 @@ enum RunWord {
     RUN_ZC0 = 1,   // RUN_ZC0 + (s mod 3): zero multiplicities the array holds after step s of the run
     RUN_BOUNDS_TICKET = 4,  // k_cell_bounds: blocks finished (the last one publishes the verdict and resets it)
     RUN_BOUNDS_CLASS = 5,   // k_cell_bounds: worst cell-size class seen so far (reset by the last block)
-    RUN_CLASS_COUNT = 6,    // RUN_CLASS_COUNT + k - 1, k = 1..3: cells of size class k seen so far (reset by the last block)
-    RUN_LIST_CURSOR = 12,   // RUN_LIST_CURSOR + k, k = 0..3: k_class_lists' fill level of class k (zeroed by k_cell_bounds)
+    RUN_LIST_CURSOR = 12,   // RUN_LIST_CURSOR + k, k = 0..3: k_cell_classes' fill level of class k's list (reset by its last block)
     RUN_WORDS = 64
 };
 // Words of the pinned, device-mapped host status block: what the host must learn WITHOUT draining the stream.
@@ -64,7 +65,7 @@ enum MappedWord {
     MAPPED_VERDICT_EPOCH = 2,  // k_cell_bounds: epoch of the last published verdict
     MAPPED_VERDICT_CLASS = 3,  //   its worst cell-size class: 0 (<= 32), 1 (<= 64), 2 (<= 128), 3 (<= 256), 4 (larger,
                                //   or the array is not non-decreasing / holds an out-of-range cell_id)
-    MAPPED_CLASS_COUNT = 4,    //   MAPPED_CLASS_COUNT + k - 1, k = 1..3: number of cells of size class k
+    MAPPED_CLASS_COUNT = 4,    //   MAPPED_CLASS_COUNT + k, k = 0..3: number of cells of size class k
     MAPPED_WORDS = 16
 };
 // Sticky words (zeroed at init and by sdm_poll_error only).
@@ -81,7 +82,7 @@ struct Workspace {
     u32* sticky;      // STICKY_WORDS
     u32* run;         // RUN_WORDS
     u32* cell_start;  // max_n_cell + 1
-    u32* class_list;  // max_n_cell: cell ids grouped by size class (k_class_lists; mixed cell sizes only)
+    u32* class_list;  // CELL_CLASSES x max_n_cell: cell ids grouped by size class (k_cell_classes)
     u64* buf_a;       // max_n_sd
     u64* buf_b;       // max_n_sd
     u32* cmp_state;   // max compaction tiles
@@ -107,7 +108,7 @@ struct Plan {  // per-step derived quantities
 namespace sdm {
 // Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
 enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
-                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_DISPLACE, PROF_CLASSES };
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_DISPLACE, PROF_CELL_CLASSES, PROF_BOX_STEP, PROF_CLASSES };
 // What the last general-path step learned about the cell_id array (pinned host memory, written by an
 // asynchronous copy; valid once `verdict_event` has completed).
 struct Verdict { u32 unsorted; u32 max_count; };
@@ -213,7 +214,6 @@ cudaError_t launch_cell_digit_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t
 // sticky SDM_ERR_BAD_DATA (explicit paths); AUTO's analysis passes strict = false and falls back instead.
 cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int64_t n_sd, int32_t n_cell,
                                int idxbits, bool strict);
-cudaError_t launch_class_lists(sdm_ctx* ctx, int32_t n_cell, const u32 (&count)[CELL_CLASSES]);
 // Zero bookkeeping / halt protocol of one fused step (all nullable / 0: see FusedArgs in sdm_cellsort.cu).
 struct StepLinks {
     u32* zc_accum;
@@ -232,6 +232,9 @@ cudaError_t launch_cell_stats(sdm_ctx* ctx, const int64_t* xi, const double* v, 
                               int64_t n_sd, int32_t n_cell, int32_t* count, int64_t* sum_xi,
                               double* sum_xi_v, double* sum_xi_v2);
 cudaError_t init_cell_fused(sdm_ctx* ctx);       // per-device function attributes, once per context
+cudaError_t init_box_step(sdm_ctx* ctx);
+cudaError_t launch_box_step(sdm_ctx* ctx, int64_t* xi, double* v, int64_t n_sd, double dtdV, const KernelParams& kp,
+                            const PhiloxKeys& pk);
 cudaError_t init_volume_spectrum(sdm_ctx* ctx);
 cudaError_t launch_volume_spectrum(sdm_ctx* ctx, const int64_t* xi, const double* v, int64_t n_sd,
                                    const double* edges_dev, int32_t n_edges, int64_t* count, int64_t* sum_xi,

@@ -26,6 +26,7 @@ constexpr u32 FLAG_PREFIX = 2u << 30;  // inclusive prefix (with the global digi
 constexpr u32 VALUE_MASK = (1u << 30) - 1u;
 constexpr int SORT_WARPS = SORT_BLOCK / 32;
 constexpr int SORT_TILE_BITS = 12;
+constexpr int LOOK_WINDOW = 8;
 static_assert((1 << SORT_TILE_BITS) == SORT_TILE, "tile-local index width");
 static_assert(SORT_BLOCK == RADIX, "one thread per digit");
 
@@ -169,15 +170,25 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
     if (tile == 0) {
         gexcl = block_excl_scan_256(ghist[d_mine], s_warp, lane, warp);  // global digit base
     } else {
+        // a window of LOOK_WINDOW predecessors per round trip to L2 (the tiles of a launch wave publish their
+        // aggregates at about the same time, so the walk back to the nearest inclusive prefix is a dozen tiles long
+        // on average: one dependent load per tile made the walk the longest stall of the pass)
         gexcl = 0;
         int t = (int)tile - 1;
-        while (true) {
-            const u32 s = ld_relaxed_u32(tile_state + (size_t)t * RADIX + d_mine);
-            const u32 flag = s & ~VALUE_MASK;
-            if (flag == 0) continue;  // predecessor not published yet
-            gexcl += s & VALUE_MASK;
-            if (flag == FLAG_PREFIX) break;
-            --t;
+        bool done = false;
+        while (!done) {
+            u32 s[LOOK_WINDOW];
+#pragma unroll
+            for (int w = 0; w < LOOK_WINDOW; ++w)
+                s[w] = (t - w >= 0) ? ld_relaxed_u32(tile_state + (size_t)(t - w) * RADIX + d_mine) : 0u;
+#pragma unroll
+            for (int w = 0; w < LOOK_WINDOW; ++w) {
+                const u32 flag = s[w] & ~VALUE_MASK;
+                if (done || flag == 0) break;  // not published yet: poll again from this tile on
+                gexcl += s[w] & VALUE_MASK;
+                --t;
+                done = flag == FLAG_PREFIX;  // tile 0 always publishes its prefix: the walk ends there at the latest
+            }
         }
     }
     st_relaxed_u32(my_state, FLAG_PREFIX | (gexcl + total));

@@ -431,6 +431,36 @@ def test_ragged_sizes_single_cell(dev, n):
     _run_parity(w, dev, bit_exact=True)
 
 
+@pytest.mark.parametrize("n", [1, 2, 3, 33, 127, 128, 129, 1000, 4097, 8191, 8192])
+@pytest.mark.parametrize("kind", ["golovin", "geometric"])
+def test_box_step_one_block(dev, n, kind):
+    """SURVEY 8(f) NEXT-1, tiny N: the whole step of a one-cell box in one block (counting placement of the keys
+    instead of radix passes).  Permutation, every gamma and the state equal the oracle's, with and without debug
+    outputs, for every bucket count the launcher picks (32 ... 2048) and ragged tails."""
+    sdm = _sdm()
+    rng = np.random.default_rng(7 * n + len(kind))
+    if kind == "golovin":
+        xi = rng.integers(1, 50, n).astype(np.int64)
+        xi[rng.random(n) < 0.3] = 7
+        v = rng.integers(1, 9, n).astype(np.float64)
+        w = W.Workload("box", xi, v, np.zeros(n, np.int32), 1, 1.0, 1.0, W.GOLOVIN, 2.0 ** -8 / max(n, 1) * 64, 0.0, 4, 2)
+    else:
+        w0 = W.cfg1(n_sd=n, n_steps=4)
+        w = W.Workload("box", w0.xi, w0.v, w0.cell_id, 1, 1.0, w0.dV / 50.0, W.GEOMETRIC, 0.0, 1.0, 4, 0)
+    st = _run_parity(w, dev, path=sdm.PATH_BOX, bit_exact=True, expect_last_path=sdm.PATH_BOX)
+    _run_parity(w, dev, path=None, check_debug=False, bit_exact=True, expect_last_path=sdm.PATH_BOX)
+    if n >= 1000:
+        assert st["gamma_nonzero"] > 0
+
+
+def test_box_path_falls_back_to_general_when_it_does_not_fit(dev):
+    sdm = _sdm()
+    w = W.small("cfg1")          # 40 123 super-droplets in one cell: more than one block takes
+    _run_parity(w, dev, path=sdm.PATH_BOX, bit_exact=True, expect_last_path=sdm.PATH_GENERAL)
+    w = W.small("cfg3")          # many cells
+    _run_parity(w, dev, path=sdm.PATH_BOX, bit_exact=True, expect_last_path=sdm.PATH_GENERAL)
+
+
 @pytest.mark.parametrize("n,n_cell", [(5000, 3), (5000, 257), (9000, 70_000), (4096, 4096), (300, 1_000_000)])
 def test_cell_count_extremes(dev, n, n_cell):
     """few big cells, one more than a digit, more cells than SDs (mostly empty), 17+ cell bits."""
