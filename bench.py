@@ -5,7 +5,9 @@
 
 One "step" = one pass of the whole hot path over the workload: the coalescence step
 (Philox keys, cell boundaries / histograms, per-cell shuffle, fused pair kernel) followed, on the configuration's
-schedule, by the zero-multiplicity compaction ("compaction every step", configs[3]).  Default workload: configs[3]
+schedule, by the zero-multiplicity compaction ("compaction every step", configs[3]).  The dominant kernel of the
+default run is k_cell_fused (per-cell register sort fused with the pair rule: the CELL_SORTED path AUTO takes on
+cell-major input); the `paths` object times the literal north_star (b) path, the LSD radix sort (k_radix_pass).  Default workload: configs[3]
 (8,388,608 super-droplets, 256x256 cells, geometric kernel) -- the configuration BASELINE.json's metric and
 target are quoted on.  The steps go through the library's time-loop entry point sdm_coalescence_steps (the same
 bits as step-by-step calls, no host round trip per step); `--loop single` times the step-by-step calls instead.
@@ -314,7 +316,9 @@ class Runner:
         return ms, plan, sd_steps, self.ctx.launch_count() - launches0
 
     def kernel_profile(self, steps: int, loop: str, peak: float):
-        """The same steps again with a CUDA-event pair around every launch (sdm_profile_*)."""
+        """The same steps again with a CUDA-event pair around every launch (sdm_profile_*).  A box_step launch runs
+        many steps on a shared-memory copy of the state: its algorithmic HBM bytes are one read and one write of the
+        state per LAUNCH."""
         w, ctx = self.w, self.ctx
         k = min(steps, max(int(w.n_steps), 1))
         self.restore()

@@ -9,8 +9,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# SDM_B200_LIBRARY: another build of the same library (kernel tuning experiments); same C ABI, no fallback
-_LIB_PATH = os.environ.get("SDM_B200_LIBRARY") or os.path.join(_HERE, "libsdm_b200.so")
+_LIB_PATH = os.path.join(_HERE, "libsdm_b200.so")
 
 GOLOVIN = 0
 GEOMETRIC = 1

@@ -425,20 +425,28 @@ bool box_fits(const sdm_ctx* ctx, const StepArgs& A) {
     return A.n_cell == 1 && A.n_sd <= BOX_MAX && (ctx->path == SDM_PATH_AUTO || ctx->path == SDM_PATH_BOX);
 }
 
-int enqueue_box_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
+constexpr int64_t BOX_RUN_MAX = 4096;  // steps of one box launch (a few tens of milliseconds)
+
+// Steps step .. step + *n_steps - 1 of the box in one launch; with debug outputs bound (they describe ONE step) a
+// single step.  *n_steps returns the number of steps enqueued.
+int enqueue_box_steps(sdm_ctx* ctx, const StepArgs& A, uint64_t step, int64_t* n_steps) {
     int rc;
     if ((rc = clear_debug_gammas(ctx, A.n_sd))) return rc;
+    int64_t k = *n_steps < BOX_RUN_MAX ? *n_steps : BOX_RUN_MAX;
+    if (ctx->dbg_perm || ctx->dbg_gamma || ctx->dbg_gamma_clamped || ctx->dbg_cell_start) k = 1;
     const PhiloxKeys pk = make_philox_keys(A.seed, step, ctx->index_base);
     ctx->zero_hint_valid = 0;
     ctx->verdict_valid = 0;
-    if ((rc = note_cuda(ctx, launch_box_step(ctx, A.xi, A.v, A.n_sd, A.dtdV, A.dkp, pk)))) return rc;
+    if ((rc = note_cuda(ctx, launch_box_steps(ctx, A.xi, A.v, A.n_sd, A.dtdV, A.dkp, pk, k)))) return rc;
     ctx->last_path = SDM_PATH_BOX;
+    *n_steps = k;
     return SDM_OK;
 }
 
-// A step without the fused per-cell kernel: the one-block box step when it fits, else the GENERAL path.
+// One step without the fused per-cell kernel: the one-block box step when it fits, else the GENERAL path.
 int enqueue_unfused_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
-    return box_fits(ctx, A) ? enqueue_box_step(ctx, A, step) : enqueue_general_step(ctx, A, step);
+    int64_t one = 1;
+    return box_fits(ctx, A) ? enqueue_box_steps(ctx, A, step, &one) : enqueue_general_step(ctx, A, step);
 }
 
 // The index runs of the fused kernel: CELL_SORTED reads the arrays directly (kind 0); HYBRID gathers through the
@@ -759,7 +767,7 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
     ctx->zero_hint_valid = 0;
     int64_t n = n_sd;
     int64_t s = 0;
-    bool general_only = (n_cell <= 1) || ctx->path == SDM_PATH_GENERAL;
+    bool general_only = (n_cell <= 1) || ctx->path == SDM_PATH_GENERAL || ctx->path == SDM_PATH_BOX;
     while (s < n_steps && n > 0) {
         const StepArgs A = make_step_args(ctx, multiplicity, volume, cell_id, n, n_cell, dt, dV, kp, seed);
         const Plan plan = make_plan(n, n_cell, ctx->skip_key_digits);
@@ -795,8 +803,15 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
             // (cells of at most 256 super-droplets), and the loop comes back to try
             bool retry_fused = false;
             while (s < n_steps && !retry_fused) {
-                if ((rc = enqueue_unfused_step(ctx, A, step0 + (uint64_t)s))) return rc;
-                ++s;
+                if (box_fits(ctx, A)) {  // every step up to the next due compaction in one launch
+                    int64_t k = n_steps - s;
+                    if (compact_every > 0 && compact_every - (s % compact_every) < k) k = compact_every - (s % compact_every);
+                    if ((rc = enqueue_box_steps(ctx, A, step0 + (uint64_t)s, &k))) return rc;
+                    s += k;
+                } else {
+                    if ((rc = enqueue_general_step(ctx, A, step0 + (uint64_t)s))) return rc;
+                    ++s;
+                }
                 if (!general_only) {
                     Verdict hint;
                     if (auto_hint(ctx, A, &hint) && hint.max_count <= (u32)CELL_FAST_MAX && hint.unsorted &&

@@ -1,23 +1,25 @@
-// The whole coalescence step of a small box (one cell, n_sd <= BOX_MAX super-droplets) in ONE launch of ONE block
+// The coalescence steps of a small box (one cell, n_sd <= BOX_MAX super-droplets) in ONE launch of ONE block
 // ("includes the single-CTA fused step for tiny N"; configs[0], the paper's own box example,
 // PAPER.md:48-53, 73-75).  The GENERAL path needs five dependent launches for such a step and is bound by their
-// latencies (44 us per step for 8192 super-droplets); here rows a1, a3 and a4 run back to back out of shared memory:
+// latencies (44 us per step for 8192 super-droplets).  Here the state (multiplicities and volumes, 128 KB) is loaded
+// into shared memory once, any number of consecutive steps run out of shared memory, and the state is written back:
 //
 //   a1  every thread generates the Philox keys of its BOX_ITEMS super-droplets (kept in registers);
 //   a3  the keys are uniform 32-bit numbers, so a counting placement replaces the comparison network: bucket = the top
-//       key bits (about 4 super-droplets per bucket), one shared-memory atomic per super-droplet gives its slot
-//       inside the bucket, an exclusive scan of the bucket counts gives the bucket starts, the 46-bit words
-//       (key << 14 | index) are scattered to start + slot, and every word then finds its exact place by counting the
-//       smaller words of its own bucket.  The result is the ascending order of (key, index): the oracle's
-//       std::stable_sort order (ties between equal keys by index), for any key distribution -- a skewed one only
-//       makes the buckets longer;
+//       13 key bits (8192 buckets: about one super-droplet per bucket), one shared-memory atomic per super-droplet
+//       gives its slot inside the bucket, an exclusive scan of the bucket counts gives the bucket starts, the 32-bit
+//       words (low 19 key bits << 13 | index) are scattered to start + slot, and every word then finds its exact
+//       place by counting the smaller words of its own bucket.  The result is the ascending order of (key, index):
+//       the oracle's std::stable_sort order (ties between equal keys by index), for any key distribution -- a skewed
+//       one only makes the buckets longer;
 //   a4  thread t takes the pairs (2p, 2p + 1), p = t, t + 1024, ...: the same pair rule as every other path
-//       (pair_collide: exact early-out, Philox block of the first member regenerated).
+//       (pair_may_collide: exact early-out; pair_apply_to: the rule in fp64), the Philox block of the first member
+//       regenerated, the attributes read and written in shared memory.
 //
 // A single block cannot beat many SMs on bandwidth, but at this size nothing is bandwidth: the step is the sum of a
-// few shared-memory round trips.  An earlier attempt with a bitonic network over the 8192 words in shared memory (91
-// stages x 16 B per word) took 95-114 us (profiles/r1c_README.md); the counting placement touches every word a
-// handful of times.
+// few shared-memory round trips, and inside a run not even a kernel launch separates two steps (3.3 us each on this
+// host).  An earlier attempt with a bitonic network over the 8192 words in shared memory (91 stages x 16 B per word)
+// took 95-114 us (profiles/r1c_README.md); the counting placement touches every word a handful of times.
 #include "sdm_internal.h"
 #include "sdm_pair.cuh"
 
@@ -25,118 +27,154 @@ namespace sdm {
 
 constexpr int BOX_THREADS = 1024;
 constexpr int BOX_ITEMS = BOX_MAX / BOX_THREADS;  // super-droplets per thread
-constexpr int BOX_IDX_BITS = 14;
-constexpr int BOX_MAX_BUCKETS = 4096;
+constexpr int BOX_IDX_BITS = 13;
+constexpr int BOX_BUCKET_BITS = 13;               // one bucket per super-droplet of a full box: runs of 1-5 words
+constexpr int BOX_BUCKETS = 1 << BOX_BUCKET_BITS;
+constexpr int BOX_PER_THREAD = BOX_BUCKETS / BOX_THREADS;
+// inside a bucket the top 13 key bits agree, so the low 19 key bits above the 13-bit index order its members: the
+// words are 32 bits wide
 static_assert(BOX_MAX <= (1 << BOX_IDX_BITS) && BOX_ITEMS * BOX_THREADS == BOX_MAX, "box tile");
+static_assert(32 - BOX_BUCKET_BITS + BOX_IDX_BITS == 32, "bucket-local sort word fills 32 bits");
 
 struct BoxArgs {
-    PairArgs pair;
-    int bucket_shift;  // bucket = key >> bucket_shift
-    int n_bucket;      // 1 << (32 - bucket_shift), a multiple of 32, <= BOX_MAX_BUCKETS
+    PairArgs pair;    // pair.pk holds the first step; pair.xi / pair.v are the caller's arrays
+    u32 n_steps;      // consecutive steps of this launch (debug outputs: 1)
     int32_t* dbg_perm;
     int32_t* dbg_cell_start;
 };
 
-__global__ void __launch_bounds__(BOX_THREADS, 1) k_box_step(const __grid_constant__ BoxArgs a) {
-    extern __shared__ u64 s_words[];                  // [n_sd] (key << 14 | index), bucket by bucket
-    __shared__ u32 s_count[BOX_MAX_BUCKETS];          // bucket counts, then bucket starts
+__global__ void __launch_bounds__(BOX_THREADS, 1) k_box_steps(const __grid_constant__ BoxArgs a) {
+    extern __shared__ long long s_xi[];               // [n_sd] the multiplicities for the whole launch
+    __shared__ u32 s_count[BOX_BUCKETS];              // bucket counts, then bucket starts
     __shared__ u32 s_warp[BOX_THREADS / 32];
     const u32 n = a.pair.n_sd;
+    double* s_v = reinterpret_cast<double*>(s_xi + n);                       // [n_sd] the volumes
+    u32* s_words = reinterpret_cast<u32*>(s_v + n);                          // [n_sd] (low key bits << 13 | index), bucket by bucket
     unsigned short* s_idx = reinterpret_cast<unsigned short*>(s_words + n);  // [n_sd] indices in shuffled order
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int b = tid; b < a.n_bucket; b += BOX_THREADS) s_count[b] = 0u;
-    __syncthreads();
-    // ---- a1 + bucket histogram ----
-    u32 key[BOX_ITEMS], slot[BOX_ITEMS];
-#pragma unroll
-    for (int k = 0; k < BOX_ITEMS; ++k) {
-        const u32 i = (u32)tid + (u32)k * BOX_THREADS;
-        key[k] = philox_perm_key(a.pair.pk, (u64)i);  // computed for every slot: the chains of a thread interleave
-        slot[k] = 0;
-        if (i < n) slot[k] = atomicAdd(&s_count[key[k] >> a.bucket_shift], 1u);
+    for (u32 i = tid; i < n; i += BOX_THREADS) {
+        s_xi[i] = a.pair.xi[i];
+        s_v[i] = a.pair.v[i];
     }
-    __syncthreads();
-    // ---- exclusive scan of the bucket counts (n_bucket / 1024 consecutive buckets per thread, at most 4) ----
-    {
-        const int per = a.n_bucket / BOX_THREADS;  // 0 when there are fewer buckets than threads
-        u32 c[BOX_MAX_BUCKETS / BOX_THREADS];
-        u32 sum = 0;
-        if (per == 0) {
-            c[0] = tid < a.n_bucket ? s_count[tid] : 0u;
-            sum = c[0];
-        } else {
-#pragma unroll
-            for (int j = 0; j < BOX_MAX_BUCKETS / BOX_THREADS; ++j) {
-                c[j] = j < per ? s_count[tid * per + j] : 0u;
-                sum += c[j];
-            }
+    const u64 step0 = ((u64)a.pair.pk.step_hi << 32) | (u64)a.pair.pk.step_lo;
+    const bool dbg = a.pair.dbg_gamma != nullptr;
+    for (u32 s = 0; s < a.n_steps; ++s) {
+        const PhiloxStep ps = make_philox_step(step0 + (u64)s);
+        {
+            uint4* z = reinterpret_cast<uint4*>(s_count);
+            for (int b = tid; b < BOX_BUCKETS / 4; b += BOX_THREADS) z[b] = make_uint4(0u, 0u, 0u, 0u);
         }
-        u32 incl = sum;
+        __syncthreads();  // also: the previous step's pair phase (or the initial load) is complete
+        // ---- a1 + bucket histogram ----
+        u32 key[BOX_ITEMS], slot[BOX_ITEMS];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const u32 y = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += y;
+        for (int k = 0; k < BOX_ITEMS; ++k) {
+            const u32 i = (u32)tid + (u32)k * BOX_THREADS;
+            key[k] = philox4x32_10(a.pair.pk, ps, (u64)i).w0;  // computed for every slot: the chains of a thread interleave
+            slot[k] = 0;
+            if (i < n) slot[k] = atomicAdd(&s_count[key[k] >> (32 - BOX_BUCKET_BITS)], 1u);
         }
-        if (lane == 31) s_warp[warp] = incl;
         __syncthreads();
-        if (warp == 0) {
-            const u32 w = s_warp[lane];
-            u32 wi = w;
+        // ---- exclusive scan of the bucket counts (BOX_PER_THREAD consecutive buckets per thread) ----
+        {
+            u32 c[BOX_PER_THREAD];
+            u32 sum = 0;
+            const uint4* src = reinterpret_cast<const uint4*>(s_count + tid * BOX_PER_THREAD);
+#pragma unroll
+            for (int j = 0; j < BOX_PER_THREAD / 4; ++j) {
+                const uint4 q = src[j];
+                c[4 * j] = q.x; c[4 * j + 1] = q.y; c[4 * j + 2] = q.z; c[4 * j + 3] = q.w;
+                sum += q.x + q.y + q.z + q.w;
+            }
+            u32 incl = sum;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                const u32 y = __shfl_up_sync(0xffffffffu, wi, o);
-                if (lane >= o) wi += y;
+                const u32 y = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += y;
             }
-            s_warp[lane] = wi - w;
+            if (lane == 31) s_warp[warp] = incl;
+            __syncthreads();
+            if (warp == 0) {
+                const u32 w = s_warp[lane];
+                u32 wi = w;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const u32 y = __shfl_up_sync(0xffffffffu, wi, o);
+                    if (lane >= o) wi += y;
+                }
+                s_warp[lane] = wi - w;
+            }
+            __syncthreads();
+            u32 run = s_warp[warp] + incl - sum;
+            uint4* dst = reinterpret_cast<uint4*>(s_count + tid * BOX_PER_THREAD);
+#pragma unroll
+            for (int j = 0; j < BOX_PER_THREAD / 4; ++j) {
+                uint4 q;
+                q.x = run; run += c[4 * j];
+                q.y = run; run += c[4 * j + 1];
+                q.z = run; run += c[4 * j + 2];
+                q.w = run; run += c[4 * j + 3];
+                dst[j] = q;
+            }
         }
         __syncthreads();
-        u32 run = s_warp[warp] + incl - sum;
-        if (per == 0) {
-            if (tid < a.n_bucket) s_count[tid] = run;
-        } else {
+        // ---- scatter into the buckets (arrival order inside a bucket) ----
 #pragma unroll
-            for (int j = 0; j < BOX_MAX_BUCKETS / BOX_THREADS; ++j) {
-                if (j < per) s_count[tid * per + j] = run;
-                run += c[j];
+        for (int k = 0; k < BOX_ITEMS; ++k) {
+            const u32 i = (u32)tid + (u32)k * BOX_THREADS;
+            if (i < n) s_words[s_count[key[k] >> (32 - BOX_BUCKET_BITS)] + slot[k]] = (key[k] << BOX_IDX_BITS) | i;
+        }
+        __syncthreads();
+        // ---- exact place inside the bucket: the number of smaller words among its members ----
+#pragma unroll
+        for (int k = 0; k < BOX_ITEMS; ++k) {
+            const u32 i = (u32)tid + (u32)k * BOX_THREADS;
+            if (i < n) {
+                const u32 b = key[k] >> (32 - BOX_BUCKET_BITS);
+                const u32 mine = (key[k] << BOX_IDX_BITS) | i;
+                const u32 lo = s_count[b], hi = (b + 1 < (u32)BOX_BUCKETS) ? s_count[b + 1] : n;
+                u32 smaller = 0;
+                for (u32 q = lo; q < hi; ++q) smaller += (s_words[q] < mine);
+                s_idx[lo + smaller] = (unsigned short)i;
             }
         }
+        __syncthreads();
+        if (a.dbg_perm)
+            for (u32 p = tid; p < n; p += BOX_THREADS) a.dbg_perm[p] = (int32_t)s_idx[p];
+        // ---- a4: pairs of neighbours in the shuffled order, on the shared-memory copy of the state ----
+        for (u32 p = tid; 2u * p + 1u < n; p += BOX_THREADS) {
+            const u32 j0 = s_idx[2u * p], k0 = s_idx[2u * p + 1u];
+            const long long x0 = s_xi[j0], x1 = s_xi[k0];
+            const double v0 = s_v[j0], v1 = s_v[k0];
+            // a dead partner: gamma~ = 0 whatever gamma is (R7); only the debug gamma output needs the probability
+            if ((x0 == 0 || x1 == 0) && !dbg) continue;
+            const PhiloxOut w = philox4x32_10(a.pair.pk, ps, (u64)j0);  // uniform of the first-shuffled member (R2)
+            const bool swap = x0 < x1;
+            if (dbg || pair_may_collide(a.pair, swap ? x1 : x0, swap ? v1 : v0, swap ? v0 : v1, w.w2, w.w3, n))
+                pair_apply_to(a.pair, s_xi, s_v, j0, k0, x0, v0, x1, v1, w.w2, w.w3, n);
+        }
+        // (the next step's first barrier orders these writes before its reads)
     }
     __syncthreads();
-    // ---- scatter into the buckets (arrival order inside a bucket) ----
-#pragma unroll
-    for (int k = 0; k < BOX_ITEMS; ++k) {
-        const u32 i = (u32)tid + (u32)k * BOX_THREADS;
-        if (i < n) s_words[s_count[key[k] >> a.bucket_shift] + slot[k]] = ((u64)key[k] << BOX_IDX_BITS) | (u64)i;
+    for (u32 i = tid; i < n; i += BOX_THREADS) {
+        a.pair.xi[i] = s_xi[i];
+        a.pair.v[i] = s_v[i];
     }
-    __syncthreads();
-    // ---- exact place inside the bucket: the number of smaller words among its members ----
-    // (a thread takes the words at positions tid, tid + 1024, ...: neighbouring lanes sit in the same or in
-    //  neighbouring buckets, so a warp's loops are about equally long)
-    for (u32 p = tid; p < n; p += BOX_THREADS) {
-        const u64 mine = s_words[p];
-        const u32 b = (u32)(mine >> (BOX_IDX_BITS + a.bucket_shift));
-        const u32 lo = s_count[b], hi = (b + 1 < (u32)a.n_bucket) ? s_count[b + 1] : n;
-        u32 smaller = 0;
-        for (u32 q = lo; q < hi; ++q) smaller += (s_words[q] < mine);
-        s_idx[lo + smaller] = (unsigned short)(mine & ((1u << BOX_IDX_BITS) - 1u));
-    }
-    __syncthreads();
-    if (a.dbg_perm)
-        for (u32 p = tid; p < n; p += BOX_THREADS) a.dbg_perm[p] = (int32_t)s_idx[p];
     if (a.dbg_cell_start && tid == 0) {
         a.dbg_cell_start[0] = 0;
         a.dbg_cell_start[1] = (int32_t)n;
     }
-    // ---- a4: pairs of neighbours in the shuffled order ----
-    for (u32 p = tid; 2u * p + 1u < n; p += BOX_THREADS) pair_collide(a.pair, (u32)s_idx[2u * p], (u32)s_idx[2u * p + 1u], n);
 }
+
+constexpr size_t BOX_SMEM_PER_SD = 8 + 8 + 4 + 2;  // xi, v, sort word, shuffled index
 
 cudaError_t init_box_step(sdm_ctx*) {
-    return cudaFuncSetAttribute(k_box_step, cudaFuncAttributeMaxDynamicSharedMemorySize, BOX_MAX * 10);
+    return cudaFuncSetAttribute(k_box_steps, cudaFuncAttributeMaxDynamicSharedMemorySize, BOX_MAX * BOX_SMEM_PER_SD);
 }
 
-cudaError_t launch_box_step(sdm_ctx* ctx, int64_t* xi, double* v, int64_t n_sd, double dtdV, const KernelParams& kp,
-                            const PhiloxKeys& pk) {
+// `pk` carries the first step; steps step .. step + n_steps - 1 run back to back inside the launch.
+cudaError_t launch_box_steps(sdm_ctx* ctx, int64_t* xi, double* v, int64_t n_sd, double dtdV, const KernelParams& kp,
+                             const PhiloxKeys& pk, int64_t n_steps) {
     BoxArgs a;
     a.pair.sorted = nullptr;
     a.pair.xi = reinterpret_cast<long long*>(xi);
@@ -152,15 +190,11 @@ cudaError_t launch_box_step(sdm_ctx* ctx, int64_t* xi, double* v, int64_t n_sd, 
     a.pair.pk = pk;
     a.pair.dbg_gamma = reinterpret_cast<long long*>(ctx->dbg_gamma);
     a.pair.dbg_gamma_clamped = reinterpret_cast<long long*>(ctx->dbg_gamma_clamped);
-    // about four super-droplets per bucket; at least one warp's worth of buckets
-    int bits = 5;
-    while ((1 << bits) * 4 < n_sd && (1 << bits) < BOX_MAX_BUCKETS) ++bits;
-    a.bucket_shift = 32 - bits;
-    a.n_bucket = 1 << bits;
+    a.n_steps = (u32)n_steps;
     a.dbg_perm = ctx->dbg_perm;
     a.dbg_cell_start = ctx->dbg_cell_start;
     LaunchScope scope(ctx, PROF_BOX_STEP);
-    k_box_step<<<1, BOX_THREADS, (size_t)n_sd * 10, ctx->stream>>>(a);
+    k_box_steps<<<1, BOX_THREADS, (size_t)n_sd * BOX_SMEM_PER_SD, ctx->stream>>>(a);
     return cudaGetLastError();
 }
 

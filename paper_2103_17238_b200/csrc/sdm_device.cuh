@@ -46,14 +46,29 @@ struct PhiloxOut {
     u32 w0, w1, w2, w3;
 };
 
-__device__ __forceinline__ PhiloxOut philox4x32_10(const PhiloxKeys& pk, u64 i) {
+// The step-dependent words of the block: counter words 2, 3 = the step, and 0xCD9E8D57 * lo32(step), the first
+// round's second product, which is the same for every super-droplet.
+struct PhiloxStep {
+    u32 step_hi, p1_lo, p1_hi;
+};
+__host__ __device__ inline PhiloxStep make_philox_step(u64 step) {
+    const u64 p1 = (u64)0xCD9E8D57u * (u64)(u32)step;
+    PhiloxStep s;
+    s.step_hi = (u32)(step >> 32);
+    s.p1_lo = (u32)p1;
+    s.p1_hi = (u32)(p1 >> 32);
+    return s;
+}
+
+// `ps` overrides the step stored in `pk` (kernels that loop over steps themselves); the round keys come from `pk`.
+__device__ __forceinline__ PhiloxOut philox4x32_10(const PhiloxKeys& pk, const PhiloxStep& ps, u64 i) {
     i += pk.index_base;
-    u32 c0 = (u32)i, c1 = (u32)(i >> 32), c2, c3 = pk.step_hi;
-    {  // round 0: the counter words 2, 3 are the step, so 0xCD9E8D57 * c2 comes precomputed from the host
+    u32 c0 = (u32)i, c1 = (u32)(i >> 32), c2, c3 = ps.step_hi;
+    {  // round 0: the counter words 2, 3 are the step, so 0xCD9E8D57 * c2 comes precomputed
         const u64 p0 = (u64)0xD2511F53u * (u64)c0;
-        const u32 n0 = pk.p1_hi ^ c1 ^ pk.k0[0];
+        const u32 n0 = ps.p1_hi ^ c1 ^ pk.k0[0];
         c2 = (u32)(p0 >> 32) ^ c3 ^ pk.k1[0];
-        c1 = pk.p1_lo;
+        c1 = ps.p1_lo;
         c3 = (u32)p0;
         c0 = n0;
     }
@@ -71,6 +86,14 @@ __device__ __forceinline__ PhiloxOut philox4x32_10(const PhiloxKeys& pk, u64 i) 
     PhiloxOut o;
     o.w0 = c0; o.w1 = c1; o.w2 = c2; o.w3 = c3;
     return o;
+}
+
+__device__ __forceinline__ PhiloxOut philox4x32_10(const PhiloxKeys& pk, u64 i) {
+    PhiloxStep ps;
+    ps.step_hi = pk.step_hi;
+    ps.p1_lo = pk.p1_lo;
+    ps.p1_hi = pk.p1_hi;
+    return philox4x32_10(pk, ps, i);
 }
 
 // Permutation key only (word 0).

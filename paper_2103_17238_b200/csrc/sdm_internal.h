@@ -5,6 +5,7 @@
 #include <cstdint>
 #include <vector>
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>  // header-only; a no-op unless a profiler is attached
 
 #include "../../include/sdm.h"
 #include "sdm_device.cuh"
@@ -171,13 +172,23 @@ struct sdm_ctx {
 
 namespace sdm {
 
-// RAII bracket around one kernel launch: counts it and, when profiling is on, records a CUDA-event pair
-// on the launching stream.
+// NVTX range names of the kernel classes (tracing): same order as ProfClass.
+inline const char* prof_class_name(int cls) {
+    static const char* const names[PROF_CLASSES] = {
+        "sdm:keys_hist", "sdm:cell_scan", "sdm:radix_pass", "sdm:pair", "sdm:count_zero", "sdm:compact", "sdm:cell_stats",
+        "sdm:other", "sdm:cell_bounds", "sdm:cell_fused", "sdm:cell_digit_hist", "sdm:tie_repair", "sdm:volume_spectrum",
+        "sdm:displace", "sdm:cell_classes", "sdm:box_steps"};
+    return (cls >= 0 && cls < PROF_CLASSES) ? names[cls] : "sdm:?";
+}
+
+// RAII bracket around one kernel launch: counts it, opens an NVTX range named after the kernel class (visible in
+// Nsight Systems / Compute timelines) and, when profiling is on, records a CUDA-event pair on the launching stream.
 struct LaunchScope {
     sdm_ctx* ctx;
     cudaEvent_t stop;
     LaunchScope(sdm_ctx* c, int cls) : ctx(c), stop(nullptr) {
         ctx->launches++;
+        nvtxRangePushA(prof_class_name(cls));
         if (!ctx->profiling) return;
         if (ctx->prof_used == ctx->prof_events->size()) {
             ProfEvent e;
@@ -191,6 +202,7 @@ struct LaunchScope {
     }
     ~LaunchScope() {
         if (stop) cudaEventRecord(stop, ctx->stream);
+        nvtxRangePop();
     }
 };
 
@@ -233,8 +245,8 @@ cudaError_t launch_cell_stats(sdm_ctx* ctx, const int64_t* xi, const double* v, 
                               double* sum_xi_v, double* sum_xi_v2);
 cudaError_t init_cell_fused(sdm_ctx* ctx);       // per-device function attributes, once per context
 cudaError_t init_box_step(sdm_ctx* ctx);
-cudaError_t launch_box_step(sdm_ctx* ctx, int64_t* xi, double* v, int64_t n_sd, double dtdV, const KernelParams& kp,
-                            const PhiloxKeys& pk);
+cudaError_t launch_box_steps(sdm_ctx* ctx, int64_t* xi, double* v, int64_t n_sd, double dtdV, const KernelParams& kp,
+                             const PhiloxKeys& pk, int64_t n_steps);
 cudaError_t init_volume_spectrum(sdm_ctx* ctx);
 cudaError_t launch_volume_spectrum(sdm_ctx* ctx, const int64_t* xi, const double* v, int64_t n_sd,
                                    const double* edges_dev, int32_t n_edges, int64_t* count, int64_t* sum_xi,

@@ -133,8 +133,10 @@ __device__ __forceinline__ bool pair_may_collide(const PairArgs& a, long long xj
 // The whole rule for one pair, exactly.  (j0, k0) = original indices in shuffled order, (x0, v0) / (x1, v1)
 // their pre-step attributes, (w2, w3) the Philox words of j0's uniform (R2).  Returns the number of
 // super-droplets whose multiplicity became 0 (the split of xi_k = 1, R14).
-__device__ __forceinline__ u32 pair_apply(const PairArgs& a, u32 j0, u32 k0, long long x0, double v0, long long x1,
-                                          double v1, u32 w2, u32 w3, u32 n_c) {
+// `xi`, `v`: where the state lives (the caller's arrays, or a shared-memory copy of them).
+__device__ __forceinline__ u32 pair_apply_to(const PairArgs& a, long long* __restrict__ xi, double* __restrict__ v, u32 j0,
+                                             u32 k0, long long x0, double v0, long long x1, double v1, u32 w2, u32 w3,
+                                             u32 n_c) {
     long long xj = x0, xk = x1;
     double vj = v0, vk = v1;
     u32 j = j0, k = k0;
@@ -163,20 +165,25 @@ __device__ __forceinline__ u32 pair_apply(const PairArgs& a, u32 j0, u32 k0, lon
         const double vnew = __dadd_rn(__dmul_rn((double)gt, vj), vk);
         const long long rem = xj - gt * xk;
         if (rem > 0) {
-            a.xi[j] = rem;
-            a.v[k] = vnew;
+            xi[j] = rem;
+            v[k] = vnew;
         } else {  // equal-multiplicity split (R14)
             const long long h = xk / 2;
-            a.xi[j] = h;
-            a.xi[k] = xk - h;
-            a.v[j] = vnew;
-            a.v[k] = vnew;
+            xi[j] = h;
+            xi[k] = xk - h;
+            v[j] = vnew;
+            v[k] = vnew;
             new_zeros = (h == 0);
         }
     }
     if (a.dbg_gamma) a.dbg_gamma[j0] = g;
     if (a.dbg_gamma_clamped) a.dbg_gamma_clamped[j0] = gt;
     return new_zeros;
+}
+
+__device__ __forceinline__ u32 pair_apply(const PairArgs& a, u32 j0, u32 k0, long long x0, double v0, long long x1,
+                                          double v1, u32 w2, u32 w3, u32 n_c) {
+    return pair_apply_to(a, a.xi, a.v, j0, k0, x0, v0, x1, v1, w2, w3, n_c);
 }
 
 // General pair kernel: gathers the attributes, regenerates j0's Philox block, runs both phases.
