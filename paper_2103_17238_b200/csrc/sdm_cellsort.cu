@@ -573,25 +573,10 @@ cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int6
     return cudaGetLastError();
 }
 
-// The staging tiles want the shared-memory end of the L1 split.  The attribute is per device and per function:
-// it is set once per context (contexts live on one device) for every instantiation, and the result is checked.
-template <int KIND, int HYB, int R>
-static cudaError_t prefer_shared_carveout() {
-    return cudaFuncSetAttribute(k_cell_fused<KIND, HYB, R>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                cudaSharedmemCarveoutMaxShared);
-}
-
-cudaError_t init_cell_fused(sdm_ctx*) {
-    cudaError_t e;
-#define SDM_CARVE(R)                                                              \
-    if ((e = prefer_shared_carveout<0, 0, R>()) != cudaSuccess) return e;         \
-    if ((e = prefer_shared_carveout<0, 1, R>()) != cudaSuccess) return e;         \
-    if ((e = prefer_shared_carveout<1, 0, R>()) != cudaSuccess) return e;         \
-    if ((e = prefer_shared_carveout<1, 1, R>()) != cudaSuccess) return e;
-    SDM_CARVE(4) SDM_CARVE(8)
-#undef SDM_CARVE
-    return cudaSuccess;
-}
+// No shared-memory carve-out preference is set for the fused kernel: it needs 6-12 KB per block, and with the L1
+// squeezed to its minimum (the round-1 setting) a warp's scattered gathers on the HYBRID path ran out of lines to
+// allocate for pending misses -- 444 us instead of 178 us on interleaved configs[3] (profiles/r2b_README.md).
+cudaError_t init_cell_fused(sdm_ctx*) { return cudaSuccess; }
 
 template <int R>
 static void launch_fused_r(const FusedArgs& a, bool hybrid, u32 grid, cudaStream_t st) {
