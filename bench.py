@@ -42,7 +42,7 @@ METRIC = "super-droplet-steps/s per coalescence step; achieved HBM GB/s vs B200 
 UNIT = "SD-steps/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 L2_BYTES = 126e6
-PATH_NAMES = {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid", 4: "box_one_block"}
+PATH_NAMES = {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid", 4: "box_one_block", 5: "bucket_msd_placement"}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -102,6 +102,7 @@ def algorithmic_bytes(n_cell: int):
         "tie_repair": 8,                             # read the sorted words (rewrites only tied runs)
         "volume_spectrum": 16,
         "cell_classes": 0,                           # reads cell_start (n_cell words)
+        "bucket": 4,                                 # hist: one reduction per SD; scatter: one 4-byte index word per SD
         "box_step": 32,                              # read xi,v 16 + write xi,v 16 (one block, keys regenerated)
     }
 

@@ -92,16 +92,24 @@ int sdm_set_collision_efficiency(sdm_ctx* ctx, const double* radius /* host */, 
  *                NEXT-1 "single-CTA fused step for tiny N"): the whole step -- keys, shuffle by counting placement of
  *                the uniform keys, pair rule -- in one launch of one block out of shared memory.  Chosen explicitly
  *                on an input that does not fit, the step takes the GENERAL path.
+ *   BUCKET       one cell of up to 2^23 super-droplets (configs[1]: a box of 2^20): the Philox keys are uniform, so a
+ *                two-level counting placement by their bits replaces the LSD passes -- coarse buckets of 1024-2048
+ *                entries by the top bits (histogram and scatter with block-local counting), then one block per
+ *                coarse bucket orders it exactly by (key, index) in shared memory the way the BOX step does -- and
+ *                the GENERAL path's pair kernel follows.  A coarse bucket of more than 4096 entries (twice the
+ *                largest average: it does not happen) would raise the sticky SDM_ERR_BAD_DATA.  Chosen explicitly on
+ *                an input that does not fit (several cells, more than 2^23 entries), the step takes the GENERAL path.
  *   AUTO         (default) never refuses valid input.  Every step first analyses cell_id on the device (one
  *                streaming read: range, order, largest cell) and the host waits for that verdict -- a few
  *                microseconds, through a mapped status word, without draining work enqueued behind it -- before
  *                it enqueues either the fused kernel (CELL_SORTED when the array is non-decreasing, HYBRID when the
  *                previous GENERAL step on the same array saw small cells in any order), the BOX step (one small
- *                cell) or the GENERAL path.  So
+ *                cell), the BUCKET path (one large cell) or the GENERAL path.  So
  *                cell_id may be rewritten in place between steps (a displacement step does exactly that): the
  *                next step simply takes the path that fits.  sdm_coalescence_steps pays the analysis once per
  *                call instead of once per step.  sdm_set_path() forgets what was learned. */
-typedef enum { SDM_PATH_AUTO = 0, SDM_PATH_GENERAL = 1, SDM_PATH_CELL_SORTED = 2, SDM_PATH_HYBRID = 3, SDM_PATH_BOX = 4 } sdm_path;
+typedef enum { SDM_PATH_AUTO = 0, SDM_PATH_GENERAL = 1, SDM_PATH_CELL_SORTED = 2, SDM_PATH_HYBRID = 3, SDM_PATH_BOX = 4,
+               SDM_PATH_BUCKET = 5 } sdm_path;
 
 /* Bytes of device workspace sdm_init() needs for problems up to (max_n_sd, max_n_cell).
  * Returns 0 when the arguments are invalid (max_n_sd < 0, max_n_sd >= 2^30, max_n_cell < 1). */
@@ -236,9 +244,12 @@ int sdm_set_path(sdm_ctx* ctx, int path);
  * SDM_OPT_FUSED_WORDS_PER_LANE (0 = automatic (default), 4, 8): sort words per lane of the fused per-cell
  * kernel's group sort (a cell of at most 32 << k entries is sorted by (32 << k) / R lanes).  A tuning / test knob:
  * every value gives the same bits; 4 cannot serve cells of more than 128 entries and then falls back to 8.
+ * SDM_OPT_BUCKET_BITS (0 = automatic (default), 1..12): coarse key bits of the BUCKET path's placement (2^bits
+ * buckets; automatic: the fewest bits that leave at most 2048 entries per bucket on average).  A test knob: every
+ * value whose buckets stay within 4096 entries gives the same bits.
  * Returns INVALID_ARG for an unknown option or value. */
 enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1, SDM_OPT_INDEX_BASE = 2, SDM_OPT_SKIP_KEY_DIGITS = 3,
-       SDM_OPT_FUSED_WORDS_PER_LANE = 4 };
+       SDM_OPT_FUSED_WORDS_PER_LANE = 4, SDM_OPT_BUCKET_BITS = 5 };
 int sdm_set_option(sdm_ctx* ctx, int option, int64_t value);
 
 /* Which path the most recent step took (an sdm_path value other than AUTO), or 0 if none ran yet.  Host-side
@@ -272,7 +283,7 @@ int64_t sdm_launch_count(sdm_ctx* ctx);
 enum { SDM_PROF_KEYS_HIST = 0, SDM_PROF_CELL_SCAN, SDM_PROF_RADIX_PASS, SDM_PROF_PAIR, SDM_PROF_COUNT_ZERO,
        SDM_PROF_COMPACT, SDM_PROF_CELL_STATS, SDM_PROF_OTHER, SDM_PROF_CELL_BOUNDS, SDM_PROF_CELL_FUSED,
        SDM_PROF_CELL_DIGIT_HIST, SDM_PROF_TIE_REPAIR, SDM_PROF_SPECTRUM, SDM_PROF_DISPLACE, SDM_PROF_CELL_CLASSES,
-       SDM_PROF_BOX_STEP, SDM_PROF_CLASSES };
+       SDM_PROF_BOX_STEP, SDM_PROF_BUCKET, SDM_PROF_CLASSES };
 int sdm_profile_enable(sdm_ctx* ctx, int on);
 int sdm_profile_read(sdm_ctx* ctx, double* ms_out /* host */, int64_t* launches_out /* host */);
 

@@ -19,11 +19,13 @@ PATH_GENERAL = 1
 PATH_CELL_SORTED = 2
 PATH_HYBRID = 3
 PATH_BOX = 4
+PATH_BUCKET = 5
 OPT_NARROW_KEY_BITS = 0
 OPT_TRACK_ZEROS = 1
 OPT_INDEX_BASE = 2
 OPT_SKIP_KEY_DIGITS = 3
 OPT_FUSED_WORDS_PER_LANE = 4
+OPT_BUCKET_BITS = 5
 
 SDM_OK = 0
 
@@ -37,7 +39,7 @@ EXPORTS = [
 ]
 
 PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
-                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum", "displace", "cell_classes", "box_step"]
+                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum", "displace", "cell_classes", "box_step", "bucket"]
 
 
 class SDMError(RuntimeError):

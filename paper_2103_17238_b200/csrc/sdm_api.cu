@@ -67,8 +67,10 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     w.tile_state = reinterpret_cast<u32*>(take((size_t)MAX_PASSES * max_tiles * RADIX * 4));
     w.cell_start = reinterpret_cast<u32*>(take(((size_t)max_n_cell + 2) * 4));
     w.class_list = reinterpret_cast<u32*>(take((size_t)CELL_CLASSES * (size_t)max_n_cell * 4));
+    w.bucket_count = reinterpret_cast<u32*>(take(((size_t)1 << BUCKET_MAX_BITS) * 4));
     w.buf_a = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
-    w.buf_b = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16));
+    // also the bucket slabs of the BUCKET path: 2^cb x (2 x average + 64) 4-byte words <= 8 n + 2^BUCKET_MAX_BITS x 264 bytes
+    w.buf_b = reinterpret_cast<u64*>(take((size_t)max_n_sd * 8 + 16 + ((size_t)512 << BUCKET_MAX_BITS)));
     w.cmp_state = reinterpret_cast<u32*>(take(cmp_tiles * 4));
     w.spec_edges = reinterpret_cast<double*>(take((size_t)SPECTRUM_MAX_EDGES * 8));
     w.eff_radius = reinterpret_cast<double*>(take((size_t)EFF_MAX_R * 8));
@@ -166,7 +168,7 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
         cudaEventCreateWithFlags(&ctx->verdict_event, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->chunk_event[0], cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->chunk_event[1], cudaEventDisableTiming) != cudaSuccess ||
-        init_cell_fused(ctx) != cudaSuccess || init_box_step(ctx) != cudaSuccess ||
+        init_cell_fused(ctx) != cudaSuccess || init_box_step(ctx) != cudaSuccess || init_bucket_path(ctx) != cudaSuccess ||
         init_volume_spectrum(ctx) != cudaSuccess) {
         free_ctx(ctx);
         return SDM_ERR_CUDA;
@@ -221,7 +223,7 @@ const char* sdm_strerror(int status) {
 }
 
 int sdm_set_path(sdm_ctx* ctx, int path) {
-    if (!ctx || path < SDM_PATH_AUTO || path > SDM_PATH_BOX) return SDM_ERR_INVALID_ARG;
+    if (!ctx || path < SDM_PATH_AUTO || path > SDM_PATH_BUCKET) return SDM_ERR_INVALID_ARG;
     ctx->path = path;
     ctx->verdict_valid = 0;  // AUTO re-learns the cell order on its next step
     return SDM_OK;
@@ -243,6 +245,10 @@ int sdm_set_option(sdm_ctx* ctx, int option, int64_t value) {
     }
     if (option == SDM_OPT_FUSED_WORDS_PER_LANE && (value == 0 || value == 4 || value == 8)) {
         ctx->fused_r = (int)value;
+        return SDM_OK;
+    }
+    if (option == SDM_OPT_BUCKET_BITS && value >= 0 && value <= BUCKET_MAX_BITS) {
+        ctx->bucket_bits_opt = (int)value;
         return SDM_OK;
     }
     if (option == SDM_OPT_TRACK_ZEROS && (value == 0 || value == 1)) {
@@ -443,10 +449,40 @@ int enqueue_box_steps(sdm_ctx* ctx, const StepArgs& A, uint64_t step, int64_t* n
     return SDM_OK;
 }
 
-// One step without the fused per-cell kernel: the one-block box step when it fits, else the GENERAL path.
+// BUCKET path: one cell too large for the box step -- two-level counting placement by the key bits, then the pair
+// kernel (sdm_bucket.cu).  AUTO takes it for every single cell above BOX_MAX that the placement can hold (at most 2048
+// entries per coarse bucket on average: 2^23 super-droplets).
+bool bucket_fits(const sdm_ctx* ctx, const StepArgs& A) {
+    if (A.n_cell != 1 || A.n_sd < 1 || A.n_sd > ((int64_t)2048 << BUCKET_MAX_BITS)) return false;
+    if (bucket_fine_bits(A.n_sd, bucket_bits(A.n_sd, ctx->bucket_bits_opt)) == 0) return false;
+    return ctx->path == SDM_PATH_BUCKET || (ctx->path == SDM_PATH_AUTO && A.n_sd > BOX_MAX);
+}
+
+int enqueue_bucket_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
+    int rc;
+    cudaStream_t st = ctx->stream;
+    Workspace& ws = ctx->ws;
+    const Plan plan = make_plan(A.n_sd, 1, ctx->skip_key_digits);  // idxbits of the pair kernel's words
+    const int cb = bucket_bits(A.n_sd, ctx->bucket_bits_opt);
+    if ((rc = clear_debug_gammas(ctx, A.n_sd))) return rc;
+    const PhiloxKeys pk = make_philox_keys(A.seed, step, ctx->index_base);
+    ctx->verdict_valid = 0;
+    ctx->zero_hint_valid = 0;
+    if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.bucket_count, 0, ((size_t)1 << cb) * 4, st)))) return rc;
+    if ((rc = note_cuda(ctx, launch_bucket_shuffle(ctx, A.n_sd, cb, pk, ws.buf_a)))) return rc;
+    if (ctx->dbg_perm)
+        if ((rc = note_cuda(ctx, launch_debug_perm(ctx, ws.buf_a, A.n_sd, plan)))) return rc;
+    if ((rc = note_cuda(ctx, launch_pair(ctx, ws.buf_a, A.xi, A.v, A.n_sd, 1, plan, A.dtdV, A.dkp, pk)))) return rc;
+    ctx->last_path = SDM_PATH_BUCKET;
+    return SDM_OK;
+}
+
+// One step without the per-cell analysis: the one-block box step or the bucket path when they fit, else GENERAL.
 int enqueue_unfused_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
     int64_t one = 1;
-    return box_fits(ctx, A) ? enqueue_box_steps(ctx, A, step, &one) : enqueue_general_step(ctx, A, step);
+    if (box_fits(ctx, A)) return enqueue_box_steps(ctx, A, step, &one);
+    if (bucket_fits(ctx, A)) return enqueue_bucket_step(ctx, A, step);
+    return enqueue_general_step(ctx, A, step);
 }
 
 // The index runs of the fused kernel: CELL_SORTED reads the arrays directly (kind 0); HYBRID gathers through the
@@ -767,7 +803,7 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
     ctx->zero_hint_valid = 0;
     int64_t n = n_sd;
     int64_t s = 0;
-    bool general_only = (n_cell <= 1) || ctx->path == SDM_PATH_GENERAL || ctx->path == SDM_PATH_BOX;
+    bool general_only = (n_cell <= 1) || ctx->path == SDM_PATH_GENERAL || ctx->path == SDM_PATH_BOX || ctx->path == SDM_PATH_BUCKET;
     while (s < n_steps && n > 0) {
         const StepArgs A = make_step_args(ctx, multiplicity, volume, cell_id, n, n_cell, dt, dV, kp, seed);
         const Plan plan = make_plan(n, n_cell, ctx->skip_key_digits);
@@ -809,7 +845,7 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
                     if ((rc = enqueue_box_steps(ctx, A, step0 + (uint64_t)s, &k))) return rc;
                     s += k;
                 } else {
-                    if ((rc = enqueue_general_step(ctx, A, step0 + (uint64_t)s))) return rc;
+                    if ((rc = enqueue_unfused_step(ctx, A, step0 + (uint64_t)s))) return rc;
                     ++s;
                 }
                 if (!general_only) {

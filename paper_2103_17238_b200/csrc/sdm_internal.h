@@ -23,6 +23,8 @@ constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
 
 // Largest cell the register-resident per-cell sort of the fast path handles (16 lanes x 16 or 32 lanes x 8 words).
 constexpr int CELL_FAST_MAX = 256;
+// Most coarse key bits of the BUCKET path's placement (sdm_bucket.cu): 4096 buckets of at most 2048 entries on average.
+constexpr int BUCKET_MAX_BITS = 12;
 // Largest single-cell problem the one-block box step takes (sdm_box.cu).
 constexpr int BOX_MAX = 8192;
 // Cell-size classes of the fused kernel: class k = cells of at most 32 << k entries.
@@ -84,6 +86,7 @@ struct Workspace {
     u32* run;         // RUN_WORDS
     u32* cell_start;  // max_n_cell + 1
     u32* class_list;  // CELL_CLASSES x max_n_cell: cell ids grouped by size class (k_cell_classes)
+    u32* bucket_count;  // BUCKET path: 2^BUCKET_MAX_BITS coarse-bucket fill counts (zeroed per step)
     u64* buf_a;       // max_n_sd
     u64* buf_b;       // max_n_sd
     u32* cmp_state;   // max compaction tiles
@@ -109,7 +112,7 @@ struct Plan {  // per-step derived quantities
 namespace sdm {
 // Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
 enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
-                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_DISPLACE, PROF_CELL_CLASSES, PROF_BOX_STEP, PROF_CLASSES };
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_DISPLACE, PROF_CELL_CLASSES, PROF_BOX_STEP, PROF_BUCKET, PROF_CLASSES };
 // What the last general-path step learned about the cell_id array (pinned host memory, written by an
 // asynchronous copy; valid once `verdict_event` has completed).
 struct Verdict { u32 unsorted; u32 max_count; };
@@ -145,6 +148,7 @@ struct sdm_ctx {
     int skip_key_digits;  // SDM_OPT_SKIP_KEY_DIGITS (-1 = automatic)
     int narrow_key_bits;  // key bits kept in the fused kernel's 32-bit sort word (SDM_OPT_NARROW_KEY_BITS)
     int fused_r;          // words per lane of the fused kernel's group sort (SDM_OPT_FUSED_WORDS_PER_LANE; 0 = automatic)
+    int bucket_bits_opt;  // key bits of the BUCKET path's placement (SDM_OPT_BUCKET_BITS; 0 = automatic)
     // optional per-launch CUDA-event timing (sdm_profile_enable)
     int profiling;
     std::vector<sdm::ProfEvent>* prof_events;
@@ -177,7 +181,7 @@ inline const char* prof_class_name(int cls) {
     static const char* const names[PROF_CLASSES] = {
         "sdm:keys_hist", "sdm:cell_scan", "sdm:radix_pass", "sdm:pair", "sdm:count_zero", "sdm:compact", "sdm:cell_stats",
         "sdm:other", "sdm:cell_bounds", "sdm:cell_fused", "sdm:cell_digit_hist", "sdm:tie_repair", "sdm:volume_spectrum",
-        "sdm:displace", "sdm:cell_classes", "sdm:box_steps"};
+        "sdm:displace", "sdm:cell_classes", "sdm:box_steps", "sdm:bucket"};
     return (cls >= 0 && cls < PROF_CLASSES) ? names[cls] : "sdm:?";
 }
 
@@ -213,6 +217,10 @@ Plan make_plan(int64_t n_sd, int32_t n_cell, int skip_key_digits /* -1 = choose 
 cudaError_t launch_keys_hist(sdm_ctx* ctx, const int32_t* cell_id, int64_t n_sd, int32_t n_cell,
                              const Plan& plan, const PhiloxKeys& pk, u64* sortkey_out);
 cudaError_t launch_cell_scan(sdm_ctx* ctx, int32_t n_cell, int64_t n_sd);
+int bucket_bits(int64_t n_sd, int bits_override);
+int bucket_fine_bits(int64_t n_sd, int cb);
+cudaError_t init_bucket_path(sdm_ctx* ctx);
+cudaError_t launch_bucket_shuffle(sdm_ctx* ctx, int64_t n_sd, int cb, const PhiloxKeys& pk, u64* sorted);
 cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, int64_t n_sd,
                              const Plan& plan);
 cudaError_t launch_pair(sdm_ctx* ctx, const u64* sorted, int64_t* xi, double* v, int64_t n_sd,

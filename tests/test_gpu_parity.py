@@ -52,7 +52,7 @@ def _assert_vol_close(got, want, what=""):
 
 
 def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key_bits=None, expect_last_path=None,
-                track_zeros=False, skip_key_digits=None, fused_r=None):
+                track_zeros=False, skip_key_digits=None, fused_r=None, bucket_bits=None):
     """Steps the oracle and the GPU side by side over w.n_steps steps, comparing after every step."""
     sdm = _sdm()
     ow = w.copy()
@@ -68,6 +68,8 @@ def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key
             ctx.set_option(sdm.OPT_SKIP_KEY_DIGITS, skip_key_digits)
         if fused_r is not None:
             ctx.set_option(sdm.OPT_FUSED_WORDS_PER_LANE, fused_r)
+        if bucket_bits is not None:
+            ctx.set_option(sdm.OPT_BUCKET_BITS, bucket_bits)
         xi, v, cell = _to_dev(w, dev)
         dbg = ctx.debug_outputs(n, w.n_cell) if check_debug else None
         okp, gkp = _okp(w), _gkp(w)
@@ -451,6 +453,54 @@ def test_box_step_one_block(dev, n, kind):
     _run_parity(w, dev, path=None, check_debug=False, bit_exact=True, expect_last_path=sdm.PATH_BOX)
     if n >= 1000:
         assert st["gamma_nonzero"] > 0
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 64, 129, 1000, 4097, 8193, 40_123, 300_001])
+@pytest.mark.parametrize("kind", ["golovin", "geometric"])
+@pytest.mark.parametrize("bits", [0, 1, 3])
+def test_bucket_path_single_cell(dev, n, kind, bits):
+    """One cell in key buckets (two-level counting placement + the pair kernel): the permutation, every gamma and the
+    state equal the oracle's for every coarse bucket count (bits: 0 = automatic, else that many more key bits than
+    automatic: few entries in many buckets, empty buckets), ragged sizes and both kernels."""
+    sdm = _sdm()
+    rng = np.random.default_rng(11 * n + len(kind))
+    if kind == "golovin":
+        xi = rng.integers(1, 50, n).astype(np.int64)
+        xi[rng.random(n) < 0.3] = 7
+        v = rng.integers(1, 9, n).astype(np.float64)
+        w = W.Workload("box", xi, v, np.zeros(n, np.int32), 1, 1.0, 1.0, W.GOLOVIN, 2.0 ** -8 / max(n, 1) * 64, 0.0, 4, 2)
+    else:
+        w0 = W.cfg1(n_sd=n, n_steps=4)
+        w = W.Workload("box", w0.xi, w0.v, w0.cell_id, 1, 1.0, w0.dV / 50.0, W.GEOMETRIC, 0.0, 1.0, 4, 0)
+    auto_bits = 1
+    while auto_bits < 12 and (2048 << auto_bits) < n:
+        auto_bits += 1
+    opts = {} if bits == 0 else {"bucket_bits": min(auto_bits + 3 * bits, 12)}
+    st = _run_parity(w, dev, path=sdm.PATH_BUCKET, bit_exact=True, expect_last_path=sdm.PATH_BUCKET, **opts)
+    _run_parity(w, dev, path=sdm.PATH_BUCKET, check_debug=False, bit_exact=True, track_zeros=True, **opts)
+    if n >= 1000:
+        assert st["gamma_nonzero"] > 0
+
+
+def test_auto_takes_the_bucket_path_for_a_large_single_cell(dev):
+    sdm = _sdm()
+    _run_parity(W.small("cfg1"), dev, path=None, bit_exact=True, expect_last_path=sdm.PATH_BUCKET)
+    _run_parity(W.small("cfg3"), dev, path=sdm.PATH_BUCKET, bit_exact=True, expect_last_path=sdm.PATH_GENERAL)
+
+
+def test_bucket_overflow_is_reported(dev):
+    """A coarse bucket of more than 4096 entries cannot happen with the automatic bucket count (twice the largest
+    average); forced with two key bits on 20 000 super-droplets it is reported, not silently mishandled."""
+    sdm = _sdm()
+    n = 20_000
+    with sdm.SDMContext(n, 1, device=dev) as ctx:
+        ctx.set_path(sdm.PATH_BUCKET)
+        ctx.set_option(sdm.OPT_BUCKET_BITS, 2)
+        xi = torch.full((n,), 5, dtype=torch.int64, device=dev)
+        v = torch.ones(n, dtype=torch.float64, device=dev)
+        cell = torch.zeros(n, dtype=torch.int32, device=dev)
+        ctx.coalescence_step(xi, v, cell, 1, 1.0, 1.0, sdm.golovin(1e-3), 42, 0)
+        assert ctx.poll_error() == -4
 
 
 def test_box_path_falls_back_to_general_when_it_does_not_fit(dev):
