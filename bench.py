@@ -251,7 +251,7 @@ class Runner:
         self.ctx = sdm.SDMContext(max(w.n_sd, 1), w.n_cell, device=dev, host_staging=host_staging)
         if path:
             self.ctx.set_path({"auto": sdm.PATH_AUTO, "general": sdm.PATH_GENERAL, "cell_sorted": sdm.PATH_CELL_SORTED,
-                               "hybrid": sdm.PATH_HYBRID}[path])
+                               "hybrid": sdm.PATH_HYBRID, "box": sdm.PATH_BOX, "bucket": sdm.PATH_BUCKET}[path])
         if index_base:
             self.ctx.set_option(sdm.OPT_INDEX_BASE, index_base)
         if track_zeros:
@@ -586,7 +586,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
-    ap.add_argument("--path", default=None, choices=[None, "auto", "general", "cell_sorted", "hybrid"])
+    ap.add_argument("--path", default=None, choices=[None, "auto", "general", "cell_sorted", "hybrid", "box", "bucket"])
     ap.add_argument("--loop", default="multi", choices=["multi", "single"],
                     help="multi: sdm_coalescence_steps (default); single: one sdm_coalescence_step (+ compaction) call per step")
     ap.add_argument("--quick", action="store_true", help="headline only: skip the `paths` and `configs` objects")
