@@ -707,6 +707,51 @@ def test_multi_step_entry_interleaved_auto_and_resume(dev):
     _run_multi(W.small("cfg0"), dev, None, 40, 0, chunks=(1, 39))
 
 
+@pytest.mark.parametrize("n,path", [(3000, "box"), (8192, "box"), (20_000, "bucket"), (20_000, "general")])
+@pytest.mark.parametrize("compact_every", [0, 1, 4])
+def test_single_cell_time_loop_with_zeros(dev, n, path, compact_every):
+    """One cell whose multiplicities are small (1 .. 3): equal-multiplicity splits produce zeros all the time.  The
+    time loop on the BOX path (many steps inside one launch, cut at every due compaction), the BUCKET path and the
+    GENERAL path equals oracle.run for every compaction schedule, and the array really shrinks."""
+    sdm = _sdm()
+    rng = np.random.default_rng(n + compact_every)
+    xi = rng.integers(1, 4, n).astype(np.int64)
+    v = rng.integers(1, 9, n).astype(np.float64)
+    w = W.Workload("box", xi, v, np.zeros(n, np.int32), 1, 1.0, 1.0, W.GOLOVIN, 0.5 / n, 0.0, 12, compact_every)
+    p = {"box": sdm.PATH_BOX, "bucket": sdm.PATH_BUCKET, "general": sdm.PATH_GENERAL}[path]
+    n_out, last = _run_multi(w, dev, p, 12, compact_every)
+    assert last == p
+    if compact_every:
+        assert n_out < n
+    _run_multi(w, dev, None, 12, compact_every, chunks=(4, 8))      # AUTO, resumed
+
+
+@pytest.mark.parametrize("n,path", [(5000, "box"), (30_000, "bucket")])
+def test_single_cell_paths_honour_index_base_and_the_table_kernel(dev, n, path):
+    """SDM_OPT_INDEX_BASE (R34) and SDM_KERNEL_GEOMETRIC_TABLE (R39) on the single-cell paths: the same bits as the
+    oracle with the same counter offset / table."""
+    sdm = _sdm()
+    p = {"box": sdm.PATH_BOX, "bucket": sdm.PATH_BUCKET}[path]
+    w0 = W.cfg1(n_sd=n, n_steps=3)
+    radius = np.array([1e-6, 2e-5, 1e-4, 2e-3])
+    table = np.array([[0.1, 0.3, 0.2], [0.5, 0.9, 0.7], [1.0, 0.8, 1.2], [0.6, 1.1, 0.4]])
+    base = 7_000_000_123
+    with sdm.SDMContext(n, 1, device=dev) as ctx:
+        ctx.set_path(p)
+        ctx.set_option(sdm.OPT_INDEX_BASE, base)
+        ctx.set_collision_efficiency(radius, table)
+        xi, v, cell = _to_dev(w0, dev)
+        ow = w0.copy()
+        okp = oracle.geometric_table(radius, table)
+        for s in range(3):
+            ctx.coalescence_step(xi, v, cell, 1, 1.0, w0.dV / 200.0, sdm.geometric_table(), 42, s)
+            oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, 1, 1.0, w0.dV / 200.0, okp, 42, s, index_base=base)
+        assert ctx.poll_error() == 0 and ctx.last_path() == p
+        assert np.array_equal(xi.cpu().numpy(), ow.xi)
+        assert np.array_equal(v.cpu().numpy().view(np.int64), ow.v.view(np.int64))
+        assert np.count_nonzero(ow.xi != w0.xi) > 0
+
+
 def test_multi_step_entry_edge_cases(dev):
     sdm = _sdm()
     w = W.small("cfg3")
