@@ -247,9 +247,11 @@ int sdm_set_path(sdm_ctx* ctx, int path);
  * SDM_OPT_BUCKET_BITS (0 = automatic (default), 1..12): coarse key bits of the BUCKET path's placement (2^bits
  * buckets; automatic: the fewest bits that leave at most 2048 entries per bucket on average).  A test knob: every
  * value whose buckets stay within 4096 entries gives the same bits.
+ * SDM_OPT_BOX_CLUSTER (0 / 1, default 1): the BOX path on a thread-block cluster of eight blocks (distributed shared
+ * memory) or on one block.  Same bits either way.
  * Returns INVALID_ARG for an unknown option or value. */
 enum { SDM_OPT_NARROW_KEY_BITS = 0, SDM_OPT_TRACK_ZEROS = 1, SDM_OPT_INDEX_BASE = 2, SDM_OPT_SKIP_KEY_DIGITS = 3,
-       SDM_OPT_FUSED_WORDS_PER_LANE = 4, SDM_OPT_BUCKET_BITS = 5 };
+       SDM_OPT_FUSED_WORDS_PER_LANE = 4, SDM_OPT_BUCKET_BITS = 5, SDM_OPT_BOX_CLUSTER = 6 };
 int sdm_set_option(sdm_ctx* ctx, int option, int64_t value);
 
 /* Which path the most recent step took (an sdm_path value other than AUTO), or 0 if none ran yet.  Host-side

@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     OPT_SKIP_KEY_DIGITS,
     OPT_FUSED_WORDS_PER_LANE,
     OPT_BUCKET_BITS,
+    OPT_BOX_CLUSTER,
     KernelParams,
     SDMContext,
     SDMError,
@@ -35,6 +36,6 @@ from .binding import (  # noqa: F401
 
 __all__ = [
     "SDMContext", "SDMError", "KernelParams", "golovin", "geometric", "geometric_table", "GOLOVIN", "GEOMETRIC", "GEOMETRIC_TABLE",
-    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "PATH_BOX", "PATH_BUCKET", "OPT_NARROW_KEY_BITS", "OPT_TRACK_ZEROS", "OPT_INDEX_BASE", "OPT_SKIP_KEY_DIGITS", "OPT_FUSED_WORDS_PER_LANE", "OPT_BUCKET_BITS", "workspace_bytes", "host_staging_bytes",
+    "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "PATH_BOX", "PATH_BUCKET", "OPT_NARROW_KEY_BITS", "OPT_TRACK_ZEROS", "OPT_INDEX_BASE", "OPT_SKIP_KEY_DIGITS", "OPT_FUSED_WORDS_PER_LANE", "OPT_BUCKET_BITS", "OPT_BOX_CLUSTER", "workspace_bytes", "host_staging_bytes",
     "load_library", "library_path",
 ]

@@ -26,6 +26,7 @@ OPT_INDEX_BASE = 2
 OPT_SKIP_KEY_DIGITS = 3
 OPT_FUSED_WORDS_PER_LANE = 4
 OPT_BUCKET_BITS = 5
+OPT_BOX_CLUSTER = 6
 
 SDM_OK = 0
 

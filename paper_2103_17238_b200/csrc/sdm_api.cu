@@ -152,6 +152,7 @@ int sdm_init(sdm_ctx** out, int device, int64_t max_n_sd, int32_t max_n_cell, vo
     ctx->ws = carve_workspace(workspace_dev, max_n_sd, max_n_cell);
     ctx->path = SDM_PATH_AUTO;
     ctx->narrow_key_bits = 24;
+    ctx->box_cluster = 1;
     ctx->skip_key_digits = -1;
     ctx->epoch = 2;
     int sms = 0;
@@ -245,6 +246,10 @@ int sdm_set_option(sdm_ctx* ctx, int option, int64_t value) {
     }
     if (option == SDM_OPT_FUSED_WORDS_PER_LANE && (value == 0 || value == 4 || value == 8)) {
         ctx->fused_r = (int)value;
+        return SDM_OK;
+    }
+    if (option == SDM_OPT_BOX_CLUSTER && (value == 0 || value == 1)) {
+        ctx->box_cluster = (int)value;
         return SDM_OK;
     }
     if (option == SDM_OPT_BUCKET_BITS && value >= 0 && value <= BUCKET_MAX_BITS) {

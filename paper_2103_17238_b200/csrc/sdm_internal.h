@@ -149,6 +149,7 @@ struct sdm_ctx {
     int narrow_key_bits;  // key bits kept in the fused kernel's 32-bit sort word (SDM_OPT_NARROW_KEY_BITS)
     int fused_r;          // words per lane of the fused kernel's group sort (SDM_OPT_FUSED_WORDS_PER_LANE; 0 = automatic)
     int bucket_bits_opt;  // key bits of the BUCKET path's placement (SDM_OPT_BUCKET_BITS; 0 = automatic)
+    int box_cluster;      // BOX path on a cluster of eight blocks (SDM_OPT_BOX_CLUSTER; default 1) or on one block
     // optional per-launch CUDA-event timing (sdm_profile_enable)
     int profiling;
     std::vector<sdm::ProfEvent>* prof_events;

@@ -130,20 +130,22 @@ __device__ __forceinline__ bool pair_may_collide(const PairArgs& a, long long xj
     return unsure || !(u_lo >= p_ub);
 }
 
-// The whole rule for one pair, exactly.  (j0, k0) = original indices in shuffled order, (x0, v0) / (x1, v1)
-// their pre-step attributes, (w2, w3) the Philox words of j0's uniform (R2).  Returns the number of
+// The whole rule for one pair, exactly.  (j0, k0) = original indices in shuffled order, (x0, v0) / (x1, v1) their pre-step
+// attributes, (w2, w3) the Philox words of j0's uniform (R2).  (px0, pv0) / (px1, pv1): where the attributes of j0 / k0
+// live (the caller's arrays, a shared-memory copy, or another block's shared memory).  Returns the number of
 // super-droplets whose multiplicity became 0 (the split of xi_k = 1, R14).
-// `xi`, `v`: where the state lives (the caller's arrays, or a shared-memory copy of them).
-__device__ __forceinline__ u32 pair_apply_to(const PairArgs& a, long long* __restrict__ xi, double* __restrict__ v, u32 j0,
-                                             u32 k0, long long x0, double v0, long long x1, double v1, u32 w2, u32 w3,
+__device__ __forceinline__ u32 pair_apply_at(const PairArgs& a, long long* px0, double* pv0, long long* px1, double* pv1,
+                                             u32 j0, long long x0, double v0, long long x1, double v1, u32 w2, u32 w3,
                                              u32 n_c) {
     long long xj = x0, xk = x1;
     double vj = v0, vk = v1;
-    u32 j = j0, k = k0;
+    long long *pxj = px0, *pxk = px1;
+    double *pvj = pv0, *pvk = pv1;
     if (xj < xk) {  // order so that xi_j >= xi_k; ties keep the shuffled order (R8)
         xj = x1; xk = x0;
         vj = v1; vk = v0;
-        j = k0; k = j0;
+        pxj = px1; pxk = px0;
+        pvj = pv1; pvk = pv0;
     }
     const double u = uniform_from_words(w2, w3);
     const double K = coalescence_kernel(a.kp, vj, vk);
@@ -165,20 +167,27 @@ __device__ __forceinline__ u32 pair_apply_to(const PairArgs& a, long long* __res
         const double vnew = __dadd_rn(__dmul_rn((double)gt, vj), vk);
         const long long rem = xj - gt * xk;
         if (rem > 0) {
-            xi[j] = rem;
-            v[k] = vnew;
+            *pxj = rem;
+            *pvk = vnew;
         } else {  // equal-multiplicity split (R14)
             const long long h = xk / 2;
-            xi[j] = h;
-            xi[k] = xk - h;
-            v[j] = vnew;
-            v[k] = vnew;
+            *pxj = h;
+            *pxk = xk - h;
+            *pvj = vnew;
+            *pvk = vnew;
             new_zeros = (h == 0);
         }
     }
     if (a.dbg_gamma) a.dbg_gamma[j0] = g;
     if (a.dbg_gamma_clamped) a.dbg_gamma_clamped[j0] = gt;
     return new_zeros;
+}
+
+// `xi`, `v`: arrays indexed by the original index (the caller's arrays, or a shared-memory copy of them).
+__device__ __forceinline__ u32 pair_apply_to(const PairArgs& a, long long* __restrict__ xi, double* __restrict__ v, u32 j0,
+                                             u32 k0, long long x0, double v0, long long x1, double v1, u32 w2, u32 w3,
+                                             u32 n_c) {
+    return pair_apply_at(a, xi + j0, v + j0, xi + k0, v + k0, j0, x0, v0, x1, v1, w2, w3, n_c);
 }
 
 __device__ __forceinline__ u32 pair_apply(const PairArgs& a, u32 j0, u32 k0, long long x0, double v0, long long x1,

@@ -52,7 +52,7 @@ def _assert_vol_close(got, want, what=""):
 
 
 def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key_bits=None, expect_last_path=None,
-                track_zeros=False, skip_key_digits=None, fused_r=None, bucket_bits=None):
+                track_zeros=False, skip_key_digits=None, fused_r=None, bucket_bits=None, box_cluster=None):
     """Steps the oracle and the GPU side by side over w.n_steps steps, comparing after every step."""
     sdm = _sdm()
     ow = w.copy()
@@ -70,6 +70,8 @@ def _run_parity(w, dev, path=None, check_debug=True, bit_exact=False, narrow_key
             ctx.set_option(sdm.OPT_FUSED_WORDS_PER_LANE, fused_r)
         if bucket_bits is not None:
             ctx.set_option(sdm.OPT_BUCKET_BITS, bucket_bits)
+        if box_cluster is not None:
+            ctx.set_option(sdm.OPT_BOX_CLUSTER, box_cluster)
         xi, v, cell = _to_dev(w, dev)
         dbg = ctx.debug_outputs(n, w.n_cell) if check_debug else None
         okp, gkp = _okp(w), _gkp(w)
@@ -433,12 +435,14 @@ def test_ragged_sizes_single_cell(dev, n):
     _run_parity(w, dev, bit_exact=True)
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 33, 127, 128, 129, 1000, 4097, 8191, 8192])
+@pytest.mark.parametrize("n", [1, 2, 3, 33, 127, 128, 129, 1000, 1024, 1025, 2049, 4097, 8191, 8192])
 @pytest.mark.parametrize("kind", ["golovin", "geometric"])
-def test_box_step_one_block(dev, n, kind):
-    """SURVEY 8(f) NEXT-1, tiny N: the whole step of a one-cell box in one block (counting placement of the keys
-    instead of radix passes).  Permutation, every gamma and the state equal the oracle's, with and without debug
-    outputs, for every bucket count the launcher picks (32 ... 2048) and ragged tails."""
+@pytest.mark.parametrize("box_cluster", [1, 0])
+def test_box_step_one_block(dev, n, kind, box_cluster):
+    """SURVEY 8(f) NEXT-1, tiny N: the whole step of a one-cell box in one launch (counting placement of the keys
+    instead of radix passes), on a cluster of eight blocks with the state in distributed shared memory and on one
+    block.  Permutation, every gamma and the state equal the oracle's, with and without debug outputs, for ragged
+    sizes around the per-block share of 1024."""
     sdm = _sdm()
     rng = np.random.default_rng(7 * n + len(kind))
     if kind == "golovin":
@@ -449,8 +453,8 @@ def test_box_step_one_block(dev, n, kind):
     else:
         w0 = W.cfg1(n_sd=n, n_steps=4)
         w = W.Workload("box", w0.xi, w0.v, w0.cell_id, 1, 1.0, w0.dV / 50.0, W.GEOMETRIC, 0.0, 1.0, 4, 0)
-    st = _run_parity(w, dev, path=sdm.PATH_BOX, bit_exact=True, expect_last_path=sdm.PATH_BOX)
-    _run_parity(w, dev, path=None, check_debug=False, bit_exact=True, expect_last_path=sdm.PATH_BOX)
+    st = _run_parity(w, dev, path=sdm.PATH_BOX, bit_exact=True, expect_last_path=sdm.PATH_BOX, box_cluster=box_cluster)
+    _run_parity(w, dev, path=None, check_debug=False, bit_exact=True, expect_last_path=sdm.PATH_BOX, box_cluster=box_cluster)
     if n >= 1000:
         assert st["gamma_nonzero"] > 0
 
