@@ -42,7 +42,7 @@ METRIC = "super-droplet-steps/s per coalescence step; achieved HBM GB/s vs B200 
 UNIT = "SD-steps/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 L2_BYTES = 126e6
-PATH_NAMES = {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid", 4: "box_one_block", 5: "bucket_msd_placement"}
+PATH_NAMES = {1: "general_lsd_radix", 2: "cell_sorted", 3: "hybrid", 4: "box_cluster", 5: "bucket_msd_placement"}
 
 
 # ------------------------------------------------------------------------------------------------
