@@ -199,6 +199,12 @@ struct __align__(16) BoxState {
 // GOLOVIN: the kernel kind as a compile-time constant -- the pair rule of a Golovin box then carries none of the
 // geometric kernel's code (cube roots, fall speeds, efficiency table); with ONE pair per thread and step the fetch of
 // that straight-line code, not its execution, was most of the pair phase.
+// Cluster barrier with release / acquire at cluster scope (the phases only exchange data through the cluster's
+// shared memory): cooperative_groups' cluster.sync() adds a GPU-scope fence and an L1 invalidation to every barrier.
+__device__ __forceinline__ void cluster_barrier() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
 template <bool GOLOVIN>
 __global__ void __cluster_dims__(BC_CLUSTER, 1, 1) __launch_bounds__(BC_THREADS, 1)
 k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
@@ -228,7 +234,7 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
     const bool dbg = a.pair.dbg_gamma != nullptr;
     PairArgs pa = a.pair;  // (only the fields the pair rule reads are materialised)
     if (GOLOVIN) pa.kp.kind = 0;
-    cluster.sync();
+    cluster_barrier();
     for (u32 s = 0; s < a.n_steps; ++s) {
         const PhiloxStep ps = make_philox_step(step0 + (u64)s);
         // ---- a1 + rank among the block's entries of the bucket ----
@@ -236,7 +242,7 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
         const u32 gb = key >> (32 - BOX_BUCKET_BITS);  // bucket 0 .. 8191; its owner is gb >> 10
         u32 slot = 0;
         if (i < n) slot = atomicAdd(&s_hist[gb], 1u);
-        cluster.sync();
+        cluster_barrier();
         // ---- owner side: the eight blocks' counts of my bucket, scan of the totals, starts back to the sources ----
         {
             const u32 g = rank * BC_THREADS + (u32)tid;
@@ -275,7 +281,7 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
                 run += c[b];
             }
         }
-        cluster.sync();
+        cluster_barrier();
         // ---- scatter into the owner's buckets; everybody learns every block's total ----
         if (tid < BC_CLUSTER) s_tot[tid] = *cluster.map_shared_rank(&s_total, tid);
         if (i < n) {
@@ -283,7 +289,7 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
             if (pos < (u32)BC_CAP) cluster.map_shared_rank(s_words, gb / BC_THREADS)[pos] = (key << BOX_IDX_BITS) | i;
             else sticky[STICKY_BAD_DATA] = 1u;  // cannot happen: twice the average in one eighth of the key range
         }
-        cluster.sync();
+        cluster_barrier();
         // ---- exact order inside my bucket (about one word): place = number of smaller words ----
         const u32 total = min(s_tot[rank], (u32)BC_CAP);
         {
@@ -295,7 +301,7 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
                 s_idx[lo + smaller] = (unsigned short)(mine & ((1u << BOX_IDX_BITS) - 1u));
             }
         }
-        cluster.sync();
+        cluster_barrier();
         // ---- a4: the pairs whose first member is one of this block's shuffled positions ----
         u32 first = 0;  // global shuffled position of the block's first word
         for (u32 r = 0; r < rank; ++r) first += s_tot[r];
@@ -329,7 +335,7 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
             uint4* z = reinterpret_cast<uint4*>(s_hist);
             for (int q = tid; q < BOX_BUCKETS / 4; q += BC_THREADS) z[q] = make_uint4(0u, 0u, 0u, 0u);
         }
-        cluster.sync();
+        cluster_barrier();
     }
     if (i < n) {
         a.pair.xi[i] = s_state[tid].xi;
