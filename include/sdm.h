@@ -90,7 +90,8 @@ int sdm_set_collision_efficiency(sdm_ctx* ctx, const double* radius /* host */, 
  *                (it fixes the launch geometry) without draining the stream.
  *   BOX          one cell of at most 8192 super-droplets (the paper's box example; SURVEY 8(f)
  *                NEXT-1 "single-CTA fused step for tiny N"): the whole step -- keys, shuffle by counting placement of
- *                the uniform keys, pair rule -- in one launch of one block out of shared memory.  Chosen explicitly
+ *                the uniform keys, pair rule -- for any number of consecutive steps in one launch of a cluster of eight
+ *                blocks (or of one block, SDM_OPT_BOX_CLUSTER) out of (distributed) shared memory.  Chosen explicitly
  *                on an input that does not fit, the step takes the GENERAL path.
  *   BUCKET       one cell of up to 2^23 super-droplets (configs[1]: a box of 2^20): the Philox keys are uniform, so a
  *                two-level counting placement by their bits replaces the LSD passes -- coarse buckets of 1024-2048

@@ -431,7 +431,7 @@ int enqueue_general_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
     return SDM_OK;
 }
 
-// BOX path: a single cell of at most BOX_MAX super-droplets, the whole step in one launch of one block.
+// BOX path: a single cell of at most BOX_MAX super-droplets, whole steps inside one launch (one cluster or one block).
 bool box_fits(const sdm_ctx* ctx, const StepArgs& A) {
     return A.n_cell == 1 && A.n_sd <= BOX_MAX && (ctx->path == SDM_PATH_AUTO || ctx->path == SDM_PATH_BOX);
 }
@@ -482,7 +482,7 @@ int enqueue_bucket_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
     return SDM_OK;
 }
 
-// One step without the per-cell analysis: the one-block box step or the bucket path when they fit, else GENERAL.
+// One step without the per-cell analysis: the box step or the bucket path when they fit, else GENERAL.
 int enqueue_unfused_step(sdm_ctx* ctx, const StepArgs& A, uint64_t step) {
     int64_t one = 1;
     if (box_fits(ctx, A)) return enqueue_box_steps(ctx, A, step, &one);

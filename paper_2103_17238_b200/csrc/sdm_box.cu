@@ -1,4 +1,5 @@
-// The coalescence steps of a small box (one cell, n_sd <= BOX_MAX super-droplets) in ONE launch of ONE block
+// The coalescence steps of a small box (one cell, n_sd <= BOX_MAX super-droplets) in ONE launch: of one block
+// (k_box_steps, described first) or of a cluster of eight blocks (k_box_cluster, further down: the default)
 // ("includes the single-CTA fused step for tiny N"; configs[0], the paper's own box example,
 // PAPER.md:48-53, 73-75).  The GENERAL path needs five dependent launches for such a step and is bound by their
 // latencies (44 us per step for 8192 super-droplets).  Here the state (multiplicities and volumes, 128 KB) is loaded

@@ -25,7 +25,7 @@ constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
 constexpr int CELL_FAST_MAX = 256;
 // Most coarse key bits of the BUCKET path's placement (sdm_bucket.cu): 4096 buckets of at most 2048 entries on average.
 constexpr int BUCKET_MAX_BITS = 12;
-// Largest single-cell problem the one-block box step takes (sdm_box.cu).
+// Largest single-cell problem the box step takes (sdm_box.cu).
 constexpr int BOX_MAX = 8192;
 // Cell-size classes of the fused kernel: class k = cells of at most 32 << k entries.
 constexpr int CELL_CLASSES = 4;
