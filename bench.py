@@ -477,7 +477,7 @@ def run_ours(args):
     e_ms, e_units = aggregate_over_ranks(e0.elapsed_time(e1), float(sd_e), dist, dev)
     e2e = {"value": e_units / (e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 20 * n0,
            "d2h_bytes_per_step": 16 * n0 + 8, "steps": e_steps,
-           "api": "sdm_coalescence_step_host (pinned host buffers, compaction included)"}
+           "api": "sdm_coalescence_step_host (pinned host buffers, compaction included; uploads, step and downloads pipelined in eight pieces)"}
     del hxi, hv, hc
 
     # ---- product call outside the step: the volume spectrum on 31 log bins over the state ----

@@ -261,7 +261,12 @@ int sdm_last_path(sdm_ctx* ctx);
 
 /* End-to-end variant with HOST buffers (bench.py `e2e`): copies multiplicity, volume and cell_id to the
  * device staging area bound with sdm_bind_host_staging(), runs sdm_coalescence_step there, copies
- * multiplicity and volume back, and synchronises.  Host buffers should be pinned for full PCIe speed. */
+ * multiplicity and volume back, and synchronises.  Host buffers should be pinned for full PCIe speed.
+ * Cell-major arrays of at least 2^18 entries whose cells are small and of nearly one size (configs[2], [3]) go through
+ * a pipeline under AUTO: cell_id is uploaded and analysed as a whole, the attributes travel in eight pieces cut at cell
+ * boundaries on a stream of their own, the fused kernel runs on the cells of a piece as soon as it has arrived, and
+ * the piece returns on a third stream while the next one is arriving -- PCIe carries both directions at once.  Same
+ * bits; every other input takes the plain sequence upload, step, download. */
 size_t sdm_host_staging_bytes(int64_t max_n_sd);
 int sdm_bind_host_staging(sdm_ctx* ctx, void* staging_dev, size_t staging_bytes);
 /* With compact != 0 the step is followed by sdm_remove_zero_multiplicity on the staged arrays; the

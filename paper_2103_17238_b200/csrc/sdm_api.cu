@@ -1,6 +1,7 @@
 // The C ABI of libsdm_b200.so (include/sdm.h): argument validation, workspace carving and the
 // launch sequence of one coalescence step.  No device memory is allocated here; everything is
 // enqueued on the caller's stream.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdlib>
@@ -104,6 +105,9 @@ static void note_zero_hint(sdm_ctx* ctx, const void* xi, int64_t n_sd) {
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+constexpr int HOST_CHUNKS = 8;                 // pieces of sdm_coalescence_step_host's pipeline
+constexpr int64_t HOST_PIPE_MIN = 1 << 18;     // smaller problems are not worth the extra stream traffic
+
 }  // namespace sdm
 
 using namespace sdm;
@@ -120,6 +124,12 @@ static void free_ctx(sdm_ctx* ctx) {
     if (ctx->verdict_event) cudaEventDestroy(ctx->verdict_event);
     for (cudaEvent_t e : ctx->chunk_event)
         if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->host_in)
+        if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->host_done)
+        if (e) cudaEventDestroy(e);
+    if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
+    if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
     delete ctx;
 }
 
@@ -565,6 +575,7 @@ int wait_verdict(sdm_ctx* ctx, u32 epoch, int32_t n_cell, CellClasses* cc) {
     std::atomic_thread_fence(std::memory_order_acquire);
     cc->worst = m[MAPPED_VERDICT_CLASS];
     cc->mixed = false;
+    cc->cell_offset = 0;
     for (int k = 0; k < CELL_CLASSES; ++k) cc->count[k] = 0;
     if (cc->worst >= (u32)CELL_CLASSES) return SDM_OK;
     uint64_t total = 0;
@@ -979,8 +990,107 @@ int sdm_bind_host_staging(sdm_ctx* ctx, void* staging_dev, size_t staging_bytes)
     if (staging_bytes < sdm_host_staging_bytes(ctx->max_n_sd)) return SDM_ERR_CAPACITY;
     ctx->staging = staging_dev;
     ctx->staging_bytes = staging_bytes;
+    if (!ctx->copy_in) {  // the host entry point overlaps uploads, step and downloads on streams of its own
+        if (cudaSetDevice(ctx->device) != cudaSuccess) return SDM_ERR_CUDA;
+        if (cudaStreamCreateWithFlags(&ctx->copy_in, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&ctx->copy_out, cudaStreamNonBlocking) != cudaSuccess)
+            return SDM_ERR_CUDA;
+        for (int k = 0; k < HOST_CHUNKS; ++k)
+            if (cudaEventCreateWithFlags(&ctx->host_in[k], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&ctx->host_done[k], cudaEventDisableTiming) != cudaSuccess)
+                return SDM_ERR_CUDA;
+    }
     return SDM_OK;
 }
+
+namespace {
+
+// The host entry point as a pipeline (cell-major arrays of many small cells: configs[2..4]).  cell_id goes up first and is
+// analysed as a whole; the attributes go up in HOST_CHUNKS pieces cut at cell boundaries on a stream of their own, the
+// fused kernel runs on the cells of a piece as soon as it has arrived, and the piece goes back on a third stream while
+// the next one is still arriving -- PCIe carries both directions at once, so the call costs about the larger of upload
+// and download instead of their sum.  Returns SDM_OK with *done = false when the input does not qualify (nothing has
+// been applied; cell_id and the attributes are on the device by then, on ctx->stream's side of an event): the caller
+// runs the plain sequence.
+int host_step_pipelined(sdm_ctx* ctx, int64_t* xi_h, double* v_h, int32_t* c_h, int64_t* d_xi, double* d_v, int32_t* d_c,
+                        int64_t n_sd, int32_t n_cell, double dt, double dV, const sdm_kernel_params* kp, uint64_t seed,
+                        uint64_t step, int compact, int64_t* n_sd_out, bool* done) {
+    int rc;
+    *done = false;
+    cudaStream_t st = ctx->stream;
+    // piece boundaries: whole cells (the lower bound of a cell id in the -- presumably sorted -- host array)
+    int64_t cut[HOST_CHUNKS + 1];
+    int32_t cell_cut[HOST_CHUNKS + 1];
+    for (int k = 0; k <= HOST_CHUNKS; ++k) {
+        cell_cut[k] = (int32_t)(((int64_t)n_cell * k) / HOST_CHUNKS);
+        cut[k] = k == HOST_CHUNKS ? n_sd : (int64_t)(std::lower_bound(c_h, c_h + n_sd, cell_cut[k]) - c_h);
+    }
+    cut[0] = 0;
+    for (int k = 1; k <= HOST_CHUNKS; ++k)  // an unsorted array gives arbitrary bounds: keep the pieces a partition of [0, n_sd)
+        if (cut[k] < cut[k - 1]) cut[k] = cut[k - 1];
+    if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_c, c_h, (size_t)n_sd * 4, cudaMemcpyHostToDevice, st)))) return rc;
+    for (int k = 0; k < HOST_CHUNKS; ++k) {
+        const size_t off = (size_t)cut[k], len = (size_t)(cut[k + 1] - cut[k]);
+        if (len) {
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_xi + off, xi_h + off, len * 8, cudaMemcpyHostToDevice, ctx->copy_in)))) return rc;
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_v + off, v_h + off, len * 8, cudaMemcpyHostToDevice, ctx->copy_in)))) return rc;
+        }
+        if ((rc = note_cuda(ctx, cudaEventRecord(ctx->host_in[k], ctx->copy_in)))) return rc;
+    }
+    // the analysis of the whole array: sorted, small cells of nearly one size?
+    const StepArgs A = make_step_args(ctx, d_xi, d_v, d_c, n_sd, n_cell, dt, dV, kp, seed);
+    FusedSource src;
+    if ((rc = enqueue_sorted_prepare(ctx, A, false, &src))) return rc;
+    if ((rc = wait_verdict(ctx, ctx->epoch, n_cell, &src.cc))) return rc;
+    if (src.cc.worst >= (u32)CELL_CLASSES || src.cc.mixed) {
+        // not this path's input: hand the (uploaded) arrays to the plain sequence
+        if ((rc = note_cuda(ctx, cudaStreamWaitEvent(st, ctx->host_in[HOST_CHUNKS - 1], 0)))) return rc;
+        return SDM_OK;
+    }
+    // sorted (verified on the device), so the lower bounds above are the cells' true first entries
+    if ((rc = clear_debug_gammas(ctx, n_sd))) return rc;
+    const PhiloxKeys pk = make_philox_keys(seed, step, ctx->index_base);
+    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u};
+    for (int k = 0; k < HOST_CHUNKS; ++k) {
+        const size_t off = (size_t)cut[k], len = (size_t)(cut[k + 1] - cut[k]);
+        const u32 cells = (u32)(cell_cut[k + 1] - cell_cut[k]);
+        if ((rc = note_cuda(ctx, cudaStreamWaitEvent(st, ctx->host_in[k], 0)))) return rc;
+        if (cells) {
+            CellClasses cc = src.cc;
+            cc.count[cc.worst] = cells;
+            cc.cell_offset = (u32)cell_cut[k];
+            if ((rc = note_cuda(ctx, launch_cell_fused(ctx, 0, nullptr, 0, cc, d_xi, d_v, n_sd, n_cell, A.dtdV, A.dkp, pk, no_links))))
+                return rc;
+        }
+        if ((rc = note_cuda(ctx, cudaEventRecord(ctx->host_done[k], st)))) return rc;
+        if ((rc = note_cuda(ctx, cudaStreamWaitEvent(ctx->copy_out, ctx->host_done[k], 0)))) return rc;
+        if (len) {
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(xi_h + off, d_xi + off, len * 8, cudaMemcpyDeviceToHost, ctx->copy_out)))) return rc;
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(v_h + off, d_v + off, len * 8, cudaMemcpyDeviceToHost, ctx->copy_out)))) return rc;
+        }
+    }
+    ctx->last_path = SDM_PATH_CELL_SORTED;
+    *done = true;
+    int64_t n_out = n_sd;
+    if (compact) {
+        // the fused launches have counted the zeros (k_cell_bounds cleared the count): no counting pass
+        ctx->zero_hint_valid = 1;
+        ctx->zero_hint_xi = d_xi;
+        ctx->zero_hint_n_sd = n_sd;
+        if ((rc = sdm_remove_zero_multiplicity(ctx, d_xi, d_v, d_c, n_sd, &n_out))) return rc;
+        *n_sd_out = n_out;
+        if (n_out != n_sd) {  // entries moved: what is on its way to the host is stale -- fetch the compacted arrays
+            if ((rc = note_cuda(ctx, cudaStreamSynchronize(ctx->copy_out)))) return rc;
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(c_h, d_c, (size_t)n_out * 4, cudaMemcpyDeviceToHost, st)))) return rc;
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(xi_h, d_xi, (size_t)n_out * 8, cudaMemcpyDeviceToHost, st)))) return rc;
+            if ((rc = note_cuda(ctx, cudaMemcpyAsync(v_h, d_v, (size_t)n_out * 8, cudaMemcpyDeviceToHost, st)))) return rc;
+        }
+    }
+    if ((rc = note_cuda(ctx, cudaStreamSynchronize(ctx->copy_out)))) return rc;
+    return finish_run(ctx);
+}
+
+}  // namespace
 
 int sdm_coalescence_step_host(sdm_ctx* ctx, int64_t* multiplicity_host, double* volume_host,
                               int32_t* cell_id_host, int64_t n_sd, int32_t n_cell, double dt, double dV,
@@ -998,11 +1108,19 @@ int sdm_coalescence_step_host(sdm_ctx* ctx, int64_t* multiplicity_host, double* 
     double* d_v = reinterpret_cast<double*>(base + align_up(n * 8 + 16, 256));
     int32_t* d_c = reinterpret_cast<int32_t*>(base + 2 * align_up(n * 8 + 16, 256));
     cudaStream_t st = ctx->stream;
-    if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_xi, multiplicity_host, (size_t)n_sd * 8, cudaMemcpyHostToDevice, st)))) return rc;
-    if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_v, volume_host, (size_t)n_sd * 8, cudaMemcpyHostToDevice, st)))) return rc;
-    if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_c, cell_id_host, (size_t)n_sd * 4, cudaMemcpyHostToDevice, st)))) return rc;
     // the staging area is refilled by every call: what AUTO learned about the previous contents does not carry over
     ctx->verdict_valid = 0;
+    const bool no_debug = !ctx->dbg_perm && !ctx->dbg_cell_start;
+    if (ctx->path == SDM_PATH_AUTO && n_cell > 1 && n_sd >= HOST_PIPE_MIN && no_debug && aligned16(d_xi) && aligned16(d_v)) {
+        bool done = false;
+        rc = host_step_pipelined(ctx, multiplicity_host, volume_host, cell_id_host, d_xi, d_v, d_c, n_sd, n_cell, dt, dV, kp, seed,
+                                 step, compact, n_sd_out, &done);
+        if (rc != SDM_OK || done) return rc;
+    } else {
+        if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_xi, multiplicity_host, (size_t)n_sd * 8, cudaMemcpyHostToDevice, st)))) return rc;
+        if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_v, volume_host, (size_t)n_sd * 8, cudaMemcpyHostToDevice, st)))) return rc;
+        if ((rc = note_cuda(ctx, cudaMemcpyAsync(d_c, cell_id_host, (size_t)n_sd * 4, cudaMemcpyHostToDevice, st)))) return rc;
+    }
     rc = sdm_coalescence_step(ctx, d_xi, d_v, d_c, n_sd, n_cell, dt, dV, kp, seed, step);
     if (rc != SDM_OK) return rc;
     int64_t n_out = n_sd;

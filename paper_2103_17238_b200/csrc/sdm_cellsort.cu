@@ -278,6 +278,7 @@ struct FusedArgs {
     const u32* class_cells[CELL_CLASSES];  // cell ids of the class; nullptr = the cells 0 .. class_count - 1 themselves
     u32 class_count[CELL_CLASSES];
     u32 class_block_end[CELL_CLASSES];
+    u32 cell_offset;      // class_cells == nullptr: the first cell of the launch
     // zero bookkeeping (row a5 fused into a4) and the halt protocol of sdm_coalescence_steps (see sdm_api.cu):
     u32* zc_accum;        // += zero multiplicities the array holds after this step
     const u32* zc_check;  // non-null: the previous step's count, after which a compaction was due -- if it is not 0
@@ -473,7 +474,7 @@ __device__ __forceinline__ u32 class_cells(const FusedArgs& a, WarpStage<R>& st,
     const u32 ci = wfirst * (u32)(32 / G) + (u32)(lane / G);
     u32 start = 0, n_c = 0;
     if (ci < count) {
-        const u32 c = list ? __ldg(list + ci) : ci;
+        const u32 c = list ? __ldg(list + ci) : ci + a.cell_offset;
         start = __ldg(a.pair.cell_start + c);
         n_c = __ldg(a.pair.cell_start + c + 1) - start;
     }
@@ -617,6 +618,7 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.pair.dbg_gamma = reinterpret_cast<long long*>(ctx->dbg_gamma);
     a.pair.dbg_gamma_clamped = reinterpret_cast<long long*>(ctx->dbg_gamma_clamped);
     a.n_cell = n_cell;
+    a.cell_offset = cc.mixed ? 0u : cc.cell_offset;
     a.key_bits = ctx->narrow_key_bits;
     a.run_idx = run_idx;
     a.run_u32 = src_kind == 2;

@@ -122,6 +122,7 @@ struct CellClasses {
     u32 worst;                 // largest class present (CELL_CLASSES: the fused kernel cannot take the input)
     u32 count[CELL_CLASSES];   // cells served as class k (not mixed: every cell as class `worst`)
     bool mixed;                // the cells are dealt out class by class through ws.class_list
+    u32 cell_offset;           // not mixed: the launch serves the cells cell_offset .. cell_offset + count[worst] - 1
 };
 }  // namespace sdm
 
@@ -144,6 +145,8 @@ struct sdm_ctx {
     // host staging
     void* staging;
     size_t staging_bytes;
+    cudaStream_t copy_in, copy_out;          // sdm_coalescence_step_host: uploads / downloads beside the step's stream
+    cudaEvent_t host_in[8], host_done[8];    // per chunk: attributes uploaded / step applied
     int sm_count;
     int skip_key_digits;  // SDM_OPT_SKIP_KEY_DIGITS (-1 = automatic)
     int narrow_key_bits;  // key bits kept in the fused kernel's 32-bit sort word (SDM_OPT_NARROW_KEY_BITS)

@@ -794,6 +794,38 @@ def test_host_entry_with_a_different_cell_layout_per_call(dev):
         assert ctx.poll_error() == 0
 
 
+@pytest.mark.parametrize("case", ["sorted", "sorted_zeros", "interleaved", "mixed_sizes", "ragged"])
+def test_host_entry_pipeline(dev, case):
+    """sdm_coalescence_step_host on arrays large enough for its pipeline (uploads in pieces cut at cell boundaries, the
+    step on every piece as it arrives, downloads on a third stream): cell-major cells of one size take it; input zeros
+    with compaction make it fetch the compacted arrays; interleaved order and mixed cell sizes fall back to the plain
+    sequence; a piece count that does not divide the cells.  Two calls each, against the oracle."""
+    sdm = _sdm()
+    if case == "mixed_sizes":
+        w = W.cfg4(n_cell=5003, n_steps=2)
+    else:
+        w = W.cfg3(n_cell=2311 if case == "ragged" else 2400, per_cell=128, n_steps=2, interleave=(case == "interleaved"),
+                   zero_fraction=0.02 if case == "sorted_zeros" else 0.0)
+    assert w.n_sd >= 1 << 18
+    ow = w.copy()
+    xi, v, cell = (torch.from_numpy(a.copy()).pin_memory() for a in (w.xi, w.v, w.cell_id))
+    n = n_o = w.n_sd
+    with sdm.SDMContext(w.n_sd, w.n_cell, device=dev, host_staging=True) as ctx:
+        for s in range(2):
+            oracle.coalescence_step(ow.xi, ow.v, ow.cell_id, w.n_cell, w.dt, w.dV, _okp(w), 42, s, n_sd=n_o)
+            n_o = oracle.remove_zero_multiplicity(ow.xi, ow.v, ow.cell_id, n_sd=n_o)
+            n = ctx.coalescence_step_host(xi, v, cell, w.n_cell, w.dt, w.dV, _gkp(w), 42, s, n_sd=n, compact=True)
+            assert n == n_o, f"call {s}"
+            assert np.array_equal(xi.numpy()[:n], ow.xi[:n]), f"call {s}"
+            assert np.array_equal(cell.numpy()[:n], ow.cell_id[:n]), f"call {s}"
+            assert np.array_equal(v.numpy()[:n].view(np.int64), ow.v[:n].view(np.int64)), f"call {s}"
+        assert ctx.poll_error() == 0
+        if case in ("sorted", "sorted_zeros", "ragged"):
+            assert ctx.last_path() == sdm.PATH_CELL_SORTED
+    if case == "sorted_zeros":
+        assert n < w.n_sd
+
+
 # ------------------------------------------------------------------------------------------- full size
 FULL = {
     "cfg0": lambda: W.cfg0(),
