@@ -650,7 +650,7 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         return SDM_OK;
     }
     const StepArgs A = make_step_args(ctx, multiplicity, volume, cell_id, n_sd, n_cell, dt, dV, kp, seed);
-    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u};
+    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u, 1u};
     ctx->zero_hint_valid = 0;
     // ---- path selection (include/sdm.h, sdm_path) ----
     FusedSource src;
@@ -733,6 +733,8 @@ int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* vo
 namespace {
 
 constexpr int64_t RUN_CHUNK = 64;  // fused steps enqueued between two looks at the halt word
+constexpr int64_t RUN_STEPS_PER_LAUNCH = 16;  // at most this many steps inside one launch of the fused kernel
+constexpr int64_t RUN_MULTI_STEP_MAX_SD = 1 << 21;  // ... for problems up to this size (configs[2]: 7.6 -> 3.4 us per step)
 
 // Reads and clears the sticky data-error flag after the stream has been drained.
 int finish_run(sdm_ctx* ctx) {
@@ -766,18 +768,30 @@ int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, uin
     ctx->mapped[MAPPED_HALT] = 0u;
     if ((rc = note_cuda(ctx, cudaMemsetAsync(run + RUN_HALT, 0, 4 * 4, st)))) return rc;  // halt word + three zero slots
     int64_t enq = s_begin;  // steps enqueued so far
+    int64_t launch = 0;     // launches so far: launch L counts its zeros into slot L mod 3
     int n_chunks = 0;
     bool halted = false;
+    // cells never interact, so one launch can take its cells through several steps (k_cell_fused, n_steps) as long as no
+    // compaction falls between them; debug outputs describe one step
+    // (large problems gain nothing -- configs[4]: 93 us per step either way -- and keep the shorter launches)
+    const bool one_by_one = ctx->dbg_perm || ctx->dbg_gamma || ctx->dbg_gamma_clamped || ctx->dbg_cell_start ||
+                            A.n_sd > RUN_MULTI_STEP_MAX_SD || !fused_multi_step(ctx, src.cc);
     while (enq < n_steps && !halted) {
         const int64_t c_end = (n_steps - enq > RUN_CHUNK) ? enq + RUN_CHUNK : n_steps;
-        for (; enq < c_end; ++enq) {
+        while (enq < c_end) {
+            int64_t k = c_end - enq < RUN_STEPS_PER_LAUNCH ? c_end - enq : RUN_STEPS_PER_LAUNCH;
+            if (compact_every > 0 && compact_every - (enq % compact_every) < k) k = compact_every - (enq % compact_every);
+            if (one_by_one) k = 1;
             StepLinks links;
-            links.zc_accum = run + RUN_ZC0 + (enq % 3);
-            links.zc_clear = run + RUN_ZC0 + ((enq + 1) % 3);
+            links.zc_accum = run + RUN_ZC0 + (launch % 3);
+            links.zc_clear = run + RUN_ZC0 + ((launch + 1) % 3);
             const bool due_before = compact_every > 0 && enq > s_begin && (enq % compact_every) == 0;
-            links.zc_check = due_before ? run + RUN_ZC0 + ((enq - 1) % 3) : nullptr;
+            links.zc_check = due_before ? run + RUN_ZC0 + ((launch + 2) % 3) : nullptr;  // the previous launch's slot
             links.halt_tag = (u32)(enq - s_begin) + 1u;
+            links.n_steps = (u32)k;
             if ((rc = enqueue_fused_step(ctx, A, src, step0 + (uint64_t)enq, links, true))) return rc;
+            enq += k;
+            ++launch;
         }
         if ((rc = note_cuda(ctx, cudaEventRecord(ctx->chunk_event[n_chunks & 1], st)))) return rc;
         ++n_chunks;
@@ -798,7 +812,7 @@ int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, uin
     // a compaction due after the last step: its count sits in that step's slot
     if (compact_every > 0 && n_steps > s_begin && (n_steps % compact_every) == 0) {
         u32 z = 0;
-        if ((rc = note_cuda(ctx, cudaMemcpy(&z, run + RUN_ZC0 + ((n_steps - 1) % 3), 4, cudaMemcpyDeviceToHost)))) return rc;
+        if ((rc = note_cuda(ctx, cudaMemcpy(&z, run + RUN_ZC0 + ((launch + 2) % 3), 4, cudaMemcpyDeviceToHost)))) return rc;
         *halt_zeros = (int64_t)z;
     }
     return SDM_OK;
@@ -1050,7 +1064,7 @@ int host_step_pipelined(sdm_ctx* ctx, int64_t* xi_h, double* v_h, int32_t* c_h, 
     // sorted (verified on the device), so the lower bounds above are the cells' true first entries
     if ((rc = clear_debug_gammas(ctx, n_sd))) return rc;
     const PhiloxKeys pk = make_philox_keys(seed, step, ctx->index_base);
-    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u};
+    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u, 1u};
     for (int k = 0; k < HOST_CHUNKS; ++k) {
         const size_t off = (size_t)cut[k], len = (size_t)(cut[k + 1] - cut[k]);
         const u32 cells = (u32)(cell_cut[k + 1] - cell_cut[k]);

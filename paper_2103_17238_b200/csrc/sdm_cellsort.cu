@@ -279,6 +279,7 @@ struct FusedArgs {
     u32 class_count[CELL_CLASSES];
     u32 class_block_end[CELL_CLASSES];
     u32 cell_offset;      // class_cells == nullptr: the first cell of the launch
+    u32 n_steps;          // consecutive steps of the launch (pair.pk holds the first); > 1 only without compactions and debug outputs
     // zero bookkeeping (row a5 fused into a4) and the halt protocol of sdm_coalescence_steps (see sdm_api.cu):
     u32* zc_accum;        // += zero multiplicities the array holds after this step
     const u32* zc_check;  // non-null: the previous step's count, after which a compaction was due -- if it is not 0
@@ -318,17 +319,17 @@ __device__ __forceinline__ u32 select_reg(const u32 (&x)[R], int i) {
 
 // The full Philox permutation key of position e of a run (the rare tie repair only; kept out of line).
 template <int HYB>
-__device__ __noinline__ u32 tie_full_key(const FusedArgs* a, u32 start, u32 e) {
-    return philox_perm_key(a->pair.pk, (u64)run_index<HYB>(*a, start, e));
+__device__ __noinline__ u32 tie_full_key(const FusedArgs* a, PhiloxStep ps, u32 start, u32 e) {
+    return philox4x32_10(a->pair.pk, ps, (u64)run_index<HYB>(*a, start, e)).w0;
 }
 
 // Two neighbouring sort words (wa before wb) that agree on the truncated key: is (full key, position) of wa larger
 // than that of wb?  Padding words (position >= n_c) count as key 0xFFFFFFFF: a real word never moves behind them.
 template <int HYB>
-__device__ __forceinline__ bool tie_out_of_order(const FusedArgs& a, u32 start, u32 n_c, u32 wa, u32 wb) {
+__device__ __forceinline__ bool tie_out_of_order(const FusedArgs& a, const PhiloxStep& ps, u32 start, u32 n_c, u32 wa, u32 wb) {
     const u32 ea = wa & 0xFFu, eb = wb & 0xFFu;
-    const u32 ka = ea < n_c ? tie_full_key<HYB>(&a, start, ea) : 0xFFFFFFFFu;
-    const u32 kb = eb < n_c ? tie_full_key<HYB>(&a, start, eb) : 0xFFFFFFFFu;
+    const u32 ka = ea < n_c ? tie_full_key<HYB>(&a, ps, start, ea) : 0xFFFFFFFFu;
+    const u32 kb = eb < n_c ? tie_full_key<HYB>(&a, ps, start, eb) : 0xFFFFFFFFu;
     return ka > kb || (ka == kb && ea > eb);
 }
 
@@ -336,22 +337,22 @@ __device__ __forceinline__ bool tie_out_of_order(const FusedArgs& a, u32 start, 
 // dropped decide their true order.  Odd-even style repair in registers: a bubble pass inside every lane, one
 // exchange across each lane boundary of the group, repeated until a pass swaps nothing anywhere in the warp.
 template <int HYB, int G, int R>
-__device__ __forceinline__ void repair_ties(const FusedArgs& a, u32 (&x)[R], u32 start, u32 n_c, int lg) {
+__device__ __forceinline__ void repair_ties(const FusedArgs& a, const PhiloxStep& ps, u32 (&x)[R], u32 start, u32 n_c, int lg) {
     static_assert(R >= 2, "the two boundary words of a lane are different registers");
     bool again;
     do {
         bool sw = false;
 #pragma unroll
         for (int r = 0; r + 1 < R; ++r) {
-            if ((x[r] ^ x[r + 1]) < 0x100u && tie_out_of_order<HYB>(a, start, n_c, x[r], x[r + 1])) {
+            if ((x[r] ^ x[r + 1]) < 0x100u && tie_out_of_order<HYB>(a, ps, start, n_c, x[r], x[r + 1])) {
                 const u32 t = x[r]; x[r] = x[r + 1]; x[r + 1] = t;
                 sw = true;
             }
         }
         // both lanes of a boundary take the same decision from the same two words
         const u32 nx = __shfl_down_sync(0xffffffffu, x[0], 1), pv = __shfl_up_sync(0xffffffffu, x[R - 1], 1);
-        const bool swn = lg < G - 1 && (x[R - 1] ^ nx) < 0x100u && tie_out_of_order<HYB>(a, start, n_c, x[R - 1], nx);
-        const bool swp = lg > 0 && (pv ^ x[0]) < 0x100u && tie_out_of_order<HYB>(a, start, n_c, pv, x[0]);
+        const bool swn = lg < G - 1 && (x[R - 1] ^ nx) < 0x100u && tie_out_of_order<HYB>(a, ps, start, n_c, x[R - 1], nx);
+        const bool swp = lg > 0 && (pv ^ x[0]) < 0x100u && tie_out_of_order<HYB>(a, ps, start, n_c, pv, x[0]);
         if (swn) x[R - 1] = nx;
         if (swp) x[0] = pv;
         sw |= swn | swp;
@@ -365,8 +366,8 @@ __device__ __forceinline__ void repair_ties(const FusedArgs& a, u32 (&x)[R], u32
 // the first-level pair test are predicated, not branched.
 // FULL: every group of the warp has n_c == G R (no padding, no guards); the caller branches warp-uniformly.
 template <int KIND, int HYB, int G, int R, bool FULL>
-__device__ __forceinline__ u32 group_cells(const FusedArgs& a, WarpStage<R>& st, const u32 start, const u32 n_c_in,
-                                           const int lane) {
+__device__ __forceinline__ u32 group_cells(const FusedArgs& a, const PhiloxStep& ps, WarpStage<R>& st, const u32 start,
+                                           const u32 n_c_in, const int lane) {
     constexpr int P = G * R;
     static_assert(P <= 256, "the position takes 8 bits of the sort word");
     const u32 n_c = FULL ? (u32)P : n_c_in;
@@ -398,7 +399,7 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, WarpStage<R>& st,
         for (int t = 0; t < LB; ++t) {
             const u32 e = (u32)(b + t) * G + lg;
             // keys first: Philox needs only the index, so the attribute loads stay in flight under it
-            const PhiloxOut w = philox4x32_10(pa.pk, (u64)idx[t]);
+            const PhiloxOut w = philox4x32_10(pa.pk, ps, (u64)idx[t]);
             // padding sorts to the end (a real word with the same upper bits has a smaller position) and keeps a
             // position inside the cell's staging slice, so that the unguarded reads of the pair test stay in bounds
             x[b + t] = (FULL || e < n_c) ? (((w.w0 >> drop) << 8) | e) : (0xFFFFFF00u | e);
@@ -420,7 +421,7 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, WarpStage<R>& st,
         if (FULL || (u32)(lg * R + r + 1) < n_c) ties = min(ties, x[r] ^ x[r + 1]);
     if (lg < G - 1 && (FULL || (u32)(lg * R + R) < n_c)) ties = min(ties, x[R - 1] ^ nxt);
     __syncwarp();  // the staging writes of all lanes are visible from here on
-    if (__any_sync(0xffffffffu, ties < 0x100u)) repair_ties<HYB, G, R>(a, x, start, n_c, lg);
+    if (__any_sync(0xffffffffu, ties < 0x100u)) repair_ties<HYB, G, R>(a, ps, x, start, n_c, lg);
     if (a.dbg_perm) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -458,7 +459,7 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, WarpStage<R>& st,
             const bool swap = xa < xb;
             // w2 = 0 makes u a lower bound of the true uniform: the test stays conservative
             if (dbg || pair_may_collide(pa, swap ? xb : xa, swap ? vb : va, swap ? va : vb, 0u, st.w3[cbase + ea], n_c)) {
-                const PhiloxOut w = philox4x32_10(pa.pk, (u64)ja);  // the exact uniform of the first member (R2)
+                const PhiloxOut w = philox4x32_10(pa.pk, ps, (u64)ja);  // the exact uniform of the first member (R2)
                 zeros += pair_apply(pa, ja, jb, xa, va, xb, vb, w.w2, w.w3, n_c);
             }
         }
@@ -468,8 +469,8 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, WarpStage<R>& st,
 
 // The warp's 32 / G cells of size class P = G R: cells [wfirst * 32 / G, ...) of the class list.
 template <int KIND, int HYB, int G, int R>
-__device__ __forceinline__ u32 class_cells(const FusedArgs& a, WarpStage<R>& st, const u32* __restrict__ list, u32 count,
-                                           u32 wfirst, int lane) {
+__device__ __forceinline__ u32 class_cells(const FusedArgs& a, const PhiloxStep& ps, WarpStage<R>& st,
+                                           const u32* __restrict__ list, u32 count, u32 wfirst, int lane) {
     constexpr int P = G * R;
     const u32 ci = wfirst * (u32)(32 / G) + (u32)(lane / G);
     u32 start = 0, n_c = 0;
@@ -491,8 +492,8 @@ __device__ __forceinline__ u32 class_cells(const FusedArgs& a, WarpStage<R>& st,
     if (n_c < 2) n_c = 0;
     if (!__any_sync(0xffffffffu, n_c != 0)) return zeros;
     // regular grids fill their slots exactly (configs[2], [3]: 32 and 128 per cell): that case runs without guards
-    if (__all_sync(0xffffffffu, n_c == (u32)P)) return zeros + group_cells<KIND, HYB, G, R, true>(a, st, start, n_c, lane);
-    return zeros + group_cells<KIND, HYB, G, R, false>(a, st, start, n_c, lane);
+    if (__all_sync(0xffffffffu, n_c == (u32)P)) return zeros + group_cells<KIND, HYB, G, R, true>(a, ps, st, start, n_c, lane);
+    return zeros + group_cells<KIND, HYB, G, R, false>(a, ps, st, start, n_c, lane);
 }
 
 template <int KIND, int HYB, int R>
@@ -517,23 +518,44 @@ __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const __
     WarpStage<R>& st = s_stage[warp];
     // blocks are dealt out class by class, one launch wave after another: the block scheduler balances the
     // (data-dependent) cost of the cells; a persistent strided loop measured 12 % slower on cfg3
+    // (taking the block ranges from the back, largest cells first, measured 1.5 % slower on cfg4)
+    const u32 bid = blockIdx.x;
     u32 cls = 0, bfirst = 0;
 #pragma unroll
     for (u32 k = 0; k + 1 < (u32)CELL_CLASSES; ++k)
-        if (blockIdx.x >= a.class_block_end[k]) { cls = k + 1; bfirst = a.class_block_end[k]; }
-    const u32 wfirst = (blockIdx.x - bfirst) * CF_WARPS + warp;
+        if (bid >= a.class_block_end[k]) { cls = k + 1; bfirst = a.class_block_end[k]; }
+    const u32 wfirst = (bid - bfirst) * CF_WARPS + warp;
+    // n_steps > 1 (a run without compactions, sdm_coalescence_steps): cells never interact, so the warp takes its cells
+    // through all the steps of the launch by itself -- their attributes come back from L1 / L2, and no kernel boundary
+    // (ramp, tail, launch) separates two steps of a small problem
+    // (only the R = 4 kernels, the ones small problems run, carry the loop: in the R = 8 kernels its live values cost
+    // spills -- configs[4] 93 -> 103 us)
+    constexpr bool MULTI = FUSED_MULTI_STEP(R);
+    const u64 step0 = ((u64)a.pair.pk.step_hi << 32) | (u64)a.pair.pk.step_lo;
+    const u32 n_steps = MULTI ? a.n_steps : 1u;
     u32 zeros = 0;
-    // class k: P = 32 << k slots per cell on G = P / R lanes
-    if (cls == 0) {
-        if constexpr (32 / R >= 2) zeros = class_cells<KIND, HYB, 32 / R, R>(a, st, a.class_cells[0], a.class_count[0], wfirst, lane);
-    } else if (cls == 1) {
-        if constexpr (64 / R >= 2 && 64 / R <= 32) zeros = class_cells<KIND, HYB, 64 / R, R>(a, st, a.class_cells[1], a.class_count[1], wfirst, lane);
-    } else if (cls == 2) {
-        if constexpr (128 / R >= 2 && 128 / R <= 32) zeros = class_cells<KIND, HYB, 128 / R, R>(a, st, a.class_cells[2], a.class_count[2], wfirst, lane);
-    } else {
-        if constexpr (256 / R >= 2 && 256 / R <= 32) zeros = class_cells<KIND, HYB, 256 / R, R>(a, st, a.class_cells[3], a.class_count[3], wfirst, lane);
+    for (u32 s = 0; s < n_steps; ++s) {
+        PhiloxStep ps;
+        if constexpr (MULTI) {
+            ps = make_philox_step(step0 + (u64)s);
+        } else {
+            ps.step_hi = a.pair.pk.step_hi;
+            ps.p1_lo = a.pair.pk.p1_lo;
+            ps.p1_hi = a.pair.pk.p1_hi;
+        }
+        // class k: P = 32 << k slots per cell on G = P / R lanes
+        if (cls == 0) {
+            if constexpr (32 / R >= 2) zeros = class_cells<KIND, HYB, 32 / R, R>(a, ps, st, a.class_cells[0], a.class_count[0], wfirst, lane);
+        } else if (cls == 1) {
+            if constexpr (64 / R >= 2 && 64 / R <= 32) zeros = class_cells<KIND, HYB, 64 / R, R>(a, ps, st, a.class_cells[1], a.class_count[1], wfirst, lane);
+        } else if (cls == 2) {
+            if constexpr (128 / R >= 2 && 128 / R <= 32) zeros = class_cells<KIND, HYB, 128 / R, R>(a, ps, st, a.class_cells[2], a.class_count[2], wfirst, lane);
+        } else {
+            if constexpr (256 / R >= 2 && 256 / R <= 32) zeros = class_cells<KIND, HYB, 256 / R, R>(a, ps, st, a.class_cells[3], a.class_count[3], wfirst, lane);
+        }
+        __syncwarp();  // the next step's loads (other lanes) see this step's updates; the staging tile is free again
     }
-    // a5, fused: the number of zero multiplicities after the step (sdm_remove_zero_multiplicity reads it)
+    // a5, fused: the number of zero multiplicities after the (last) step (sdm_remove_zero_multiplicity reads it)
     zeros = __reduce_add_sync(0xffffffffu, zeros);
     if (lane == 0 && zeros) atomicAdd(a.zc_accum, zeros);
 }
@@ -599,6 +621,8 @@ int fused_words_per_lane(const sdm_ctx* ctx, const CellClasses& cc) {
     return slots / (32 * 8) >= (long long)ctx->sm_count * 32 ? 8 : 4;
 }
 
+bool fused_multi_step(const sdm_ctx* ctx, const CellClasses& cc) { return FUSED_MULTI_STEP(fused_words_per_lane(ctx, cc)); }
+
 cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, const CellClasses& cc,
                               int64_t* xi, double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
                               const PhiloxKeys& pk, const StepLinks& links) {
@@ -619,6 +643,8 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.pair.dbg_gamma_clamped = reinterpret_cast<long long*>(ctx->dbg_gamma_clamped);
     a.n_cell = n_cell;
     a.cell_offset = cc.mixed ? 0u : cc.cell_offset;
+    a.n_steps = links.n_steps ? links.n_steps : 1u;
+    if (a.n_steps > 1u && !fused_multi_step(ctx, cc)) return cudaErrorInvalidValue;
     a.key_bits = ctx->narrow_key_bits;
     a.run_idx = run_idx;
     a.run_u32 = src_kind == 2;

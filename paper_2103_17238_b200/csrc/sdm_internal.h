@@ -244,7 +244,11 @@ struct StepLinks {
     const u32* zc_check;
     u32* zc_clear;
     u32 halt_tag;
+    u32 n_steps;  // 0 / 1: one step; more: that many consecutive steps inside the launch (no compaction in between)
 };
+// whether the fused kernel this input gets can take several steps per launch (StepLinks.n_steps > 1)
+#define FUSED_MULTI_STEP(R) ((R) == 4)
+bool fused_multi_step(const sdm_ctx* ctx, const CellClasses& cc);
 cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, int idxbits, const CellClasses& cc,
                               int64_t* xi, double* v, int64_t n_sd, int32_t n_cell, double dtdV, const KernelParams& kp,
                               const PhiloxKeys& pk, const StepLinks& links);
