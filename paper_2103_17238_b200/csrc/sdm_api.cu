@@ -43,7 +43,7 @@ Plan make_plan(int64_t n_sd, int32_t n_cell, int skip_key_digits) {
 // packed = (sortkey >> 8) << idxbits | idx must fit 64 bits, and pass 1 carries a 12-bit tile-local
 // index below the (32 + cbits)-bit sort key.
 static bool plan_fits(const Plan& p) {
-    return (24 + p.cbits + p.idxbits <= 64) && (32 + p.cbits + 12 <= 64);
+    return (24 + p.cbits + p.idxbits <= 64) && (32 + p.cbits + SORT_TILE_BITS <= 64);
 }
 
 Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
@@ -84,7 +84,7 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
 }
 
 // hybrid words: (cell_id << idxbits | index) in 64 bits, and pass 0 stages (cell_id << 12 | tile-local index)
-static bool hybrid_fits(const Plan& p) { return p.cbits >= 1 && p.cbits + p.idxbits <= 64 && p.cbits + 12 <= 64; }
+static bool hybrid_fits(const Plan& p) { return p.cbits >= 1 && p.cbits + p.idxbits <= 64 && p.cbits + SORT_TILE_BITS <= 64; }
 
 static bool sizes_ok(int64_t max_n_sd, int32_t max_n_cell) {
     return max_n_sd >= 0 && max_n_sd < (1LL << 30) && max_n_cell >= 1;
@@ -524,7 +524,7 @@ int enqueue_hybrid_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, bo
     Workspace& ws = ctx->ws;
     if ((rc = next_epoch(ctx))) return rc;
     const int n_cpass = plan.n_cpass;
-    const bool narrow = plan.cbits + plan.idxbits <= 32 && plan.cbits + 12 <= 32;
+    const bool narrow = plan.cbits + plan.idxbits <= 32 && plan.cbits + SORT_TILE_BITS <= 32;
     if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.ctl, 0, ws.zero_bytes_fixed, st)))) return rc;
     if ((rc = note_cuda(ctx, cudaMemsetAsync(ws.tile_state, 0, (size_t)n_cpass * plan.n_tiles * RADIX * 4, st))))
         return rc;

@@ -17,9 +17,16 @@ constexpr int RADIX = 1 << RADIX_BITS;
 constexpr int MAX_PASSES = 8;  // 4 key digits + up to 4 cell-id digits (n_cell <= 2^31)
 
 // Onesweep pass tile: SORT_BLOCK threads x SORT_ITEMS keys.
-constexpr int SORT_BLOCK = 256;
-constexpr int SORT_ITEMS = 16;
+#ifndef SORT_BLOCK_THREADS
+#define SORT_BLOCK_THREADS 256
+#endif
+#ifndef SORT_ITEMS_PER_THREAD
+#define SORT_ITEMS_PER_THREAD 16
+#endif
+constexpr int SORT_BLOCK = SORT_BLOCK_THREADS;
+constexpr int SORT_ITEMS = SORT_ITEMS_PER_THREAD;
 constexpr int SORT_TILE = SORT_BLOCK * SORT_ITEMS;
+constexpr int SORT_TILE_BITS = SORT_TILE == 4096 ? 12 : SORT_TILE == 8192 ? 13 : SORT_TILE == 2048 ? 11 : -1;
 
 // Largest cell the register-resident per-cell sort of the fast path handles (16 lanes x 16 or 32 lanes x 8 words).
 constexpr int CELL_FAST_MAX = 256;

@@ -25,15 +25,17 @@ constexpr u32 FLAG_AGG = 1u << 30;     // tile aggregate available
 constexpr u32 FLAG_PREFIX = 2u << 30;  // inclusive prefix (with the global digit base) available
 constexpr u32 VALUE_MASK = (1u << 30) - 1u;
 constexpr int SORT_WARPS = SORT_BLOCK / 32;
-constexpr int SORT_TILE_BITS = 12;
 constexpr int LOOK_WINDOW = 8;
 static_assert((1 << SORT_TILE_BITS) == SORT_TILE, "tile-local index width");
-static_assert(SORT_BLOCK == RADIX, "one thread per digit");
+static_assert(SORT_BLOCK >= RADIX && SORT_BLOCK % RADIX == 0, "the first RADIX threads own one digit each");
+#ifndef SORT_MIN_BLOCKS
+#define SORT_MIN_BLOCKS (1024 / SORT_BLOCK_THREADS)
+#endif
 
 enum { MODE_KEY_FIRST = 0, MODE_CELL_FIRST = 1, MODE_LATER = 2 };
 
-// Block-wide exclusive scan of one value per thread (SORT_BLOCK == RADIX threads).
-__device__ __forceinline__ u32 block_excl_scan_256(u32 x, u32* s_warp /*[8]*/, int lane, int warp) {
+// Block-wide exclusive scan of one value per digit thread (the first RADIX threads; the others pass 0 and get nothing).
+__device__ __forceinline__ u32 block_excl_scan_256(u32 x, u32* s_warp /*[SORT_WARPS]*/, int lane, int warp) {
     u32 incl = x;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -44,7 +46,7 @@ __device__ __forceinline__ u32 block_excl_scan_256(u32 x, u32* s_warp /*[8]*/, i
     __syncthreads();
     u32 woff = 0;
 #pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w)
+    for (int w = 0; w < RADIX / 32; ++w)
         if (w < warp) woff += s_warp[w];
     __syncthreads();  // s_warp reusable afterwards
     return woff + incl - x;
@@ -62,10 +64,11 @@ __device__ __forceinline__ u32 ld_stream<u32>(const u32* p) {
 }
 
 template <typename TIn, typename TW, int MODE>
-__global__ void __launch_bounds__(SORT_BLOCK, 4)
+__global__ void __launch_bounds__(SORT_BLOCK, SORT_MIN_BLOCKS)
 k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shift, int idxbits, int n_cell,
              const u32* __restrict__ ghist /*[RADIX] global histogram of this digit*/,
              u32* __restrict__ ticket, u32* __restrict__ tile_state /*[n_tiles][RADIX]*/) {
+    static_assert(sizeof(TW) * SORT_TILE >= (size_t)SORT_WARPS * RADIX * 4, "the lane-mask table aliases the staging buffer");
     __shared__ TW s_stage[SORT_TILE];
     __shared__ u32 s_whist[SORT_WARPS][RADIX];
     __shared__ u32 s_goff[RADIX];
@@ -75,15 +78,15 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(ticket, 1u);
 #pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w) {
-        s_whist[w][tid] = 0;
-        reinterpret_cast<u32*>(s_stage)[w * RADIX + tid] = 0;  // the lane-mask table of the ranking phase
-    }
+    for (int i = 0; i < SORT_WARPS * RADIX / SORT_BLOCK; ++i) (&s_whist[0][0])[i * SORT_BLOCK + tid] = 0;
+#pragma unroll
+    for (int i = 0; i < SORT_WARPS * RADIX / SORT_BLOCK; ++i)
+        reinterpret_cast<u32*>(s_stage)[i * SORT_BLOCK + tid] = 0;  // the lane-mask table of the ranking phase
     __syncthreads();
     const u32 tile = s_tile;
     const u32 base = tile * (u32)SORT_TILE;
     const u32 n_valid = min((u32)SORT_TILE, n_sd - base);
-    // where the digit sits in the staged word (first passes stage `word << 12 | tile-local index`)
+    // where the digit sits in the staged word (first passes stage `word << SORT_TILE_BITS | tile-local index`)
     const int dshift = (MODE == MODE_LATER) ? shift : SORT_TILE_BITS + shift;
 
     // ---- load (warp-striped: round k of warp w = 32 consecutive elements) ----
@@ -110,7 +113,7 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
     // ---- stable ranks inside the warp, round by round (32 consecutive elements each) ----
     // The peers of a lane (lanes of the round with the same digit) are collected in a per-warp table of
     // lane masks: one shared-memory atomic OR per element instead of eight ballots and their selects; the
-    // first peer then advances the warp's running digit counter and clears the mask for the next round.
+    // first peer then advances the warp's running digit counter and clears the mask for the next use.
     // The table aliases the staging buffer, which is not written before every warp has finished ranking.
     u32 (*s_mask)[RADIX] = reinterpret_cast<u32 (*)[RADIX]>(s_stage);
     u32 info[SORT_ITEMS];  // [23:16] digit, [15:0] rank among this warp's elements with that digit
@@ -131,12 +134,16 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
             atomicOr(&s_mask[warp][d], me);
             __syncwarp();
             peers = s_mask[warp][d];
-            old = s_whist[warp][d];
-            __syncwarp();
+            __syncwarp();  // every lane has its mask before the first peer clears it
+            // the first peer takes the warp's running count of the digit forward and hands the old value to the others
+            // (one atomic by the first peers and a shuffle instead of a load by every lane and a store by the first
+            // peers: the pass is bound by the shared-memory pipe, profiles/r2d_README.md)
+            old = 0;
             if ((peers & lt) == 0) {
-                s_whist[warp][d] = old + __popc(peers);
+                old = atomicAdd(&s_whist[warp][d], (u32)__popc(peers));
                 s_mask[warp][d] = 0u;
             }
+            old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
         }
         __syncwarp();
         const u32 pre = __popc(peers & lt);
@@ -144,21 +151,26 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
     }
     __syncthreads();
 
-    // ---- per-digit: scan over warps, tile totals, tile-local digit starts ----
-    const u32 d_mine = tid;  // one thread per digit
+    // ---- per-digit (the first RADIX threads): scan over warps, tile totals, tile-local digit starts ----
+    const u32 d_mine = tid & (RADIX - 1);
+    const bool digit_thread = SORT_BLOCK == RADIX || tid < RADIX;
     u32 total = 0;
+    if (digit_thread) {
 #pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w) {
-        const u32 t = s_whist[w][d_mine];
-        s_whist[w][d_mine] = total;
-        total += t;
+        for (int w = 0; w < SORT_WARPS; ++w) {
+            const u32 t = s_whist[w][d_mine];
+            s_whist[w][d_mine] = total;
+            total += t;
+        }
     }
     // publish the aggregate as early as possible (tile 0 publishes its inclusive prefix below)
     u32* my_state = tile_state + (size_t)tile * RADIX + d_mine;
-    if (tile != 0) st_relaxed_u32(my_state, FLAG_AGG | total);
+    if (digit_thread && tile != 0) st_relaxed_u32(my_state, FLAG_AGG | total);
     const u32 lstart = block_excl_scan_256(total, s_warp, lane, warp);  // tile-local start of digit
+    if (digit_thread) {
 #pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w) s_whist[w][d_mine] += lstart;
+        for (int w = 0; w < SORT_WARPS; ++w) s_whist[w][d_mine] += lstart;
+    }
     __syncthreads();
 
     // ---- stage in shared memory in sorted order ----
@@ -166,14 +178,13 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
     for (int k = 0; k < SORT_ITEMS; ++k) s_stage[s_whist[warp][info[k] >> 16] + (info[k] & 0xFFFFu)] = item[k];
 
     // ---- decoupled look-back: global position of this tile's first element of digit d ----
-    u32 gexcl;
+    u32 gexcl = 0;
     if (tile == 0) {
-        gexcl = block_excl_scan_256(ghist[d_mine], s_warp, lane, warp);  // global digit base
-    } else {
+        gexcl = block_excl_scan_256(digit_thread ? ghist[d_mine] : 0u, s_warp, lane, warp);  // global digit base
+    } else if (digit_thread) {
         // a window of LOOK_WINDOW predecessors per round trip to L2 (the tiles of a launch wave publish their
         // aggregates at about the same time, so the walk back to the nearest inclusive prefix is a dozen tiles long
         // on average: one dependent load per tile made the walk the longest stall of the pass)
-        gexcl = 0;
         int t = (int)tile - 1;
         bool done = false;
         while (!done) {
@@ -191,8 +202,10 @@ k_radix_pass(const TIn* __restrict__ in, TW* __restrict__ out, u32 n_sd, int shi
             }
         }
     }
-    st_relaxed_u32(my_state, FLAG_PREFIX | (gexcl + total));
-    s_goff[d_mine] = gexcl - lstart;
+    if (digit_thread) {
+        st_relaxed_u32(my_state, FLAG_PREFIX | (gexcl + total));
+        s_goff[d_mine] = gexcl - lstart;
+    }
     __syncthreads();
 
     // ---- coalesced scatter: consecutive staged positions of one digit are consecutive in `out` ----
