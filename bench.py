@@ -103,6 +103,7 @@ def algorithmic_bytes(n_cell: int):
         "volume_spectrum": 16,
         "cell_classes": 0,                           # reads cell_start (n_cell words)
         "bucket": 4,                                 # hist: one reduction per SD; scatter: one 4-byte index word per SD
+        "resident_move": 36,                         # r index word 4, gather xi,v 16, w xi,v 16 (twice per HYBRID run)
         "box_step": 32,                              # read xi,v 16 + write xi,v 16 (one block, keys regenerated)
     }
 
@@ -537,7 +538,8 @@ def run_ours(args):
                 if wi.n_cell == 1 and pth == "hybrid":
                     continue
                 rr = Runner(wi, dev, path=pth, track_zeros=not args.no_track_zeros)
-                paths[f"{pth}/{label}"] = summarize(rr, 40, 5, args.loop, barrier, peak)
+                # (a HYBRID run pays one gather and one scatter of the attributes per call: 100 steps, as in the configs)
+                paths[f"{pth}/{label}"] = summarize(rr, 100 if pth == "hybrid" else 40, 5, args.loop, barrier, peak)
                 rr.close()
                 del rr
                 torch.cuda.empty_cache()

@@ -157,7 +157,9 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
  * due compaction costs nothing while no multiplicity is 0: every fused step counts the zeros it leaves behind, and
  * only a non-zero count at a due step halts the run on the device until the host has compacted.  On the cell-sorted
  * paths small inputs (n_sd <= 2^21) take up to 16 consecutive steps inside one kernel launch when no compaction is
- * due in between (a candidate pair lies inside one cell, so cells never interact); the bits are those of the step-by-step loop.  cell_id is written
+ * due in between (a candidate pair lies inside one cell, so cells never interact), and a HYBRID run of
+ * eight steps or more works on cell-grouped copies of the attributes in the workspace (gathered once, scattered back
+ * before the call returns or compacts); the bits are those of the step-by-step loop.  cell_id is written
  * only by a compaction.  *n_sd_out (host) receives the final number of super-droplets; the call synchronises the
  * stream once, at its end, and then also reports a pending SDM_ERR_BAD_DATA.  n_steps == 0 and n_sd == 0 are no-ops.
  * Errors: as sdm_coalescence_step, plus INVALID_ARG for n_steps < 0, compact_every < 0 or a null n_sd_out. */

@@ -40,7 +40,7 @@ EXPORTS = [
 ]
 
 PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
-                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum", "displace", "cell_classes", "box_step", "bucket"]
+                "cell_bounds", "cell_fused", "cell_digit_hist", "tie_repair", "volume_spectrum", "displace", "cell_classes", "box_step", "bucket", "resident_move"]
 
 
 class SDMError(RuntimeError):

@@ -79,6 +79,8 @@ Workspace carve_workspace(void* base, int64_t max_n_sd, int32_t max_n_cell) {
     w.scan_state_bytes = ((size_t)max_n_cell / 4096 + 2) * 8;
     w.scan_state = reinterpret_cast<u64*>(take(w.scan_state_bytes));
     w.run = reinterpret_cast<u32*>(take(RUN_WORDS * 4));
+    w.res_xi = reinterpret_cast<int64_t*>(take((size_t)max_n_sd * 8 + 16));
+    w.res_v = reinterpret_cast<double*>(take((size_t)max_n_sd * 8 + 16));
     w.total_bytes = off;
     return w;
 }
@@ -507,13 +509,14 @@ struct FusedSource {
     const void* run_idx;
     int idxbits;
     CellClasses cc;  // filled in by wait_verdict
+    bool resident;   // the steps work on ws.res_xi / ws.res_v (run_fused_steps)
 };
 
 // cell boundaries straight from cell_id (CELL_SORTED)
 int enqueue_sorted_prepare(sdm_ctx* ctx, const StepArgs& A, bool strict, FusedSource* src) {
     int rc;
     if ((rc = next_epoch(ctx))) return rc;
-    src->kind = 0; src->run_idx = nullptr; src->idxbits = 0;
+    src->kind = 0; src->run_idx = nullptr; src->idxbits = 0; src->resident = false;
     return note_cuda(ctx, launch_cell_bounds(ctx, 0, A.cell_id, A.n_sd, A.n_cell, 0, strict));
 }
 
@@ -538,6 +541,7 @@ int enqueue_hybrid_prepare(sdm_ctx* ctx, const StepArgs& A, const Plan& plan, bo
         out = (out == (void*)ws.buf_a) ? (void*)ws.buf_b : (void*)ws.buf_a;
     }
     src->kind = narrow ? 2 : 1;
+    src->resident = false;
     src->run_idx = in;
     src->idxbits = plan.idxbits;
     return note_cuda(ctx, launch_cell_bounds(ctx, src->kind, in, A.n_sd, A.n_cell, plan.idxbits, strict));
@@ -549,8 +553,11 @@ int enqueue_fused_step(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, 
     if ((rc = clear_debug_gammas(ctx, A.n_sd))) return rc;
     if (bump_epoch && (rc = next_epoch(ctx))) return rc;
     const PhiloxKeys pk = make_philox_keys(A.seed, step, ctx->index_base);
-    if ((rc = note_cuda(ctx, launch_cell_fused(ctx, src.kind, src.run_idx, src.idxbits, src.cc, A.xi, A.v, A.n_sd,
-                                               A.n_cell, A.dtdV, A.dkp, pk, links))))
+    StepLinks l = links;
+    l.resident = src.resident;
+    if ((rc = note_cuda(ctx, launch_cell_fused(ctx, src.kind, src.run_idx, src.idxbits, src.cc,
+                                               src.resident ? ctx->ws.res_xi : A.xi, src.resident ? ctx->ws.res_v : A.v,
+                                               A.n_sd, A.n_cell, A.dtdV, A.dkp, pk, l))))
         return rc;
     ctx->last_path = src.kind == 0 ? SDM_PATH_CELL_SORTED : SDM_PATH_HYBRID;
     return SDM_OK;
@@ -650,7 +657,7 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
         return SDM_OK;
     }
     const StepArgs A = make_step_args(ctx, multiplicity, volume, cell_id, n_sd, n_cell, dt, dV, kp, seed);
-    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u, 1u};
+    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u, 1u, false};
     ctx->zero_hint_valid = 0;
     // ---- path selection (include/sdm.h, sdm_path) ----
     FusedSource src;
@@ -734,6 +741,9 @@ namespace {
 
 constexpr int64_t RUN_CHUNK = 64;  // fused steps enqueued between two looks at the halt word
 constexpr int64_t RUN_STEPS_PER_LAUNCH = 16;  // at most this many steps inside one launch of the fused kernel
+// HYBRID runs at least this long keep cell-grouped copies of the attributes (interleaved configs[3]: the two moves cost
+// 670 us together, every step saves 110 us)
+constexpr int64_t RUN_RESIDENT_MIN_STEPS = 8;
 constexpr int64_t RUN_MULTI_STEP_MAX_SD = 1 << 21;  // ... for problems up to this size (configs[2]: 7.6 -> 3.4 us per step)
 
 // Reads and clears the sticky data-error flag after the stream has been drained.
@@ -758,9 +768,10 @@ int finish_run(sdm_ctx* ctx) {
 // enqueued exit without touching the state, and the host -- which watches the mapped halt word from one chunk
 // behind -- compacts and resumes from the halted step.  Returns with *s = first step not yet applied,
 // *halt_zeros > 0 when a compaction of that many zeros is due before step *s (stream drained), else 0.
-int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, uint64_t step0, int64_t* s,
-                    int64_t n_steps, int64_t compact_every, int64_t* halt_zeros) {
+int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src_in, uint64_t step0, int64_t* s,
+                    int64_t n_steps, int64_t compact_every, bool allow_resident, int64_t* halt_zeros) {
     int rc;
+    FusedSource src = src_in;
     cudaStream_t st = ctx->stream;
     u32* run = ctx->ws.run;
     *halt_zeros = 0;
@@ -774,8 +785,14 @@ int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, uin
     // cells never interact, so one launch can take its cells through several steps (k_cell_fused, n_steps) as long as no
     // compaction falls between them; debug outputs describe one step
     // (large problems gain nothing -- configs[4]: 93 us per step either way -- and keep the shorter launches)
-    const bool one_by_one = ctx->dbg_perm || ctx->dbg_gamma || ctx->dbg_gamma_clamped || ctx->dbg_cell_start ||
-                            A.n_sd > RUN_MULTI_STEP_MAX_SD || !fused_multi_step(ctx, src.cc);
+    const bool debug_out = ctx->dbg_perm || ctx->dbg_gamma || ctx->dbg_gamma_clamped || ctx->dbg_cell_start;
+    const bool one_by_one = debug_out || A.n_sd > RUN_MULTI_STEP_MAX_SD || !fused_multi_step(ctx, src.cc);
+    // HYBRID: a long enough run works on cell-grouped copies of the attributes (gathered once here,
+    // scattered back below) instead of gathering them through the index words in every step
+    src.resident = src.kind != 0 && !debug_out && allow_resident && n_steps - s_begin >= RUN_RESIDENT_MIN_STEPS;
+    if (src.resident &&
+        (rc = note_cuda(ctx, launch_resident_move(ctx, false, src.kind, src.run_idx, src.idxbits, A.xi, A.v, A.n_sd))))
+        return rc;
     while (enq < n_steps && !halted) {
         const int64_t c_end = (n_steps - enq > RUN_CHUNK) ? enq + RUN_CHUNK : n_steps;
         while (enq < c_end) {
@@ -800,6 +817,10 @@ int run_fused_steps(sdm_ctx* ctx, const StepArgs& A, const FusedSource& src, uin
             halted = ctx->mapped[MAPPED_HALT] != 0u;
         }
     }
+    // (a halted run left the copies as the last applied step wrote them)
+    if (src.resident &&
+        (rc = note_cuda(ctx, launch_resident_move(ctx, true, src.kind, src.run_idx, src.idxbits, A.xi, A.v, A.n_sd))))
+        return rc;
     if ((rc = note_cuda(ctx, cudaStreamSynchronize(st)))) return rc;
     std::atomic_thread_fence(std::memory_order_acquire);
     const u32 tag = ctx->mapped[MAPPED_HALT];
@@ -834,6 +855,7 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
     int64_t n = n_sd;
     int64_t s = 0;
     bool general_only = (n_cell <= 1) || ctx->path == SDM_PATH_GENERAL || ctx->path == SDM_PATH_BOX || ctx->path == SDM_PATH_BUCKET;
+    bool allow_resident = true;
     while (s < n_steps && n > 0) {
         const StepArgs A = make_step_args(ctx, multiplicity, volume, cell_id, n, n_cell, dt, dV, kp, seed);
         const Plan plan = make_plan(n, n_cell, ctx->skip_key_digits);
@@ -859,7 +881,10 @@ int sdm_coalescence_steps(sdm_ctx* ctx, int64_t* multiplicity, double* volume, i
         }
         int64_t zeros = 0;
         if (fused) {
-            if ((rc = run_fused_steps(ctx, A, src, step0, &s, n_steps, compact_every, &zeros))) return rc;
+            const int64_t s_before = s;
+            if ((rc = run_fused_steps(ctx, A, src, step0, &s, n_steps, compact_every, allow_resident, &zeros))) return rc;
+            // compactions that keep finding zeros after a few steps: the next runs gather in every step instead
+            if (zeros > 0 && s - s_before < RUN_RESIDENT_MIN_STEPS) allow_resident = false;
             if (zeros > 0) {
                 if ((rc = enqueue_compact(ctx, multiplicity, volume, cell_id, n))) return rc;
                 n -= zeros;
@@ -1064,7 +1089,7 @@ int host_step_pipelined(sdm_ctx* ctx, int64_t* xi_h, double* v_h, int32_t* c_h, 
     // sorted (verified on the device), so the lower bounds above are the cells' true first entries
     if ((rc = clear_debug_gammas(ctx, n_sd))) return rc;
     const PhiloxKeys pk = make_philox_keys(seed, step, ctx->index_base);
-    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u, 1u};
+    const StepLinks no_links = {nullptr, nullptr, nullptr, 0u, 1u, false};
     for (int k = 0; k < HOST_CHUNKS; ++k) {
         const size_t off = (size_t)cut[k], len = (size_t)(cut[k + 1] - cut[k]);
         const u32 cells = (u32)(cell_cut[k + 1] - cell_cut[k]);

@@ -291,13 +291,20 @@ struct FusedArgs {
     volatile u32* mapped; // pinned host status words (MAPPED_*), written with a system-scope fence
 };
 
-// Original array index of position e of the run that starts at `start`.
+// Original array index of position e of the run that starts at `start` (the Philox counter, R1).
+// HYB: 0 = the arrays are in run order; 1 = HYBRID, attributes gathered through the index words; 2 = HYBRID with a
+// resident copy: pair.xi / pair.v are cell-grouped copies in run order, only the Philox counter comes from the words.
 template <int HYB>
 __device__ __forceinline__ u32 run_index(const FusedArgs& a, u32 start, u32 e) {
     if (HYB == 0) return start + e;
     if (a.run_u32) return __ldg(reinterpret_cast<const u32*>(a.run_idx) + start + e) & (u32)a.idx_mask;
     return (u32)(__ldg(reinterpret_cast<const u64*>(a.run_idx) + start + e) & a.idx_mask);
 }
+
+// Where position e of the run keeps its attributes: HYB = 0 / 2 at the position itself (the arrays, or the
+// cell-grouped copy of a resident run, are in run order), HYB = 1 at its original index.
+template <int HYB>
+__device__ __forceinline__ u32 attr_index(u32 start, u32 e, u32 idx) { return HYB == 1 ? idx : start + e; }
 
 // Per-warp staging of the fp32 side values of the first-level pair test, indexed by cell-in-warp * P + position
 // in the run: written once per super-droplet right after the (coalesced) attribute load, read by sorted position.
@@ -391,8 +398,9 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, const PhiloxStep&
             idx[t] = 0; xi[t] = 1; vol[t] = 0.0;
             if (FULL || e < n_c) {
                 idx[t] = run_index<HYB>(a, start, e);
-                xi[t] = pa.xi[idx[t]];
-                vol[t] = pa.v[idx[t]];
+                const u32 at = attr_index<HYB>(start, e, idx[t]);
+                xi[t] = pa.xi[at];
+                vol[t] = pa.v[at];
             }
         }
 #pragma unroll
@@ -454,13 +462,15 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, const PhiloxStep&
             need &= need - 1u;
             const u32 ea = select_reg<R>(x, 2 * q) & 0xFFu, eb = select_reg<R>(x, 2 * q + 1) & 0xFFu;
             const u32 ja = run_index<HYB>(a, start, ea), jb = run_index<HYB>(a, start, eb);
-            const long long xa = pa.xi[ja], xb = pa.xi[jb];
-            const double va = pa.v[ja], vb = pa.v[jb];
+            const u32 ta = attr_index<HYB>(start, ea, ja), tb = attr_index<HYB>(start, eb, jb);
+            const long long xa = pa.xi[ta], xb = pa.xi[tb];
+            const double va = pa.v[ta], vb = pa.v[tb];
             const bool swap = xa < xb;
             // w2 = 0 makes u a lower bound of the true uniform: the test stays conservative
             if (dbg || pair_may_collide(pa, swap ? xb : xa, swap ? vb : va, swap ? va : vb, 0u, st.w3[cbase + ea], n_c)) {
                 const PhiloxOut w = philox4x32_10(pa.pk, ps, (u64)ja);  // the exact uniform of the first member (R2)
-                zeros += pair_apply(pa, ja, jb, xa, va, xb, vb, w.w2, w.w3, n_c);
+                // (a resident run has no debug outputs, the only other use of the first index)
+                zeros += pair_apply(pa, ta, tb, xa, va, xb, vb, w.w2, w.w3, n_c);
             }
         }
     }
@@ -482,7 +492,7 @@ __device__ __forceinline__ u32 class_cells(const FusedArgs& a, const PhiloxStep&
     u32 zeros = 0;
     if (n_c == 1 && (lane & (G - 1)) == 0) {  // nothing to pair; a lone super-droplet still counts as a zero when its multiplicity is 0
         const u32 i = run_index<HYB>(a, start, 0);
-        zeros = (a.pair.xi[i] == 0);
+        zeros = (a.pair.xi[attr_index<HYB>(start, 0, i)] == 0);
         if (a.dbg_perm) a.dbg_perm[start] = (int32_t)i;
     }
     if (n_c > (u32)P) {  // unreachable: k_cell_bounds refuses such cells and the lists follow its classes
@@ -602,12 +612,78 @@ cudaError_t launch_cell_bounds(sdm_ctx* ctx, int src_kind, const void* src, int6
 cudaError_t init_cell_fused(sdm_ctx*) { return cudaSuccess; }
 
 template <int R>
-static void launch_fused_r(const FusedArgs& a, bool hybrid, u32 grid, cudaStream_t st) {
+static void launch_fused_r(const FusedArgs& a, int hyb, u32 grid, cudaStream_t st) {
     const bool golovin = a.pair.kp.kind == 0;
-    if (golovin && !hybrid) k_cell_fused<0, 0, R><<<grid, CF_BLOCK, 0, st>>>(a);
-    else if (golovin) k_cell_fused<0, 1, R><<<grid, CF_BLOCK, 0, st>>>(a);
-    else if (!hybrid) k_cell_fused<1, 0, R><<<grid, CF_BLOCK, 0, st>>>(a);
-    else k_cell_fused<1, 1, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    if (golovin && hyb == 0) k_cell_fused<0, 0, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    else if (golovin && hyb == 1) k_cell_fused<0, 1, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    else if (golovin) k_cell_fused<0, 2, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    else if (hyb == 0) k_cell_fused<1, 0, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    else if (hyb == 1) k_cell_fused<1, 1, R><<<grid, CF_BLOCK, 0, st>>>(a);
+    else k_cell_fused<1, 2, R><<<grid, CF_BLOCK, 0, st>>>(a);
+}
+
+// A resident HYBRID run (sdm_coalescence_steps): the attributes are gathered ONCE into cell-grouped copies, every step
+// of the run then streams them like the CELL_SORTED path (the gather through the index words costs 180 us per step on
+// interleaved configs[3], the coalesced step 70 us), and they are scattered back when the run ends or halts.
+template <typename TW, bool BACK>
+__global__ void __launch_bounds__(256) k_resident_move(const TW* __restrict__ words, TW idx_mask, u32 n_sd,
+                                                        long long* __restrict__ xi, double* __restrict__ v,
+                                                        long long* __restrict__ res_xi, double* __restrict__ res_v) {
+    constexpr int U = 4;  // independent random accesses in flight per thread
+    const u32 stride = gridDim.x * 256u * U;
+    for (u32 p0 = blockIdx.x * 256u * U + threadIdx.x; p0 < n_sd; p0 += stride) {
+        u32 i[U];
+        long long x[U];
+        double w[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const u32 p = p0 + (u32)u * 256u;
+            i[u] = p < n_sd ? (u32)(words[p] & idx_mask) : 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const u32 p = p0 + (u32)u * 256u;
+            if (p < n_sd) {
+                x[u] = BACK ? res_xi[p] : xi[i[u]];
+                w[u] = BACK ? res_v[p] : v[i[u]];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const u32 p = p0 + (u32)u * 256u;
+            if (p < n_sd) {
+                if (BACK) {
+                    xi[i[u]] = x[u];
+                    v[i[u]] = w[u];
+                } else {
+                    res_xi[p] = x[u];
+                    res_v[p] = w[u];
+                }
+            }
+        }
+    }
+}
+
+cudaError_t launch_resident_move(sdm_ctx* ctx, bool back, int src_kind, const void* run_idx, int idxbits, int64_t* xi,
+                                 double* v, int64_t n_sd) {
+    LaunchScope scope(ctx, PROF_RESIDENT_MOVE);
+    const u32 need = (u32)((n_sd + 1023) / 1024);
+    const u32 cap = (u32)ctx->sm_count * 8u;
+    const u32 grid = need < cap ? need : cap;
+    long long* x = reinterpret_cast<long long*>(xi);
+    long long* rx = reinterpret_cast<long long*>(ctx->ws.res_xi);
+    double* rv = ctx->ws.res_v;
+    const u64 mask = (1ull << idxbits) - 1ull;
+    if (src_kind == 2) {
+        const u32* w = reinterpret_cast<const u32*>(run_idx);
+        if (back) k_resident_move<u32, true><<<grid, 256, 0, ctx->stream>>>(w, (u32)mask, (u32)n_sd, x, v, rx, rv);
+        else k_resident_move<u32, false><<<grid, 256, 0, ctx->stream>>>(w, (u32)mask, (u32)n_sd, x, v, rx, rv);
+    } else {
+        const u64* w = reinterpret_cast<const u64*>(run_idx);
+        if (back) k_resident_move<u64, true><<<grid, 256, 0, ctx->stream>>>(w, mask, (u32)n_sd, x, v, rx, rv);
+        else k_resident_move<u64, false><<<grid, 256, 0, ctx->stream>>>(w, mask, (u32)n_sd, x, v, rx, rv);
+    }
+    return cudaGetLastError();
 }
 
 // Words per lane of the group sort.  8 costs fewer instructions per super-droplet (more of the bitonic stages stay
@@ -670,8 +746,9 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     }
     if (blocks == 0) return cudaSuccess;
     LaunchScope scope(ctx, PROF_CELL_FUSED);
-    if (R == 4) launch_fused_r<4>(a, src_kind != 0, blocks, ctx->stream);
-    else launch_fused_r<8>(a, src_kind != 0, blocks, ctx->stream);
+    const int hyb = src_kind == 0 ? 0 : (links.resident ? 2 : 1);
+    if (R == 4) launch_fused_r<4>(a, hyb, blocks, ctx->stream);
+    else launch_fused_r<8>(a, hyb, blocks, ctx->stream);
     return cudaGetLastError();
 }
 

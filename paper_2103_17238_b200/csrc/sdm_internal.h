@@ -93,6 +93,8 @@ struct Workspace {
     u32* run;         // RUN_WORDS
     u32* cell_start;  // max_n_cell + 1
     u32* class_list;  // CELL_CLASSES x max_n_cell: cell ids grouped by size class (k_cell_classes)
+    int64_t* res_xi;  // max_n_sd each: the cell-grouped copies of a resident HYBRID run (launch_resident_move)
+    double* res_v;
     u32* bucket_count;  // BUCKET path: 2^BUCKET_MAX_BITS coarse-bucket fill counts (zeroed per step)
     u64* buf_a;       // max_n_sd
     u64* buf_b;       // max_n_sd
@@ -119,7 +121,7 @@ struct Plan {  // per-step derived quantities
 namespace sdm {
 // Kernel classes for sdm_profile_read (same order as SDM_PROF_* in include/sdm.h).
 enum ProfClass { PROF_KEYS_HIST = 0, PROF_CELL_SCAN, PROF_RADIX_PASS, PROF_PAIR, PROF_COUNT_ZERO, PROF_COMPACT,
-                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_DISPLACE, PROF_CELL_CLASSES, PROF_BOX_STEP, PROF_BUCKET, PROF_CLASSES };
+                 PROF_CELL_STATS, PROF_OTHER, PROF_CELL_BOUNDS, PROF_CELL_FUSED, PROF_CELL_DIGIT_HIST, PROF_TIE_REPAIR, PROF_SPECTRUM, PROF_DISPLACE, PROF_CELL_CLASSES, PROF_BOX_STEP, PROF_BUCKET, PROF_RESIDENT_MOVE, PROF_CLASSES };
 // What the last general-path step learned about the cell_id array (pinned host memory, written by an
 // asynchronous copy; valid once `verdict_event` has completed).
 struct Verdict { u32 unsorted; u32 max_count; };
@@ -192,7 +194,7 @@ inline const char* prof_class_name(int cls) {
     static const char* const names[PROF_CLASSES] = {
         "sdm:keys_hist", "sdm:cell_scan", "sdm:radix_pass", "sdm:pair", "sdm:count_zero", "sdm:compact", "sdm:cell_stats",
         "sdm:other", "sdm:cell_bounds", "sdm:cell_fused", "sdm:cell_digit_hist", "sdm:tie_repair", "sdm:volume_spectrum",
-        "sdm:displace", "sdm:cell_classes", "sdm:box_steps", "sdm:bucket"};
+        "sdm:displace", "sdm:cell_classes", "sdm:box_steps", "sdm:bucket", "sdm:resident_move"};
     return (cls >= 0 && cls < PROF_CLASSES) ? names[cls] : "sdm:?";
 }
 
@@ -252,7 +254,12 @@ struct StepLinks {
     u32* zc_clear;
     u32 halt_tag;
     u32 n_steps;  // 0 / 1: one step; more: that many consecutive steps inside the launch (no compaction in between)
+    bool resident;  // HYBRID: xi / v are the cell-grouped resident copies (launch_resident_move), not the caller's arrays
 };
+// HYBRID runs of sdm_coalescence_steps: gather the attributes into ws.res_xi / ws.res_v in run order (back = false),
+// scatter them back to the caller's arrays (back = true)
+cudaError_t launch_resident_move(sdm_ctx* ctx, bool back, int src_kind, const void* run_idx, int idxbits, int64_t* xi,
+                                 double* v, int64_t n_sd);
 // whether the fused kernel this input gets can take several steps per launch (StepLinks.n_steps > 1)
 #define FUSED_MULTI_STEP(R) ((R) == 4)
 bool fused_multi_step(const sdm_ctx* ctx, const CellClasses& cc);

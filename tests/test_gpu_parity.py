@@ -702,6 +702,20 @@ def test_multi_step_entry_compaction_schedules(dev, name, compact_every):
     _run_multi(w, dev, None, 150 if name == "cfg4s" else 9, compact_every)
 
 
+@pytest.mark.parametrize("name,compact_every,n_steps", [("cfg2", 0, 20), ("cfg3", 1, 12), ("cfg3z", 5, 20), ("cfg4", 0, 24),
+                                                        ("cfg4s", 0, 40), ("cfg4s", 10, 40), ("cfg4s", 1, 12)])
+@pytest.mark.parametrize("path", ["hybrid", "auto"])
+def test_multi_step_entry_resident_hybrid_run(dev, name, compact_every, n_steps, path):
+    """HYBRID runs of eight steps or more work on cell-grouped copies of the attributes (gathered once per run,
+    scattered back when it ends or halts for a compaction): same bits as the step-by-step loop on interleaved input,
+    with no compaction, with compactions that find nothing, with a halt in the first steps (cfg3z) and with halts all
+    the time (cfg4s, every step: the runs fall back to gathering in every step)."""
+    sdm = _sdm()
+    w = W.small(name, interleave=True)
+    _, last = _run_multi(w, dev, sdm.PATH_HYBRID if path == "hybrid" else None, n_steps, compact_every)
+    assert last == sdm.PATH_HYBRID
+
+
 def test_multi_step_entry_interleaved_auto_and_resume(dev):
     """AUTO on an interleaved array: one GENERAL step, then HYBRID for the rest of the call; and a run split into
     three calls equals the run in one call (counter-based RNG: step0 carries the position)."""
