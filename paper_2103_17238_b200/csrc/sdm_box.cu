@@ -211,7 +211,8 @@ __global__ void __cluster_dims__(BC_CLUSTER, 1, 1) __launch_bounds__(BC_THREADS,
 k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
-    extern __shared__ u32 s_hist[];                   // [8192] the block's counts of every bucket -> where its entries start
+    extern __shared__ u32 s_hist2[];                  // 2 x [8192] the block's counts of every bucket -> where its entries
+                                                      // start; steps alternate between the halves (see the end of the loop)
     __shared__ BoxState s_state[BC_THREADS];          // the block's super-droplets, for the whole launch
     __shared__ u32 s_start[BC_THREADS];               // starts of the owned buckets in s_words
     __shared__ u32 s_words[BC_CAP];                   // (low 19 key bits << 13 | index), bucket by bucket
@@ -219,6 +220,8 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
     __shared__ u32 s_warp[BC_THREADS / 32];
     __shared__ u32 s_total;                           // entries in this block's buckets
     __shared__ u32 s_tot[BC_CLUSTER];                 // every block's total (copied after the scan)
+    __shared__ u32 s_head;                            // (step + 1) << 16 | first shuffled index: published after the ranking
+                                                      // (a launch runs at most 4096 steps, BOX_RUN_MAX in sdm_api.cu)
     const u32 n = a.pair.n_sd;
     const u32 rank = cluster.block_rank();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -228,9 +231,10 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
         s_state[tid].v = a.pair.v[i];
     }
     {
-        uint4* z = reinterpret_cast<uint4*>(s_hist);
+        uint4* z = reinterpret_cast<uint4*>(s_hist2);
         for (int q = tid; q < BOX_BUCKETS / 4; q += BC_THREADS) z[q] = make_uint4(0u, 0u, 0u, 0u);
     }
+    if (tid == 0) s_head = 0u;
     const u64 step0 = ((u64)a.pair.pk.step_hi << 32) | (u64)a.pair.pk.step_lo;
     const bool dbg = a.pair.dbg_gamma != nullptr;
     PairArgs pa = a.pair;  // (only the fields the pair rule reads are materialised)
@@ -238,6 +242,7 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
     cluster_barrier();
     for (u32 s = 0; s < a.n_steps; ++s) {
         const PhiloxStep ps = make_philox_step(step0 + (u64)s);
+        u32* s_hist = s_hist2 + (s & 1u) * (u32)BOX_BUCKETS;
         // ---- a1 + rank among the block's entries of the bucket ----
         const u32 key = philox4x32_10(a.pair.pk, ps, (u64)i).w0;
         const u32 gb = key >> (32 - BOX_BUCKET_BITS);  // bucket 0 .. 8191; its owner is gb >> 10
@@ -302,7 +307,14 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
                 s_idx[lo + smaller] = (unsigned short)(mine & ((1u << BOX_IDX_BITS) - 1u));
             }
         }
-        cluster_barrier();
+        // No cluster barrier here: the pairs work on state that no block touches during the ranking, and the one word a
+        // block needs from a neighbour's ranking -- the partner of its last word, the neighbour's first shuffled index
+        // -- is published with the step's tag and polled by the one thread that needs it.
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence_block();
+            *reinterpret_cast<volatile u32*>(&s_head) = ((s + 1u) << 16) | (u32)s_idx[0];
+        }
         // ---- a4: the pairs whose first member is one of this block's shuffled positions ----
         u32 first = 0;  // global shuffled position of the block's first word
         for (u32 r = 0; r < rank; ++r) first += s_tot[r];
@@ -318,7 +330,10 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
             } else {  // the partner opens the next non-empty block
                 u32 r = rank + 1u;
                 while (s_tot[r] == 0u) ++r;  // g + 1 < n: there is one
-                k0 = cluster.map_shared_rank(s_idx, r)[0];
+                const volatile u32* head = cluster.map_shared_rank(&s_head, r);
+                u32 h;
+                do h = *head; while ((h >> 16) != s + 1u);  // that block's ranking of this step is complete
+                k0 = h & 0xFFFFu;
             }
             BoxState* p0 = cluster.map_shared_rank(s_state, j0 / BC_THREADS) + (j0 % BC_THREADS);
             BoxState* p1 = cluster.map_shared_rank(s_state, k0 / BC_THREADS) + (k0 % BC_THREADS);
@@ -332,12 +347,16 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
             if (dbg || pair_may_collide(pa, swap ? x1 : x0, swap ? v1 : v0, swap ? v0 : v1, w.w2, w.w3, n))
                 pair_apply_at(pa, &p0->xi, &p0->v, &p1->xi, &p1->v, j0, x0, v0, x1, v1, w.w2, w.w3, n);
         }
-        {   // for the next step: every source has used the starts in its histogram (barrier before the ranking)
-            uint4* z = reinterpret_cast<uint4*>(s_hist);
+        {   // the next step's histogram: the other half, which nobody has touched since the scatter of the step before
+            // this one.  No cluster barrier closes the step: the next one starts with block-local work (keys, local
+            // histogram), and what the others may still be doing here -- pairs on this block's state, a look at its
+            // first shuffled index -- is not touched again before the barriers of the next step's exchange.
+            uint4* z = reinterpret_cast<uint4*>(s_hist2 + ((s + 1u) & 1u) * (u32)BOX_BUCKETS);
             for (int q = tid; q < BOX_BUCKETS / 4; q += BC_THREADS) z[q] = make_uint4(0u, 0u, 0u, 0u);
         }
-        cluster_barrier();
+        __syncthreads();
     }
+    cluster_barrier();  // the last step's pairs have written this block's state
     if (i < n) {
         a.pair.xi[i] = s_state[tid].xi;
         a.pair.v[i] = s_state[tid].v;
@@ -351,9 +370,9 @@ k_box_cluster(const __grid_constant__ BoxArgs a, u32* __restrict__ sticky) {
 constexpr size_t BOX_SMEM_PER_SD = 8 + 8 + 4 + 2;  // xi, v, sort word, shuffled index
 
 cudaError_t init_box_step(sdm_ctx*) {
-    cudaError_t e = cudaFuncSetAttribute(k_box_cluster<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, BOX_BUCKETS * 4);
+    cudaError_t e = cudaFuncSetAttribute(k_box_cluster<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BOX_BUCKETS * 4);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_box_cluster<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, BOX_BUCKETS * 4);
+    e = cudaFuncSetAttribute(k_box_cluster<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BOX_BUCKETS * 4);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_box_steps, cudaFuncAttributeMaxDynamicSharedMemorySize, BOX_MAX * BOX_SMEM_PER_SD);
 }
@@ -381,9 +400,9 @@ cudaError_t launch_box_steps(sdm_ctx* ctx, int64_t* xi, double* v, int64_t n_sd,
     a.dbg_cell_start = ctx->dbg_cell_start;
     LaunchScope scope(ctx, PROF_BOX_STEP);
     if (ctx->box_cluster && kp.kind == 0)  // one cluster of eight blocks
-        k_box_cluster<true><<<BC_CLUSTER, BC_THREADS, BOX_BUCKETS * 4, ctx->stream>>>(a, ctx->ws.sticky);
+        k_box_cluster<true><<<BC_CLUSTER, BC_THREADS, 2 * BOX_BUCKETS * 4, ctx->stream>>>(a, ctx->ws.sticky);
     else if (ctx->box_cluster)
-        k_box_cluster<false><<<BC_CLUSTER, BC_THREADS, BOX_BUCKETS * 4, ctx->stream>>>(a, ctx->ws.sticky);
+        k_box_cluster<false><<<BC_CLUSTER, BC_THREADS, 2 * BOX_BUCKETS * 4, ctx->stream>>>(a, ctx->ws.sticky);
     else
         k_box_steps<<<1, BOX_THREADS, (size_t)n_sd * BOX_SMEM_PER_SD, ctx->stream>>>(a);
     return cudaGetLastError();
