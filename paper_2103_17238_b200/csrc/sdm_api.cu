@@ -303,7 +303,7 @@ int sdm_volume_spectrum(sdm_ctx* ctx, const int64_t* multiplicity, const double*
     if ((rc = note_cuda(ctx, cudaMemcpyAsync(ctx->ws.spec_edges, volume_edges, (size_t)n_edges * 8,
                                              cudaMemcpyHostToDevice, st))))
         return rc;
-    return note_cuda(ctx, launch_volume_spectrum(ctx, multiplicity, volume, n_sd, ctx->ws.spec_edges, n_edges, count,
+    return note_cuda(ctx, launch_volume_spectrum(ctx, multiplicity, volume, n_sd, ctx->ws.spec_edges, n_edges, volume_edges[0] > 0.0, count,
                                                  sum_xi, sum_xi_v));
 }
 

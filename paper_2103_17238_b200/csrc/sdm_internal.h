@@ -279,7 +279,7 @@ cudaError_t launch_box_steps(sdm_ctx* ctx, int64_t* xi, double* v, int64_t n_sd,
                              const PhiloxKeys& pk, int64_t n_steps);
 cudaError_t init_volume_spectrum(sdm_ctx* ctx);
 cudaError_t launch_volume_spectrum(sdm_ctx* ctx, const int64_t* xi, const double* v, int64_t n_sd,
-                                   const double* edges_dev, int32_t n_edges, int64_t* count, int64_t* sum_xi,
+                                   const double* edges_dev, int32_t n_edges, bool lut_ok /* edges[0] > 0 */, int64_t* count, int64_t* sum_xi,
                                    double* sum_xi_v);
 cudaError_t launch_displace(sdm_ctx* ctx, bool move, double* x, double* z, int32_t* cell_id, int64_t n_sd, int32_t nx,
                             int32_t nz, const double* u_cell, const double* w_cell, double dt);

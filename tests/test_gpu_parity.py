@@ -1078,6 +1078,43 @@ def test_volume_spectrum_against_oracle(dev, name):
     assert np.allclose(got[2], want[2], rtol=VOL_RTOL, atol=0.0)
 
 
+@pytest.mark.parametrize("case", ["log31", "from_zero", "negative", "narrow38", "wide3", "bins39", "bins200"])
+def test_volume_spectrum_bin_search_variants(dev, case):
+    """Both kernels of the product and both bin searches: up to 38 bins take lane-private columns (no atomics) and
+    find the bin through a table over the high word of the volume when every edge is positive (bins far narrower
+    and far wider than a table cell, values exactly on edges), by binary search otherwise; more bins take the
+    atomic kernel.  Ragged odd length."""
+    sdm = _sdm()
+    rng = np.random.default_rng(7)
+    n = 100_003
+    v = np.exp(rng.normal(np.log(1e-15), 2.0, n))
+    xi = rng.integers(0, 10**9, n).astype(np.int64)
+    if case == "log31":
+        edges = np.exp(np.linspace(np.log(1e-18), np.log(1e-12), 32))
+    elif case == "from_zero":
+        edges = np.linspace(0.0, 5e-15, 11)
+    elif case == "negative":
+        edges = np.linspace(-1e-15, 4e-15, 8)
+        v[::7] *= -1.0
+    elif case == "narrow38":
+        edges = 1e-15 * (1.0 + np.arange(39) * 1e-9)     # 38 bins inside a few low-word steps of one high word
+        v[: n // 2] = 1e-15 * (1.0 + rng.random(n // 2) * 39e-9)
+    elif case == "wide3":
+        edges = np.array([1e-300, 1e-16, 1e-14, 1e300])
+    elif case == "bins39":
+        edges = np.exp(np.linspace(np.log(1e-18), np.log(1e-12), 40))
+    else:
+        edges = np.exp(np.linspace(np.log(1e-18), np.log(1e-12), 201))
+    v[:edges.size] = edges                                 # values exactly on the edges (the last one is outside)
+    with sdm.SDMContext(n, 1, device=dev) as ctx:
+        got = [t.cpu().numpy() for t in ctx.volume_spectrum(torch.from_numpy(xi).to(dev), torch.from_numpy(v).to(dev), edges)]
+    want = oracle.volume_spectrum(xi, v, edges)
+    assert want[0].sum() > 0
+    assert np.array_equal(got[0], want[0])
+    assert np.array_equal(got[1], want[1])
+    assert np.allclose(got[2], want[2], rtol=VOL_RTOL, atol=0.0)
+
+
 def test_volume_spectrum_edges_and_degenerate_inputs(dev):
     sdm = _sdm()
     edges = np.array([1.0, 2.0, 4.0, 8.0])
