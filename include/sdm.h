@@ -44,7 +44,8 @@ typedef enum {
     SDM_ERR_INVALID_ARG = -1,
     SDM_ERR_CAPACITY = -2,
     SDM_ERR_CUDA = -3,
-    SDM_ERR_BAD_DATA = -4
+    SDM_ERR_BAD_DATA = -4,
+    SDM_ERR_STATIC_LIMIT = -5 /* sdm_remove_zero_multiplicity_static: n_sd beyond sdm_static_max_n_sd() */
 } sdm_status;
 
 typedef enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GEOMETRIC = 1, SDM_KERNEL_GEOMETRIC_TABLE = 2 } sdm_kernel_kind;
@@ -307,6 +308,28 @@ int sdm_philox_fill(sdm_ctx* ctx, uint64_t seed, uint64_t step, uint64_t i0, int
 /* Test hook for the kernel function alone: K_out[i] = K(vj[i], vk[i]) on device arrays. */
 int sdm_kernel_eval(sdm_ctx* ctx, const sdm_kernel_params* kp, const double* vj, const double* vk,
                     int64_t n, double* K_out);
+
+/* ---- the entry point that allocates nothing (csrc/sdm_noalloc.cu) ----
+ * For callers that cannot call cudaMalloc -- code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * allocation.  The same operation as sdm_remove_zero_multiplicity (north_star (d); stable
+ * in-place removal of the entries whose multiplicity is 0; the prefix [0, n_out) is the result, the tail is
+ * unspecified), but WITHOUT a context and WITHOUT a workspace: its scratch memory (a ticket counter and one word per
+ * tile of 2048 entries) is a fixed device array inside the library, 128.25 KB, which every GPU that loads the
+ * library holds until the process exits.  The call makes no cudaMalloc / cudaFree / allocating library call, creates
+ * no stream or event, and never synchronises:
+ *   multiplicity, volume, cell_id   device arrays of n_sd entries, compacted in place
+ *   n_sd                            0 <= n_sd <= sdm_static_max_n_sd() = 2^26; larger -> SDM_ERR_STATIC_LIMIT, nothing touched
+ *   n_sd_out_dev                    DEVICE int64: receives the number of survivors (written by the kernel)
+ *   cuda_stream                     the stream everything is enqueued on (a memset of the scratch words + one kernel)
+ * It runs on the CURRENT device.  The first call on a device looks the array's device address up (the set-up step;
+ * sdm_static_setup() does only that, for callers who want it done before a graph capture starts).
+ * The scratch array is SHARED by all calls on a device and keeps the last call's contents; every call clears what it
+ * uses on its own stream.  Two calls that overlap on the GPU (different streams or host threads) race on it: the
+ * caller orders them.  Errors: INVALID_ARG (null pointers, n_sd < 0), STATIC_LIMIT, CUDA. */
+int64_t sdm_static_max_n_sd(void);
+int sdm_static_setup(void);
+int sdm_remove_zero_multiplicity_static(int64_t* multiplicity, double* volume, int32_t* cell_id, int64_t n_sd,
+                                        int64_t* n_sd_out_dev /* device */, void* cuda_stream);
 
 const char* sdm_strerror(int status);
 void sdm_destroy(sdm_ctx* ctx);

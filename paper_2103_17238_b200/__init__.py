@@ -31,11 +31,13 @@ from .binding import (  # noqa: F401
     host_staging_bytes,
     library_path,
     load_library,
+    remove_zero_multiplicity_static,
+    static_max_n_sd,
     workspace_bytes,
 )
 
 __all__ = [
     "SDMContext", "SDMError", "KernelParams", "golovin", "geometric", "geometric_table", "GOLOVIN", "GEOMETRIC", "GEOMETRIC_TABLE",
     "PATH_AUTO", "PATH_GENERAL", "PATH_CELL_SORTED", "PATH_HYBRID", "PATH_BOX", "PATH_BUCKET", "OPT_NARROW_KEY_BITS", "OPT_TRACK_ZEROS", "OPT_INDEX_BASE", "OPT_SKIP_KEY_DIGITS", "OPT_FUSED_WORDS_PER_LANE", "OPT_BUCKET_BITS", "OPT_BOX_CLUSTER", "workspace_bytes", "host_staging_bytes",
-    "load_library", "library_path",
+    "load_library", "library_path", "remove_zero_multiplicity_static", "static_max_n_sd",
 ]

@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 OUT = os.path.join(HERE, "libsdm_b200.so")
 SOURCES = ["sdm_api.cu", "sdm_hist.cu", "sdm_sort.cu", "sdm_pair.cu", "sdm_cellsort.cu", "sdm_compact.cu",
-           "sdm_spectrum.cu", "sdm_displace.cu", "sdm_box.cu", "sdm_bucket.cu"]
+           "sdm_spectrum.cu", "sdm_displace.cu", "sdm_box.cu", "sdm_bucket.cu", "sdm_noalloc.cu"]
 HEADERS = ["sdm_device.cuh", "sdm_internal.h", "sdm_pair.cuh", os.path.join("..", "..", "include", "sdm.h")]
 
 NVCC_FLAGS = [

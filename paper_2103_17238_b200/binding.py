@@ -36,7 +36,7 @@ EXPORTS = [
     "sdm_bind_host_staging", "sdm_coalescence_step_host", "sdm_poll_error", "sdm_launch_count",
     "sdm_philox_fill", "sdm_kernel_eval", "sdm_strerror", "sdm_destroy", "sdm_profile_enable",
     "sdm_profile_read", "sdm_set_option", "sdm_volume_spectrum", "sdm_displace", "sdm_cell_id_from_positions",
-    "sdm_set_collision_efficiency",
+    "sdm_set_collision_efficiency", "sdm_static_max_n_sd", "sdm_static_setup", "sdm_remove_zero_multiplicity_static",
 ]
 
 PROF_CLASSES = ["keys_hist", "cell_scan", "radix_pass", "pair", "count_zero", "compact", "cell_stats", "other",
@@ -131,6 +131,12 @@ def load_library():
     lib.sdm_philox_fill.restype = C.c_int
     lib.sdm_kernel_eval.argtypes = [vp, kpp, vp, vp, i64, vp]
     lib.sdm_kernel_eval.restype = C.c_int
+    lib.sdm_static_max_n_sd.argtypes = []
+    lib.sdm_static_max_n_sd.restype = i64
+    lib.sdm_static_setup.argtypes = []
+    lib.sdm_static_setup.restype = C.c_int
+    lib.sdm_remove_zero_multiplicity_static.argtypes = [vp, vp, vp, i64, vp, vp]
+    lib.sdm_remove_zero_multiplicity_static.restype = C.c_int
     lib.sdm_strerror.argtypes = [C.c_int]
     lib.sdm_strerror.restype = C.c_char_p
     lib.sdm_destroy.argtypes = [vp]
@@ -152,6 +158,28 @@ def workspace_bytes(max_n_sd: int, max_n_cell: int) -> int:
 
 def host_staging_bytes(max_n_sd: int) -> int:
     return int(load_library().sdm_host_staging_bytes(max_n_sd))
+
+
+def static_max_n_sd() -> int:
+    """Largest n_sd the allocation-free entry point takes (its scratch is a fixed device array inside the library)."""
+    return int(load_library().sdm_static_max_n_sd())
+
+
+def remove_zero_multiplicity_static(multiplicity, volume, cell_id, n_sd_out, n_sd=None, stream=None) -> None:
+    """sdm_remove_zero_multiplicity_static: no context, no workspace, no allocation, no synchronisation.  `n_sd_out`
+    is a DEVICE int64 tensor of one element that receives the number of survivors.  Runs on the tensors' device, on
+    `stream` (default: torch's current stream there).  Calls that overlap on the GPU race on the shared scratch."""
+    import torch
+
+    lib = load_library()
+    n = int(multiplicity.shape[0] if n_sd is None else n_sd)
+    if n_sd_out.dtype != torch.int64 or n_sd_out.numel() < 1 or not n_sd_out.is_cuda:
+        raise TypeError("n_sd_out must be a CUDA int64 tensor of at least one element")
+    with torch.cuda.device(n_sd_out.device):
+        st = stream if stream is not None else torch.cuda.current_stream(n_sd_out.device)
+        rc = lib.sdm_remove_zero_multiplicity_static(_ptr(multiplicity, torch.int64), _ptr(volume, torch.float64),
+                                                     _ptr(cell_id, torch.int32), n, n_sd_out.data_ptr(), st.cuda_stream)
+    _check(rc, "sdm_remove_zero_multiplicity_static")
 
 
 def _ptr(t, dtype=None):

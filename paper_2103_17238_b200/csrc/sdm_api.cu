@@ -231,6 +231,8 @@ const char* sdm_strerror(int status) {
         case SDM_ERR_CAPACITY: return "problem larger than the context capacity (or workspace too small)";
         case SDM_ERR_CUDA: return "CUDA error";
         case SDM_ERR_BAD_DATA: return "bad data on device (cell_id out of range, or an input the explicitly chosen path cannot take)";
+        case SDM_ERR_STATIC_LIMIT:
+            return "size beyond the fixed scratch array of the allocation-free entry point (sdm_static_max_n_sd: 2^26 super-droplets)";
         default: return "unknown status";
     }
 }
