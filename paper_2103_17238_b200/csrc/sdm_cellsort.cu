@@ -10,13 +10,15 @@
 //
 //   k_cell_bounds<SRC>  reads the cell of every position once (a pure streaming kernel): verifies range and
 //                       order, writes cell_start[0..n_cell].
-//   k_cell_classes      one thread per cell: size class (<= 32, 64, 128, 256 entries), the cell ids grouped by
+//   k_cell_classes      one thread per cell: size class (<= 32, 48, 64, 96, 128, 192, 256 entries), the cell ids grouped by
 //                       class (so that every warp of the fused kernel works on cells of one class) and the
 //                       verdict (device flag for the fused kernel, mapped host words for the path choice and
 //                       the launch geometry).  When the input does not fit the fused kernel launched next,
 //                       that kernel does nothing (the state is never half-updated).
-//   k_cell_fused<R>     size class k = cells of at most P = 32 << k entries, sorted by G = P / R lanes holding
-//                       R words each; a warp takes 32 / G cells.  With R = 8 a cell of 128 runs 18 of the 28
+//   k_cell_fused<R>     size class k = cells of at most P = class_slots(k) entries.  The power-of-two classes are
+//                       sorted by G = P / R lanes holding R words each, the classes in between (48, 96, 192: a
+//                       quarter fewer slots for the cells that fit them) by P / 6 lanes holding 6 words
+//                       (group_sort6); a warp takes 32 / G cells.  With R = 8 a cell of 128 runs 18 of the 28
 //                       bitonic stages inside the lanes (1 instruction per element) and 10 across lanes
 //                       (SHFL + 2 VIMNMX per element); R = 16 (22 + 6) executes 12 % fewer instructions still but
 //                       its straight-line code no longer streams through the instruction caches (30 % of the
@@ -152,8 +154,8 @@ k_cell_bounds(const void* __restrict__ src, u32 n_sd, int n_cell, int idxbits, u
     if (__any_sync(0xffffffffu, bad) && lane == 0) atomicMax(&run[RUN_BOUNDS_CLASS], CLASS_REFUSED);
 }
 
-// Second half of the analysis, one thread per cell: the size class of every cell from cell_start (0: <= 32 entries,
-// 1: <= 64, 2: <= 128, 3: <= 256, refused: larger), the cell ids grouped by class (list[k * stride ...]: cells of
+// Second half of the analysis, one thread per cell: the size class of every cell from cell_start (class k: at most
+// class_slots(k) = 32, 48, 64, 96, 128, 192, 256 entries; refused: larger), the cell ids grouped by class (list[k * stride ...]: cells of
 // fewer than two entries go to class 0 -- the fused kernel still counts a lone zero multiplicity; the order inside a
 // class is the (nearly ascending) order in which the warps draw their slots -- cells are independent, so no result
 // depends on it), and the verdict: the last block publishes the worst class and the class counts through the mapped
@@ -170,7 +172,10 @@ k_cell_classes(const u32* __restrict__ cell_start, int n_cell, u32 strict, u32 e
     u32 cls = 0xFFu;
     if (c < n_cell) {
         const u32 n = cell_start[c + 1] - cell_start[c];
-        cls = n <= 32u ? 0u : (n <= 64u ? 1u : (n <= 128u ? 2u : (n <= 256u ? 3u : CLASS_REFUSED)));
+        cls = CLASS_REFUSED;
+#pragma unroll
+        for (int k = CELL_CLASSES - 1; k >= 0; --k)
+            if (n <= (u32)class_slots(k)) cls = (u32)k;
     }
     const u32 lt = lanemask_lt();
 #pragma unroll
@@ -220,8 +225,63 @@ __device__ __forceinline__ void cmpx_asc(T& a, T& b) {
     b = hi;
 }
 
+// The same for R = 6 words per lane (cells of up to 48 / 96 / 192 entries: three quarters of the next power of two, a
+// quarter fewer slots than that class would spend on them).  The network is the blocked bitonic sort with the lanes'
+// runs as its units: an optimal 12-comparator network sorts the six words of a lane; a merge over m lanes is the flip
+// across lanes (partner lane ^ (m - 1), registers reversed), the half-cleaners at lane distances m/4 .. 1 -- each works
+// on bitonic sequences of the even length 2 lj 6, which is all the half-cleaner theorem needs -- and then every lane
+// holds a bitonic sequence of six words: one half-cleaner at distance 3 and a 3-sorter per half put it in order.
+__device__ __forceinline__ void lane_sort6(u32 (&x)[6]) {
+    cmpx_asc(x[0], x[5]); cmpx_asc(x[1], x[3]); cmpx_asc(x[2], x[4]);
+    cmpx_asc(x[1], x[2]); cmpx_asc(x[3], x[4]);
+    cmpx_asc(x[0], x[3]); cmpx_asc(x[2], x[5]);
+    cmpx_asc(x[0], x[1]); cmpx_asc(x[2], x[3]); cmpx_asc(x[4], x[5]);
+    cmpx_asc(x[1], x[2]); cmpx_asc(x[3], x[4]);
+}
+__device__ __forceinline__ void lane_merge6(u32 (&x)[6]) {  // a bitonic sequence of six words
+    cmpx_asc(x[0], x[3]); cmpx_asc(x[1], x[4]); cmpx_asc(x[2], x[5]);
+    cmpx_asc(x[0], x[2]); cmpx_asc(x[3], x[5]);
+    cmpx_asc(x[0], x[1]); cmpx_asc(x[3], x[4]);
+    cmpx_asc(x[1], x[2]); cmpx_asc(x[4], x[5]);
+}
+template <int G>
+__device__ __forceinline__ void group_sort6(u32 (&x)[6], int lg) {
+    lane_sort6(x);
+#pragma unroll
+    for (int m = 2; m <= G; m <<= 1) {
+        {
+            const bool lower = (lg & (m >> 1)) == 0;
+            u32 y[6];
+#pragma unroll
+            for (int r = 0; r < 6; ++r) y[r] = __shfl_xor_sync(0xffffffffu, x[5 - r], m - 1);
+#pragma unroll
+            for (int r = 0; r < 6; ++r) {
+                const u32 mn = min(x[r], y[r]);
+                const u32 mx = max(x[r], y[r]);
+                x[r] = lower ? mn : mx;
+            }
+        }
+#pragma unroll
+        for (int lj = m >> 2; lj > 0; lj >>= 1) {
+            const bool lower = (lg & lj) == 0;
+#pragma unroll
+            for (int r = 0; r < 6; ++r) {
+                const u32 y = __shfl_xor_sync(0xffffffffu, x[r], lj);
+                const u32 mn = min(x[r], y);
+                const u32 mx = max(x[r], y);
+                x[r] = lower ? mn : mx;
+            }
+        }
+        lane_merge6(x);
+    }
+}
+
 template <int R, int G>
 __device__ __forceinline__ void group_bitonic_sort(u32 (&x)[R], int lg) {
+    if constexpr (R == 6) {
+        group_sort6<G>(x, lg);
+        return;
+    } else {
     constexpr int N = G * R;
 #pragma unroll
     for (int k = 2; k <= N; k <<= 1) {
@@ -261,6 +321,7 @@ __device__ __forceinline__ void group_bitonic_sort(u32 (&x)[R], int lg) {
             }
         }
     }
+    }  // R != 6
 }
 
 struct FusedArgs {
@@ -367,16 +428,18 @@ __device__ __forceinline__ void repair_ties(const FusedArgs& a, const PhiloxStep
     } while (again);
 }
 
+
 // A group of G lanes, one cell of 2 <= n_c <= G R super-droplets per group (n_c = 0: the group idles along).
 // Returns this lane's share of the number of zero multiplicities the cell holds AFTER the step.  The hot flow is
 // straight-line code: loads, Philox blocks (computed for padding slots too, so the R chains interleave), sort and
 // the first-level pair test are predicated, not branched.
 // FULL: every group of the warp has n_c == G R (no padding, no guards); the caller branches warp-uniformly.
-template <int KIND, int HYB, int G, int R, bool FULL>
-__device__ __forceinline__ u32 group_cells(const FusedArgs& a, const PhiloxStep& ps, WarpStage<R>& st, const u32 start,
+template <int KIND, int HYB, int G, int R, bool FULL, int RS>
+__device__ __forceinline__ u32 group_cells(const FusedArgs& a, const PhiloxStep& ps, WarpStage<RS>& st, const u32 start,
                                            const u32 n_c_in, const int lane) {
     constexpr int P = G * R;
     static_assert(P <= 256, "the position takes 8 bits of the sort word");
+    static_assert(R <= RS && R % 2 == 0, "the warp's cells fit the staging tile; pairs never straddle two lanes");
     const u32 n_c = FULL ? (u32)P : n_c_in;
     const PairArgs& pa = a.pair;
     const int lg = lane & (G - 1);
@@ -386,7 +449,7 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, const PhiloxStep&
     //      word 3 are parked in shared memory, the sort word stays in registers ----
     u32 x[R];
     const int drop = 32 - a.key_bits;
-    constexpr int LB = R < 4 ? R : 4;  // loads in flight per lane and batch (8 measured the same)
+    constexpr int LB = R % 4 == 0 ? 4 : (R % 3 == 0 ? 3 : 2);  // loads in flight per lane and batch (8 measured the same)
 #pragma unroll
     for (int b = 0; b < R; b += LB) {
         u32 idx[LB];
@@ -429,6 +492,8 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, const PhiloxStep&
         if (FULL || (u32)(lg * R + r + 1) < n_c) ties = min(ties, x[r] ^ x[r + 1]);
     if (lg < G - 1 && (FULL || (u32)(lg * R + R) < n_c)) ties = min(ties, x[R - 1] ^ nxt);
     __syncwarp();  // the staging writes of all lanes are visible from here on
+    // (out of line -- one copy per words-per-lane instead of one per size class -- the repair was measured 2 % slower on
+    // configs[3] and 2 % faster on configs[4]: the call pins registers around it in the whole kernel)
     if (__any_sync(0xffffffffu, ties < 0x100u)) repair_ties<HYB, G, R>(a, ps, x, start, n_c, lg);
     if (a.dbg_perm) {
 #pragma unroll
@@ -478,8 +543,8 @@ __device__ __forceinline__ u32 group_cells(const FusedArgs& a, const PhiloxStep&
 }
 
 // The warp's 32 / G cells of size class P = G R: cells [wfirst * 32 / G, ...) of the class list.
-template <int KIND, int HYB, int G, int R>
-__device__ __forceinline__ u32 class_cells(const FusedArgs& a, const PhiloxStep& ps, WarpStage<R>& st,
+template <int KIND, int HYB, int G, int R, int RS>
+__device__ __forceinline__ u32 class_cells(const FusedArgs& a, const PhiloxStep& ps, WarpStage<RS>& st,
                                            const u32* __restrict__ list, u32 count, u32 wfirst, int lane) {
     constexpr int P = G * R;
     const u32 ci = wfirst * (u32)(32 / G) + (u32)(lane / G);
@@ -502,13 +567,17 @@ __device__ __forceinline__ u32 class_cells(const FusedArgs& a, const PhiloxStep&
     if (n_c < 2) n_c = 0;
     if (!__any_sync(0xffffffffu, n_c != 0)) return zeros;
     // regular grids fill their slots exactly (configs[2], [3]: 32 and 128 per cell): that case runs without guards
-    if (__all_sync(0xffffffffu, n_c == (u32)P)) return zeros + group_cells<KIND, HYB, G, R, true>(a, ps, st, start, n_c, lane);
-    return zeros + group_cells<KIND, HYB, G, R, false>(a, ps, st, start, n_c, lane);
+    // (the odd classes do without that variant: it is 4 % faster on exactly full tiles and as much code again)
+    if constexpr (R != CELL_ODD_WORDS) {
+        if (__all_sync(0xffffffffu, n_c == (u32)P)) return zeros + group_cells<KIND, HYB, G, R, true, RS>(a, ps, st, start, n_c, lane);
+    }
+    return zeros + group_cells<KIND, HYB, G, R, false, RS>(a, ps, st, start, n_c, lane);
 }
 
 template <int KIND, int HYB, int R>
 __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const __grid_constant__ FusedArgs a) {
-    __shared__ WarpStage<R> s_stage[CF_WARPS];
+    constexpr int RS = R < CELL_ODD_WORDS ? CELL_ODD_WORDS : R;  // the odd classes hold 6 words per lane
+    __shared__ WarpStage<RS> s_stage[CF_WARPS];
     if (a.ctl[CTL_UNSORTED] == a.epoch) return;  // k_cell_bounds refused the input: the step is skipped as a whole
     if (a.halt_tag) {  // a step of sdm_coalescence_steps: a halted run stays halted until the host has compacted
         const u32 halted = a.run[RUN_HALT];
@@ -525,7 +594,7 @@ __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const __
     }
     if (a.zc_clear && blockIdx.x == 0 && threadIdx.x == 0) *a.zc_clear = 0u;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpStage<R>& st = s_stage[warp];
+    WarpStage<RS>& st = s_stage[warp];
     // blocks are dealt out class by class, one launch wave after another: the block scheduler balances the
     // (data-dependent) cost of the cells; a persistent strided loop measured 12 % slower on cfg3
     // (taking the block ranges from the back, largest cells first, measured 1.5 % slower on cfg4)
@@ -553,16 +622,23 @@ __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const __
             ps.p1_lo = a.pair.pk.p1_lo;
             ps.p1_hi = a.pair.pk.p1_hi;
         }
-        // class k: P = 32 << k slots per cell on G = P / R lanes
-        if (cls == 0) {
-            if constexpr (32 / R >= 2) zeros = class_cells<KIND, HYB, 32 / R, R>(a, ps, st, a.class_cells[0], a.class_count[0], wfirst, lane);
-        } else if (cls == 1) {
-            if constexpr (64 / R >= 2 && 64 / R <= 32) zeros = class_cells<KIND, HYB, 64 / R, R>(a, ps, st, a.class_cells[1], a.class_count[1], wfirst, lane);
-        } else if (cls == 2) {
-            if constexpr (128 / R >= 2 && 128 / R <= 32) zeros = class_cells<KIND, HYB, 128 / R, R>(a, ps, st, a.class_cells[2], a.class_count[2], wfirst, lane);
-        } else {
-            if constexpr (256 / R >= 2 && 256 / R <= 32) zeros = class_cells<KIND, HYB, 256 / R, R>(a, ps, st, a.class_cells[3], a.class_count[3], wfirst, lane);
+        // class k: P = class_slots(k) slots per cell; even classes on G = P / R lanes of R words, odd ones on P / 6 lanes of 6
+#define SDM_EVEN_CLASS(K)                                                                                              \
+    if constexpr (class_lanes(K, R) >= 2 && class_lanes(K, R) <= 32)                                                   \
+        zeros = class_cells<KIND, HYB, class_lanes(K, R), R, RS>(a, ps, st, a.class_cells[K], a.class_count[K], wfirst, lane)
+#define SDM_ODD_CLASS(K)                                                                                               \
+    zeros = class_cells<KIND, HYB, class_lanes(K, R), CELL_ODD_WORDS, RS>(a, ps, st, a.class_cells[K], a.class_count[K], wfirst, lane)
+        switch (cls) {
+            case 0: SDM_EVEN_CLASS(0); break;
+            case 1: SDM_ODD_CLASS(1); break;
+            case 2: SDM_EVEN_CLASS(2); break;
+            case 3: SDM_ODD_CLASS(3); break;
+            case 4: SDM_EVEN_CLASS(4); break;
+            case 5: SDM_ODD_CLASS(5); break;
+            default: SDM_EVEN_CLASS(6); break;
         }
+#undef SDM_EVEN_CLASS
+#undef SDM_ODD_CLASS
         __syncwarp();  // the next step's loads (other lanes) see this step's updates; the staging tile is free again
     }
     // a5, fused: the number of zero multiplicities after the (last) step (sdm_remove_zero_multiplicity reads it)
@@ -688,12 +764,12 @@ cudaError_t launch_resident_move(sdm_ctx* ctx, bool back, int src_kind, const vo
 
 // Words per lane of the group sort.  8 costs fewer instructions per super-droplet (more of the bitonic stages stay
 // inside the lanes); small problems, whose warps would not fill the machine then, take 4 (configs[2]: 10.6 us
-// against 11.8 us).  Cells of more than 128 entries need 8 (32 lanes x 8 words).
+// against 11.8 us).  Cells of more than 192 entries need 8 (32 lanes x 8 words).
 int fused_words_per_lane(const sdm_ctx* ctx, const CellClasses& cc) {
-    if (cc.worst > 2 || ctx->fused_r == 8) return 8;
+    if (cc.worst == (u32)CELL_CLASSES - 1 || ctx->fused_r == 8) return 8;
     if (ctx->fused_r == 4) return 4;
     long long slots = 0;
-    for (int k = 0; k < CELL_CLASSES; ++k) slots += (long long)cc.count[k] * (32ll << k);
+    for (int k = 0; k < CELL_CLASSES; ++k) slots += (long long)cc.count[k] * class_slots(k);
     return slots / (32 * 8) >= (long long)ctx->sm_count * 32 ? 8 : 4;
 }
 
@@ -738,7 +814,7 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     const int R = fused_words_per_lane(ctx, cc);
     u32 blocks = 0;
     for (int k = 0; k < CELL_CLASSES; ++k) {
-        const u32 cells_per_block = (u32)CF_WARPS * 32u / ((32u << k) / (u32)R);  // CF_WARPS * 32 / G
+        const u32 cells_per_block = (u32)CF_WARPS * 32u / (u32)class_lanes(k, R);  // CF_WARPS * 32 / G
         a.class_count[k] = cc.count[k];
         a.class_cells[k] = cc.mixed ? ctx->ws.class_list + (size_t)k * (size_t)ctx->max_n_cell : nullptr;
         blocks += (cc.count[k] + cells_per_block - 1) / cells_per_block;

@@ -34,8 +34,13 @@ constexpr int CELL_FAST_MAX = 256;
 constexpr int BUCKET_MAX_BITS = 12;
 // Largest single-cell problem the box step takes (sdm_box.cu).
 constexpr int BOX_MAX = 8192;
-// Cell-size classes of the fused kernel: class k = cells of at most 32 << k entries.
-constexpr int CELL_CLASSES = 4;
+// Cell-size classes of the fused kernel: class k = cells of at most class_slots(k) = 32, 48, 64, 96, 128, 192, 256
+// entries.  Even classes are sorted by P / R lanes holding R = 8 (or 4) words each, odd ones by P / 6 lanes holding 6.
+constexpr int CELL_CLASSES = 7;
+constexpr int CELL_ODD_WORDS = 6;
+__host__ __device__ constexpr int class_slots(int k) { return (k & 1) ? (48 << (k >> 1)) : (32 << (k >> 1)); }
+__host__ __device__ constexpr int class_lanes(int k, int r_even) { return (k & 1) ? (8 << (k >> 1)) : class_slots(k) / r_even; }
+static_assert(class_slots(CELL_CLASSES - 1) == CELL_FAST_MAX, "the largest class is the largest cell of the fast path");
 
 // Largest collision-efficiency table sdm_set_collision_efficiency accepts (radii x ratios).
 constexpr int EFF_MAX_R = 128;
@@ -65,7 +70,7 @@ enum RunWord {
     RUN_ZC0 = 1,   // RUN_ZC0 + (s mod 3): zero multiplicities the array holds after step s of the run
     RUN_BOUNDS_TICKET = 4,  // k_cell_bounds: blocks finished (the last one publishes the verdict and resets it)
     RUN_BOUNDS_CLASS = 5,   // k_cell_bounds: worst cell-size class seen so far (reset by the last block)
-    RUN_LIST_CURSOR = 12,   // RUN_LIST_CURSOR + k, k = 0..3: k_cell_classes' fill level of class k's list (reset by its last block)
+    RUN_LIST_CURSOR = 12,   // RUN_LIST_CURSOR + k, k = 0..CELL_CLASSES-1: k_cell_classes' fill level of class k's list (reset by its last block)
     RUN_WORDS = 64
 };
 // Words of the pinned, device-mapped host status block: what the host must learn WITHOUT draining the stream.
@@ -73,9 +78,9 @@ enum MappedWord {
     MAPPED_HALT = 0,     // RUN_HALT's tag
     MAPPED_ZEROS = 1,    // the zero count that caused the halt
     MAPPED_VERDICT_EPOCH = 2,  // k_cell_bounds: epoch of the last published verdict
-    MAPPED_VERDICT_CLASS = 3,  //   its worst cell-size class: 0 (<= 32), 1 (<= 64), 2 (<= 128), 3 (<= 256), 4 (larger,
+    MAPPED_VERDICT_CLASS = 3,  //   its worst cell-size class: 0 (<= 32 entries) .. 6 (<= 256), see class_slots; CELL_CLASSES (larger,
                                //   or the array is not non-decreasing / holds an out-of-range cell_id)
-    MAPPED_CLASS_COUNT = 4,    //   MAPPED_CLASS_COUNT + k, k = 0..3: number of cells of size class k
+    MAPPED_CLASS_COUNT = 4,    //   MAPPED_CLASS_COUNT + k, k = 0..CELL_CLASSES-1: number of cells of size class k
     MAPPED_WORDS = 16
 };
 // Sticky words (zeroed at init and by sdm_poll_error only).

@@ -253,7 +253,8 @@ def test_fused_kernel_tie_repair(dev, path, bits, fused_r):
 @pytest.mark.parametrize("path", ["cell_sorted", "hybrid"])
 @pytest.mark.parametrize("fused_r", [4, 8])
 def test_fused_kernel_words_per_lane(dev, name, path, fused_r):
-    """Every group shape of the fused kernel (G = (32 << class) / R lanes per cell, R words per lane; uniform cell
+    """Every group shape of the fused kernel (classes of 32 / 64 / 128 / 256 slots on P / R lanes of R words, classes of
+    48 / 96 / 192 slots on P / 6 lanes of 6 words; uniform cell
     sizes served as one class, mixed sizes through the class lists) gives the oracle's bits."""
     sdm = _sdm()
     p = {"cell_sorted": sdm.PATH_CELL_SORTED, "hybrid": sdm.PATH_HYBRID}[path]
@@ -292,7 +293,8 @@ def test_hybrid_path_refuses_large_cells(dev):
         assert torch.equal(xi, before[0]) and torch.equal(v, before[1])
 
 
-@pytest.mark.parametrize("per_cell", [1, 2, 3, 15, 16, 17, 31, 32, 33, 63, 64, 65, 127, 128, 129, 255, 256])
+@pytest.mark.parametrize("per_cell", [1, 2, 3, 15, 16, 17, 31, 32, 33, 47, 48, 49, 63, 64, 65, 95, 96, 97, 127, 128, 129,
+                                      191, 192, 193, 255, 256])
 @pytest.mark.parametrize("fused_r", [None, 4, 8])
 def test_cell_sorted_path_cell_sizes(dev, per_cell, fused_r):
     """every size class of the per-cell sort, at and around its boundaries, plus empty cells"""
