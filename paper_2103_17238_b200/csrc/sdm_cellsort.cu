@@ -339,6 +339,7 @@ struct FusedArgs {
     const u32* class_cells[CELL_CLASSES];  // cell ids of the class; nullptr = the cells 0 .. class_count - 1 themselves
     u32 class_count[CELL_CLASSES];
     u32 class_block_end[CELL_CLASSES];
+    u32 only_class;       // the one class that has blocks in this launch; CELL_CLASSES: several have
     u32 cell_offset;      // class_cells == nullptr: the first cell of the launch
     u32 n_steps;          // consecutive steps of the launch (pair.pk holds the first); > 1 only without compactions and debug outputs
     // zero bookkeeping (row a5 fused into a4) and the halt protocol of sdm_coalescence_steps (see sdm_api.cu):
@@ -599,10 +600,15 @@ __global__ void __launch_bounds__(CF_BLOCK, CF_MIN_BLOCKS) k_cell_fused(const __
     // (data-dependent) cost of the cells; a persistent strided loop measured 12 % slower on cfg3
     // (taking the block ranges from the back, largest cells first, measured 1.5 % slower on cfg4)
     const u32 bid = blockIdx.x;
-    u32 cls = 0, bfirst = 0;
+    // (a warp lives for two cells of configs[3], 1400 instructions: the search over the classes is skipped when the
+    // launch holds one class only -- the prologue of a warp is 6 % of the kernel's instructions)
+    u32 cls = a.only_class, bfirst = 0;
+    if (a.only_class == (u32)CELL_CLASSES) {
+        cls = 0;
 #pragma unroll
-    for (u32 k = 0; k + 1 < (u32)CELL_CLASSES; ++k)
-        if (bid >= a.class_block_end[k]) { cls = k + 1; bfirst = a.class_block_end[k]; }
+        for (u32 k = 0; k + 1 < (u32)CELL_CLASSES; ++k)
+            if (bid >= a.class_block_end[k]) { cls = k + 1; bfirst = a.class_block_end[k]; }
+    }
     const u32 wfirst = (bid - bfirst) * CF_WARPS + warp;
     // n_steps > 1 (a run without compactions, sdm_coalescence_steps): cells never interact, so the warp takes its cells
     // through all the steps of the launch by itself -- their attributes come back from L1 / L2, and no kernel boundary
@@ -813,12 +819,16 @@ cudaError_t launch_cell_fused(sdm_ctx* ctx, int src_kind, const void* run_idx, i
     a.mapped = ctx->mapped;
     const int R = fused_words_per_lane(ctx, cc);
     u32 blocks = 0;
+    int n_used = 0;
+    a.only_class = (u32)CELL_CLASSES;
     for (int k = 0; k < CELL_CLASSES; ++k) {
         const u32 cells_per_block = (u32)CF_WARPS * 32u / (u32)class_lanes(k, R);  // CF_WARPS * 32 / G
+        const u32 before = blocks;
         a.class_count[k] = cc.count[k];
         a.class_cells[k] = cc.mixed ? ctx->ws.class_list + (size_t)k * (size_t)ctx->max_n_cell : nullptr;
         blocks += (cc.count[k] + cells_per_block - 1) / cells_per_block;
         a.class_block_end[k] = blocks;
+        if (blocks > before) { a.only_class = n_used ? (u32)CELL_CLASSES : (u32)k; ++n_used; }
     }
     if (blocks == 0) return cudaSuccess;
     LaunchScope scope(ctx, PROF_CELL_FUSED);
