@@ -14,7 +14,8 @@
 // of the fine bucket -- and writes the indices to their shuffled positions.  k_pair then pairs neighbours exactly as
 // on the GENERAL path.  Against that path's four chained radix passes (each a wave of tiles waiting on its
 // predecessors: 15 us apiece at 2^20 entries) nothing here waits on a neighbour.  Same total order (key, index) =>
-// same bits.
+// same bits.  Level 1 depends on nothing but the step number: the time loop (sdm_coalescence_steps) runs the next
+// step's k_bucket_scatter on a side stream beside this step's pair kernel (enqueue_bucket_step, sdm_api.cu).
 #include "sdm_internal.h"
 
 namespace sdm {
@@ -210,28 +211,32 @@ u32 bucket_slab_words(int64_t n_sd, int cb) {
     return (u32)cap;
 }
 
-// Enqueues the placement; `sorted` (u64[n_sd]) receives the index of every shuffled position.  The slabs live in buf_b
-// (carved with room for 2^cb x cap words), the counts in ws.bucket_count (zeroed by the caller).
-cudaError_t launch_bucket_shuffle(sdm_ctx* ctx, int64_t n_sd, int cb, const PhiloxKeys& pk, u64* sorted) {
+// Level 1 of the placement on stream `st` (ctx->stream, or the context's side stream when the time loop runs it beside
+// the previous step's pair kernel): the slabs live in buf_b (carved with room for 2^cb x cap words), the counts in
+// ws.bucket_count (zeroed by the caller on the same stream).
+cudaError_t launch_bucket_scatter(sdm_ctx* ctx, int64_t n_sd, int cb, const PhiloxKeys& pk, cudaStream_t st) {
     Workspace& ws = ctx->ws;
     const u32 n_bucket = 1u << cb;
-    u32* count = ws.bucket_count;
-    u32* words = reinterpret_cast<u32*>(ws.buf_b);
+    const u32 cap = bucket_slab_words(n_sd, cb);
+    if (bucket_fine_bits(n_sd, cb) == 0) return cudaErrorInvalidValue;  // bucket_fits() keeps such shapes away
+    LaunchScope scope(ctx, PROF_BUCKET);
+    k_bucket_scatter<<<resident_grid(ctx, n_sd), BK_BLOCK, 2 * n_bucket * 4, st>>>(
+        (u32)n_sd, cb, cap, pk, ws.bucket_count, reinterpret_cast<u32*>(ws.buf_b), ws.sticky, ctx->dbg_cell_start);
+    return cudaGetLastError();
+}
+
+// Level 2 on ctx->stream; `sorted` (u64[n_sd]) receives the index of every shuffled position.
+cudaError_t launch_bucket_sort(sdm_ctx* ctx, int64_t n_sd, int cb, const PhiloxKeys& pk, u64* sorted) {
+    Workspace& ws = ctx->ws;
+    const u32 n_bucket = 1u << cb;
     const u32 cap = bucket_slab_words(n_sd, cb);
     int idxbits = 1;
     while (((int64_t)1 << idxbits) < n_sd) ++idxbits;
     const int fb = bucket_fine_bits(n_sd, cb);
-    if (fb == 0) return cudaErrorInvalidValue;  // bucket_fits() keeps such shapes away
-    {
-        LaunchScope scope(ctx, PROF_BUCKET);
-        k_bucket_scatter<<<resident_grid(ctx, n_sd), BK_BLOCK, 2 * n_bucket * 4, ctx->stream>>>(
-            (u32)n_sd, cb, cap, pk, count, words, ws.sticky, ctx->dbg_cell_start);
-        const cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-    }
+    if (fb == 0) return cudaErrorInvalidValue;
     LaunchScope scope(ctx, PROF_BUCKET);
-    k_bucket_sort<<<n_bucket, BS_BLOCK, ((size_t)(1u << fb) + BS_CAP) * 4, ctx->stream>>>(words, count, cb, cap, fb, idxbits, pk,
-                                                                                        sorted, ws.sticky);
+    k_bucket_sort<<<n_bucket, BS_BLOCK, ((size_t)(1u << fb) + BS_CAP) * 4, ctx->stream>>>(
+        reinterpret_cast<const u32*>(ws.buf_b), ws.bucket_count, cb, cap, fb, idxbits, pk, sorted, ws.sticky);
     return cudaGetLastError();
 }
 

@@ -177,6 +177,13 @@ struct sdm_ctx {
     volatile sdm::u32* mapped;   // pinned + mapped: MAPPED_* words written by kernels (same address on the device: UVA)
     cudaEvent_t verdict_event;
     cudaEvent_t chunk_event[2];  // sdm_coalescence_steps: completion of the two chunks of steps in flight
+    // BUCKET path inside sdm_coalescence_steps: level 1 of the NEXT step's placement runs on a side stream beside this
+    // step's pair kernel (they share nothing: keys depend on the step number only)
+    cudaStream_t side;
+    cudaEvent_t side_go, side_done;  // level 2 of this step done (the counts and slabs are free) / level 1 of the next step done
+    int side_valid;                  // a placement has been started ahead ...
+    uint64_t side_step;              // ... for this step
+    int64_t side_n_sd;               // ... of this many super-droplets
     // zero-multiplicity count left in ctl[CTL_ZERO_COUNT] by the last fused step (SDM_OPT_TRACK_ZEROS)
     sdm::u32 epoch;  // tag of the current fused-path step (>= 2; see k_cell_bounds)
     sdm::u64 index_base;  // SDM_OPT_INDEX_BASE
@@ -238,7 +245,8 @@ cudaError_t launch_cell_scan(sdm_ctx* ctx, int32_t n_cell, int64_t n_sd);
 int bucket_bits(int64_t n_sd, int bits_override);
 int bucket_fine_bits(int64_t n_sd, int cb);
 cudaError_t init_bucket_path(sdm_ctx* ctx);
-cudaError_t launch_bucket_shuffle(sdm_ctx* ctx, int64_t n_sd, int cb, const PhiloxKeys& pk, u64* sorted);
+cudaError_t launch_bucket_scatter(sdm_ctx* ctx, int64_t n_sd, int cb, const PhiloxKeys& pk, cudaStream_t st);
+cudaError_t launch_bucket_sort(sdm_ctx* ctx, int64_t n_sd, int cb, const PhiloxKeys& pk, u64* sorted);
 cudaError_t launch_sort_pass(sdm_ctx* ctx, int pass, const u64* in, u64* out, int64_t n_sd,
                              const Plan& plan);
 cudaError_t launch_pair(sdm_ctx* ctx, const u64* sorted, int64_t* xi, double* v, int64_t n_sd,
