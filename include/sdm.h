@@ -157,7 +157,7 @@ int sdm_coalescence_step(sdm_ctx* ctx, int64_t* multiplicity, double* volume, co
  * once per call (see sdm_path), cell boundaries -- cell_id cannot change during the call -- are computed once, and a
  * due compaction costs nothing while no multiplicity is 0: every fused step counts the zeros it leaves behind, and
  * only a non-zero count at a due step halts the run on the device until the host has compacted.  On the cell-sorted
- * paths small inputs (n_sd <= 2^21) take up to 16 consecutive steps inside one kernel launch when no compaction is
+ * paths small inputs (n_sd <= 2^21) take up to 64 consecutive steps inside one kernel launch when no compaction is
  * due in between (a candidate pair lies inside one cell, so cells never interact), and a HYBRID run of
  * eight steps or more works on cell-grouped copies of the attributes in the workspace (gathered once, scattered back
  * before the call returns or compacts); the bits are those of the step-by-step loop.  cell_id is written

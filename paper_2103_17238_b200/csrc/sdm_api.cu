@@ -773,7 +773,7 @@ int sdm_remove_zero_multiplicity(sdm_ctx* ctx, int64_t* multiplicity, double* vo
 namespace {
 
 constexpr int64_t RUN_CHUNK = 64;  // fused steps enqueued between two looks at the halt word
-constexpr int64_t RUN_STEPS_PER_LAUNCH = 16;  // at most this many steps inside one launch of the fused kernel
+constexpr int64_t RUN_STEPS_PER_LAUNCH = 64;  // at most this many steps inside one launch of the fused kernel (= one chunk)
 // HYBRID runs at least this long keep cell-grouped copies of the attributes (interleaved configs[3]: the two moves cost
 // 670 us together, every step saves 110 us)
 constexpr int64_t RUN_RESIDENT_MIN_STEPS = 8;

@@ -698,8 +698,8 @@ def test_multi_step_entry_matches_oracle_run(dev, name, path):
 @pytest.mark.parametrize("name,compact_every", [("cfg4s", 1), ("cfg4s", 3), ("cfg3z", 2), ("cfg4s", 0), ("cfg4s", 20)])
 def test_multi_step_entry_compaction_schedules(dev, name, compact_every):
     """every step / every third step / never / every 20th; more steps than one chunk of the run loop (64) so that a
-    halt is noticed while later chunks are already enqueued.  Small inputs take up to 16 steps inside one launch of the
-    fused kernel when no compaction is due in between: 0 gives launches of 16, 20 launches of 16 + 4, 3 launches of 3."""
+    halt is noticed while later chunks are already enqueued.  Small inputs take up to 64 steps inside one launch of the
+    fused kernel when no compaction is due in between: 0 gives launches of 64, 20 launches of 20, 3 launches of 3."""
     w = W.small(name)
     _run_multi(w, dev, None, 150 if name == "cfg4s" else 9, compact_every)
 
