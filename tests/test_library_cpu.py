@@ -73,6 +73,21 @@ def test_no_cpu_fallback_without_cuda(lib):
     assert not out.value
 
 
+def test_static_entry_point_host_side_checks(lib):
+    """sdm_remove_zero_multiplicity_static validates on the host before it touches CUDA: the size limit of its fixed
+    scratch array, negative sizes and null pointers are refused with their own codes (no device needed, nothing is
+    dereferenced)."""
+    limit = lib.sdm_static_max_n_sd()
+    assert limit == 2 ** 26
+    fake = C.c_void_p(1 << 20)
+    f = lib.sdm_remove_zero_multiplicity_static
+    assert f(fake, fake, fake, limit + 1, fake, None) == -5            # SDM_ERR_STATIC_LIMIT
+    assert f(fake, fake, fake, -1, fake, None) == -1                   # SDM_ERR_INVALID_ARG
+    assert f(fake, fake, fake, 10, None, None) == -1                   # no place for the result
+    assert f(None, fake, fake, 10, fake, None) == -1
+    assert b"2^26" in lib.sdm_strerror(-5)
+
+
 def test_product_package_does_not_import_oracle():
     """The product path must not route through the oracle (nor the oracle through the product)."""
     for sub in ("paper_2103_17238_b200", "sdm_workloads"):
