@@ -747,6 +747,37 @@ def test_single_cell_time_loop_with_zeros(dev, n, path, compact_every):
     _run_multi(w, dev, None, 12, compact_every, chunks=(4, 8))      # AUTO, resumed
 
 
+@pytest.mark.parametrize("compact_every", [0, 7])
+def test_bucket_time_loop_with_the_next_placement_ahead(dev, compact_every):
+    """Inside sdm_coalescence_steps the BUCKET path starts level 1 of the NEXT step's placement on a side stream beside
+    this step's pair kernel (not across a due compaction).  60 steps of 2^19 super-droplets in one call equal the same
+    steps taken one call at a time -- which never runs anything ahead -- bit for bit, and the first three equal the
+    oracle; twice, so that a placement left over from the first run cannot leak into the second."""
+    sdm = _sdm()
+    w = W.cfg1(n_sd=1 << 19, n_steps=3)
+    kp = _gkp(w)
+    ow = w.copy()
+    n_o = oracle.run(ow.xi, ow.v, ow.cell_id, 1, w.dt, w.dV, _okp(w), w.seed, 0, 3, 0)
+    with sdm.SDMContext(w.n_sd, 1, device=dev) as ctx:
+        ctx.set_path(sdm.PATH_BUCKET)
+        for rep in range(2):
+            xi, v, cell = _to_dev(w, dev)
+            n = ctx.coalescence_steps(xi, v, cell, 1, w.dt, w.dV, kp, w.seed, 0, 3, 0)
+            assert n == n_o and ctx.last_path() == sdm.PATH_BUCKET
+            assert np.array_equal(xi[:n].cpu().numpy(), ow.xi[:n])
+            assert np.array_equal(v[:n].cpu().numpy().view(np.int64), ow.v[:n].view(np.int64))
+            n = ctx.coalescence_steps(xi, v, cell, 1, w.dt, w.dV, kp, w.seed, 3, 57, compact_every, n_sd=n)
+            xs, vs, cs = _to_dev(w, dev)
+            m = w.n_sd
+            for s in range(60):
+                ctx.coalescence_step(xs, vs, cs, 1, w.dt, w.dV, kp, w.seed, s, n_sd=m)
+                if compact_every and s >= 3 and (s - 3 + 1) % compact_every == 0:   # the second call's schedule
+                    m = ctx.remove_zero_multiplicity(xs, vs, cs, n_sd=m)
+            assert ctx.poll_error() == 0
+            assert n == m
+            assert torch.equal(xi[:n], xs[:n]) and torch.equal(v[:n].view(torch.int64), vs[:n].view(torch.int64))
+
+
 @pytest.mark.parametrize("n,path", [(5000, "box"), (30_000, "bucket")])
 def test_single_cell_paths_honour_index_base_and_the_table_kernel(dev, n, path):
     """SDM_OPT_INDEX_BASE (R34) and SDM_KERNEL_GEOMETRIC_TABLE (R39) on the single-cell paths: the same bits as the
